@@ -1,0 +1,235 @@
+"""Oracle: constraint residual h(u) and explicit sparse Jacobian J(u) per kind.
+
+TEST INFRASTRUCTURE (see oracle/__init__.py).  fp64, numpy/scipy, no blocking or fusion.
+
+Layout (time-major, x fastest).  One sample:
+    u[k][j][i],  k = 0..nt-1 (time), j = 0..ny-1, i = 0..nx-1;  unknown index (k*ny + j)*nx + i.
+Constraint rows (the lambda layout of include/snap.h):
+    local block  [nt][ny][nx] : level 0 = initial-condition rows u[0] - u0   (Eq. 10, Eq. 14)
+                                level k>=1 = one-step scheme residual between levels k-1 and k (L549, L561)
+                  (kind HEAT1D_IC_MASS has only level 0: nx rows)
+    mass block   [nt]         : dx * sum_i u[k][i] - M0,  M0 = dx * sum_i u0[i]   (L573-575; kinds 0 and 4)
+The paper orders IC, mass, then flux rows (L374, L499); the order of rows does not change
+the projection, only the order of the multipliers.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import scipy.sparse as sp
+
+HEAT1D_IC_MASS = 0
+BURGERS1D_LF = 1
+FISHER1D_IE = 2
+ALLENCAHN2D_IE = 3
+BURGERS1D_LF_MASS = 4
+
+_HAS_MASS = (HEAT1D_IC_MASS, BURGERS1D_LF_MASS)
+
+
+def num_rows(kind: int, nx: int, ny: int, nt: int) -> int:
+    if kind == HEAT1D_IC_MASS:
+        return nx + nt
+    n = nx * ny * nt
+    return n + nt if kind == BURGERS1D_LF_MASS else n
+
+
+def row_slices(kind: int, nx: int, ny: int, nt: int):
+    """{'ic': slice, 'pde': slice, 'mass': slice} into the row vector (empty slices where absent)."""
+    lvl = nx * ny
+    if kind == HEAT1D_IC_MASS:
+        return {"ic": slice(0, nx), "pde": slice(nx, nx), "mass": slice(nx, nx + nt)}
+    n = lvl * nt
+    mass = slice(n, n + nt) if kind == BURGERS1D_LF_MASS else slice(n, n)
+    return {"ic": slice(0, lvl), "pde": slice(lvl, n), "mass": mass}
+
+
+def full_rank_rows(kind: int, nx: int, ny: int, nt: int) -> np.ndarray:
+    """Boolean mask of a maximal linearly independent row subset.
+
+    kind 0: the t=0 mass row is implied by the nx IC rows (the paper omits it, L493).
+    kind 4: every mass row is implied by IC + conservative periodic finite-volume rows
+            (sum_i h^P_{k,i} dx = mass_{k+1} - mass_k identically).
+    tests/test_oracle_pins.py verifies both statements by numerical rank on tiny grids."""
+    m = num_rows(kind, nx, ny, nt)
+    keep = np.ones(m, dtype=bool)
+    s = row_slices(kind, nx, ny, nt)["mass"]
+    if kind == HEAT1D_IC_MASS:
+        keep[s.start] = False
+    elif kind == BURGERS1D_LF_MASS:
+        keep[s] = False
+    return keep
+
+
+# ------------------------------------------------------------------------------------------
+# residual
+# ------------------------------------------------------------------------------------------
+
+def _lf_flux(a, b, alpha):
+    """Lax-Friedrichs numerical flux for f(u) = u^2/2 through the interface between
+    a = u_i and b = u_{i+1} (smooth stand-in for the Godunov flux of L555)."""
+    return 0.5 * (0.5 * a * a + 0.5 * b * b) - 0.5 * alpha * (b - a)
+
+
+def _mass_rows(u, u0, dx):
+    nt = u.shape[0]
+    M0 = dx * math.fsum(u0.ravel().tolist())
+    return np.array([dx * math.fsum(u[k].ravel().tolist()) - M0 for k in range(nt)])
+
+
+def residual(kind: int, u: np.ndarray, u0: np.ndarray, p: dict) -> np.ndarray:
+    """h(u) as one vector in the row layout above.  u: [nt, ny, nx], u0: [ny, nx]."""
+    u = np.asarray(u, dtype=np.float64)
+    u0 = np.asarray(u0, dtype=np.float64)
+    nt, ny, nx = u.shape
+    dx, dt = p["dx"], p["dt"]
+    ic = (u[0] - u0).ravel()
+    if kind == HEAT1D_IC_MASS:
+        return np.concatenate([ic, _mass_rows(u, u0, dx)])
+
+    loc = np.empty_like(u)
+    loc[0] = u[0] - u0
+    if kind in (BURGERS1D_LF, BURGERS1D_LF_MASS):
+        s = dt / dx
+        c = p["nu"] * dt / dx ** 2
+        al = p["alpha"]
+        for k in range(nt - 1):
+            v = u[k, 0]
+            vp = np.roll(v, -1)       # u_{i+1}
+            vm = np.roll(v, 1)        # u_{i-1}
+            F_r = _lf_flux(v, vp, al)     # F_{i+1/2}
+            F_l = _lf_flux(vm, v, al)     # F_{i-1/2}
+            # R^(k) = u^{k+1} - [u^k - dt/dx (F_{i+1/2} - F_{i-1/2})]  (L561) with explicit viscosity (R8)
+            loc[k + 1, 0] = u[k + 1, 0] - v + s * (F_r - F_l) - c * (vp - 2.0 * v + vm)
+    elif kind == FISHER1D_IE:
+        D, rho = p["D"], p["rho"]
+        for k in range(nt - 1):
+            w = u[k + 1, 0]
+            lap = np.empty(nx)
+            lap[1:-1] = (w[2:] - 2.0 * w[1:-1] + w[:-2]) / dx ** 2
+            lap[0] = (w[1] - w[0]) / dx ** 2            # ghost-cell Neumann (R10, L577-587)
+            lap[-1] = (w[-2] - w[-1]) / dx ** 2
+            loc[k + 1, 0] = w - u[k, 0] - dt * (D * lap + rho * w * (1.0 - w))
+    elif kind == ALLENCAHN2D_IE:
+        dy, eps = p["dy"], p["eps"]
+        for k in range(nt - 1):
+            w = u[k + 1]
+            lap = ((np.roll(w, -1, 1) - 2.0 * w + np.roll(w, 1, 1)) / dx ** 2
+                   + (np.roll(w, -1, 0) - 2.0 * w + np.roll(w, 1, 0)) / dy ** 2)
+            loc[k + 1] = w - u[k] - dt * (eps ** 2 * lap - w ** 3 + w)
+    else:
+        raise ValueError(f"unknown kind {kind}")
+    if kind == BURGERS1D_LF_MASS:
+        return np.concatenate([loc.ravel(), _mass_rows(u, u0, dx)])
+    return loc.ravel()
+
+
+def residual_norms(kind: int, u: np.ndarray, u0: np.ndarray, p: dict) -> np.ndarray:
+    """[ ||h||_inf, ||h_IC||_2, ||h_PDE||_2, ||h_mass||_2 ]  — the per-type Euclidean norms
+    are the per-sample terms of the paper's constraint-error metric (Eq. 27)."""
+    nt, ny, nx = np.asarray(u).shape
+    h = residual(kind, u, u0, p)
+    sl = row_slices(kind, nx, ny, nt)
+    return np.array([np.abs(h).max() if h.size else 0.0,
+                     np.linalg.norm(h[sl["ic"]]), np.linalg.norm(h[sl["pde"]]), np.linalg.norm(h[sl["mass"]])])
+
+
+# ------------------------------------------------------------------------------------------
+# Jacobian (explicit sparse matrix; fixed pattern)
+# ------------------------------------------------------------------------------------------
+
+def jacobian(kind: int, u: np.ndarray, p: dict) -> sp.csr_matrix:
+    """J(u) = dh/du as an explicit CSR matrix, rows in the layout above."""
+    u = np.asarray(u, dtype=np.float64)
+    nt, ny, nx = u.shape
+    lvl = nx * ny
+    n = lvl * nt
+    m = num_rows(kind, nx, ny, nt)
+    dx, dt = p["dx"], p["dt"]
+    rows, cols, vals = [], [], []
+
+    def add(r, c, v):
+        rows.append(np.asarray(r).ravel())
+        cols.append(np.asarray(c).ravel())
+        vals.append(np.broadcast_to(np.asarray(v, dtype=np.float64), np.asarray(r).shape).ravel())
+
+    cell = np.arange(lvl)
+    add(cell, cell, 1.0)                                 # IC rows: d(u[0]-u0)/du[0] = I
+
+    if kind in (BURGERS1D_LF, BURGERS1D_LF_MASS):
+        s = dt / dx
+        c = p["nu"] * dt / dx ** 2
+        al = p["alpha"]
+        i = np.arange(nx)
+        ip = (i + 1) % nx
+        im = (i - 1) % nx
+        for k in range(nt - 1):
+            v = u[k, 0]
+            r = (k + 1) * nx + i
+            # dF_{i+1/2}/du_i = u_i/2 + alpha/2 ; dF_{i+1/2}/du_{i+1} = u_{i+1}/2 - alpha/2
+            dFr_di, dFr_dip = 0.5 * v[i] + 0.5 * al, 0.5 * v[ip] - 0.5 * al
+            dFl_dim, dFl_di = 0.5 * v[im] + 0.5 * al, 0.5 * v[i] - 0.5 * al
+            add(r, (k + 1) * nx + i, 1.0)
+            add(r, k * nx + i, -1.0 + s * (dFr_di - dFl_di) + 2.0 * c)
+            add(r, k * nx + ip, s * dFr_dip - c)
+            add(r, k * nx + im, -s * dFl_dim - c)
+    elif kind == FISHER1D_IE:
+        D, rho = p["D"], p["rho"]
+        a = dt * D / dx ** 2
+        i = np.arange(nx)
+        for k in range(nt - 1):
+            w = u[k + 1, 0]
+            r = (k + 1) * nx + i
+            nnb = np.full(nx, 2.0)
+            nnb[0] = 1.0
+            nnb[-1] = 1.0                                  # number of neighbours (Neumann ends)
+            add(r, k * nx + i, -1.0)
+            add(r, (k + 1) * nx + i, 1.0 + a * nnb - dt * rho * (1.0 - 2.0 * w))
+            add(r[1:], (k + 1) * nx + i[:-1], -a)
+            add(r[:-1], (k + 1) * nx + i[1:], -a)
+    elif kind == ALLENCAHN2D_IE:
+        dy, eps = p["dy"], p["eps"]
+        ax = dt * eps ** 2 / dx ** 2
+        ay = dt * eps ** 2 / dy ** 2
+        jj, ii = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+        here = (jj * nx + ii).ravel()
+        xp = (jj * nx + (ii + 1) % nx).ravel()
+        xm = (jj * nx + (ii - 1) % nx).ravel()
+        yp = (((jj + 1) % ny) * nx + ii).ravel()
+        ym = (((jj - 1) % ny) * nx + ii).ravel()
+        for k in range(nt - 1):
+            w = u[k + 1].ravel()
+            r = (k + 1) * lvl + here
+            base = (k + 1) * lvl
+            add(r, k * lvl + here, -1.0)
+            add(r, base + here, 1.0 + 2.0 * ax + 2.0 * ay + dt * (3.0 * w * w - 1.0))
+            add(r, base + xp, -ax)
+            add(r, base + xm, -ax)
+            add(r, base + yp, -ay)
+            add(r, base + ym, -ay)
+    elif kind != HEAT1D_IC_MASS:
+        raise ValueError(f"unknown kind {kind}")
+
+    if kind in _HAS_MASS:
+        m0 = nx if kind == HEAT1D_IC_MASS else n
+        i = np.arange(nx)
+        for k in range(nt):
+            add(np.full(nx, m0 + k), k * nx + i, dx)
+
+    J = sp.coo_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))), shape=(m, n))
+    return J.tocsr()        # duplicates (tiny periodic grids where i+1 == i-1) are summed
+
+
+def paper_example_jacobian(nx: int, nt: int) -> np.ndarray:
+    """The paper's own worked example (Appendix C, Eq. 26): IC rows first, then for
+    k = 2..nt the left-Riemann mass row  sum_{i<nx} u_i^(k) - sum_{i<nx} u_i^(1)  (no dx weight,
+    last node excluded, first time step omitted).  Dense (nx + nt - 1) x (nx nt)."""
+    J = np.zeros((nx + nt - 1, nx * nt))
+    for i in range(nx):
+        J[i, i] = 1.0
+    for k in range(1, nt):
+        for i in range(nx - 1):
+            J[nx + k - 1, i] = -1.0
+            J[nx + k - 1, k * nx + i] = 1.0
+    return J

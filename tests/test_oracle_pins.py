@@ -1,0 +1,397 @@
+"""Pins for the CPU oracle: the oracle is checked against things other
+than itself — the paper's printed example, closed forms, textbook routines, brute force on
+tiny grids and invariants — before any CUDA result is compared with it.  CPU only."""
+import math
+import os
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import scipy.sparse.linalg as spla
+
+import oracle as O
+import workloads as W
+from oracle import constraints as C
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _wl(cfg, **kw):
+    return W.make_workload(cfg, **kw)
+
+
+def _np(t):
+    return t.numpy()
+
+
+TINY = {1: dict(batch=2, nx=5, nt=4), 2: dict(batch=2, nx=6, nt=5), 3: dict(batch=2, nx=6, nt=5),
+        4: dict(batch=2, nx=4, ny=4, nt=4), 5: dict(batch=2, nx=6, nt=5)}
+SMALL = {1: dict(batch=3, nx=20, nt=12), 2: dict(batch=3, nx=24, nt=20), 3: dict(batch=3, nx=24, nt=20),
+         4: dict(batch=2, nx=12, ny=10, nt=6), 5: dict(batch=3, nx=24, nt=20)}
+
+
+# ---------------------------------------------------------------------------------- P8
+def test_p8_paper_worked_jacobian_eq26():
+    """PAPER.md Eq. 26 (L503): the only numeric example the paper prints."""
+    gold = np.loadtxt(os.path.join(GOLDEN, "eq26_jacobian.txt"))
+    assert gold.shape == (5, 9)
+    np.testing.assert_array_equal(O.paper_example_jacobian(3, 3), gold)
+    # "rows containing a sequence of Nx-1 nonzero entries followed by a zero" (L508)
+    J = O.paper_example_jacobian(7, 4)
+    for k in range(1, 4):
+        row = J[7 + k - 1, k * 7:(k + 1) * 7]
+        np.testing.assert_array_equal(row, [1] * 6 + [0])
+
+
+def test_row_layout_matches_paper_flattening():
+    """Time-major / x-fastest flattening (L71, L497) and "IC rows first" (L499): the oracle's
+    IC block is the identity on the first nx*ny unknowns, and its mass rows differ from the
+    paper's variant only by R7 (all nx nodes, weight dx, constant target)."""
+    wl = _wl(1, **TINY[1])
+    J = O.jacobian(wl.kind, _np(wl.u_hat[0]), wl.params).toarray()
+    nx, nt = wl.nx, wl.nt
+    np.testing.assert_array_equal(J[:nx, :nx], np.eye(nx))
+    assert np.all(J[:nx, nx:] == 0)
+    for k in range(nt):
+        expect = np.zeros(nx * nt)
+        expect[k * nx:(k + 1) * nx] = wl.params["dx"]
+        np.testing.assert_allclose(J[nx + k], expect, rtol=0, atol=0)
+
+
+# ---------------------------------------------------------------------------------- P5
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_p5_jacobian_vs_central_differences(cfg):
+    wl = _wl(cfg, **TINY[cfg])
+    u = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    J = O.jacobian(wl.kind, u, wl.params).toarray()
+    n = u.size
+    eps = 1e-6
+    Jfd = np.empty_like(J)
+    for c in range(n):
+        e = np.zeros(n)
+        e[c] = eps
+        hp = O.residual(wl.kind, (u.ravel() + e).reshape(u.shape), u0, wl.params)
+        hm = O.residual(wl.kind, (u.ravel() - e).reshape(u.shape), u0, wl.params)
+        Jfd[:, c] = (hp - hm) / (2 * eps)
+    assert J.shape == (wl.m, n)
+    assert np.abs(J - Jfd).max() < 1e-8
+
+
+def test_residual_matches_handwritten_scalar_formula_burgers():
+    """Brute force: the Burgers-LF residual written out cell by cell with Python scalars
+    (SURVEY.md §8(c) expanded form) equals the vectorised flux-difference form."""
+    wl = _wl(2, **TINY[2])
+    u = _np(wl.u_hat[1])[:, 0]
+    u0 = _np(wl.cdata[1])[0]
+    p = wl.params
+    nt, nx = u.shape
+    s, c, al = p["dt"] / p["dx"], p["nu"] * p["dt"] / p["dx"] ** 2, p["alpha"]
+    h = O.residual(wl.kind, u[:, None, :], u0[None], p).reshape(nt, nx)
+    for i in range(nx):
+        assert h[0, i] == u[0, i] - u0[i]
+    for k in range(nt - 1):
+        for i in range(nx):
+            a, b, cc = u[k, (i - 1) % nx], u[k, i], u[k, (i + 1) % nx]
+            ref = (u[k + 1, i] - b + s * (0.25 * (cc * cc - a * a) - 0.5 * al * (cc - 2 * b + a))
+                   - c * (cc - 2 * b + a))
+            assert abs(h[k + 1, i] - ref) < 1e-15
+
+
+def test_residual_scalar_formula_fisher_and_allencahn():
+    wl = _wl(3, **TINY[3])
+    u = _np(wl.u_hat[0])[:, 0]
+    p = wl.params
+    nt, nx = u.shape
+    h = O.residual(wl.kind, u[:, None, :], _np(wl.cdata[0]), p).reshape(nt, nx)
+    for k in range(nt - 1):
+        for i in range(nx):
+            w = u[k + 1]
+            left = w[i - 1] if i > 0 else w[i]            # mirror ghost (L577-587)
+            right = w[i + 1] if i < nx - 1 else w[i]
+            lap = (left - 2 * w[i] + right) / p["dx"] ** 2
+            ref = w[i] - u[k, i] - p["dt"] * (p["D"] * lap + p["rho"] * w[i] * (1 - w[i]))
+            assert abs(h[k + 1, i] - ref) < 1e-15
+    wl = _wl(4, **TINY[4])
+    u = _np(wl.u_hat[0])
+    p = wl.params
+    nt, ny, nx = u.shape
+    h = O.residual(wl.kind, u, _np(wl.cdata[0]), p).reshape(nt, ny, nx)
+    for k in range(nt - 1):
+        w = u[k + 1]
+        for j in range(ny):
+            for i in range(nx):
+                lap = ((w[j, (i + 1) % nx] - 2 * w[j, i] + w[j, (i - 1) % nx]) / p["dx"] ** 2
+                       + (w[(j + 1) % ny, i] - 2 * w[j, i] + w[(j - 1) % ny, i]) / p["dy"] ** 2)
+                ref = w[j, i] - u[k, j, i] - p["dt"] * (p["eps"] ** 2 * lap - w[j, i] ** 3 + w[j, i])
+                assert abs(h[k + 1, j, i] - ref) < 1e-14
+
+
+# ---------------------------------------------------------------------------------- P1
+def _heat_closed_form(u_hat, u0, dx):
+    """SURVEY.md P1, derived by hand from u - J^T (J J^T)^+ (J u - b)."""
+    nt, nx = u_hat.shape
+    M0 = dx * u0.sum()
+    u = u_hat.copy()
+    u[0] = u0
+    lam_mass = np.zeros(nt)
+    for k in range(1, nt):
+        u[k] = u_hat[k] - u_hat[k].mean() + M0 / (nx * dx)
+        lam_mass[k] = (dx * u_hat[k].sum() - M0) / (nx * dx * dx)
+    d = u_hat[0] - u0
+    lam_mass[0] = dx * d.sum() / (1.0 + nx * dx * dx)
+    lam_ic = d - dx * lam_mass[0]
+    return u, np.concatenate([lam_ic, lam_mass])
+
+
+@pytest.mark.parametrize("kw", [TINY[1], SMALL[1], dict(batch=4)])
+def test_p1_heat_closed_form_and_pinv(kw):
+    wl = _wl(1, **kw)
+    for b in range(wl.batch):
+        uh = _np(wl.u_hat[b])
+        u0 = _np(wl.cdata[b])
+        out = O.project(wl.kind, uh, u0, wl.params)
+        u_ref, lam_ref = _heat_closed_form(uh[:, 0], u0[0], wl.params["dx"])
+        assert out["status"] == 0 and out["steps"] == 1          # "a single matrix solve" (L29)
+        np.testing.assert_allclose(out["u"][:, 0], u_ref, rtol=0, atol=2e-14)
+        np.testing.assert_allclose(out["lam"], lam_ref, rtol=0, atol=1e-11 * max(1, np.abs(lam_ref).max()))
+    # the same through the dense pseudo-inverse:  u - J^T (J J^T)^+ (J u - b)
+    uh = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    J = O.jacobian(wl.kind, uh, wl.params).toarray()
+    h = O.residual(wl.kind, uh, u0, wl.params)            # affine: h(u) = J u - b
+    lam = np.linalg.pinv(J @ J.T, rcond=1e-12, hermitian=True) @ h
+    out = O.project(wl.kind, uh, u0, wl.params)
+    np.testing.assert_allclose(out["u"].ravel(), uh.ravel() - J.T @ lam, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(out["lam"], lam, rtol=0, atol=1e-10 * max(1, np.abs(lam).max()))
+
+
+def test_p1_heat_displacement_orthogonal_to_null_space():
+    """(u* - u_hat) lies in range(J^T): orthogonal to random null vectors of J (P4)."""
+    wl = _wl(1, **SMALL[1])
+    uh = _np(wl.u_hat[0])
+    out = O.project(wl.kind, uh, _np(wl.cdata[0]), wl.params)
+    J = O.jacobian(wl.kind, uh, wl.params).toarray()
+    rng = np.random.default_rng(0)
+    Z = rng.standard_normal((J.shape[1], 5))
+    Z -= J.T @ np.linalg.lstsq(J.T, Z, rcond=None)[0]      # project onto null(J)
+    assert np.abs(J @ Z).max() < 1e-12
+    assert np.abs(Z.T @ (out["u"] - uh).ravel()).max() < 1e-12
+
+
+# ---------------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_p2_forward_solve_identity(cfg):
+    """Square nonsingular J_loc (R5): the feasible set is the scheme's own forward solution from
+    the IC, whatever the noise; lambda* is one adjoint solve J(u*)^T lam = u_hat - u*.  The
+    forward solution comes from workloads/ (update form, textbook time stepping), the adjoint
+    solve from a generic sparse LU (SuperLU) — neither touches the oracle's KKT code."""
+    kw = dict(SMALL[cfg])
+    wl = _wl(cfg, **kw)
+    p = dict(wl.params, lambda_mode=1)
+    for b in range(wl.batch):
+        uh = _np(wl.u_hat[b])
+        out = O.project(wl.kind, uh, _np(wl.cdata[b]), p)
+        ut = _np(wl.u_true[b])
+        assert out["status"] == 0
+        assert np.abs(out["u"] - ut).max() < 5e-12
+        J = O.jacobian(wl.kind, ut, p)
+        keep = O.full_rank_rows(wl.kind, wl.nx, wl.ny, wl.nt)
+        lam_sq = spla.spsolve(sp.csc_matrix(J[keep].T), (uh - ut).ravel())
+        tol = (2e-9 if cfg == 4 else 1e-10) * max(1.0, np.abs(lam_sq).max())
+        np.testing.assert_allclose(out["lam"][keep], lam_sq, rtol=0, atol=tol)
+        assert np.all(out["lam"][~keep] == 0)
+
+
+# ---------------------------------------------------------------------------------- P3
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_p3_dense_kkt_lu_on_tiny_grids(cfg):
+    """nx = nt = 4..6: the banded-Cholesky / CG Schur routes take the same Gauss-Newton path as a
+    dense LU of the full (n+m)x(n+m) KKT matrix [I J^T; J 0] (north_star), and one step from the
+    same point agrees to 1e-12."""
+    wl = _wl(cfg, **TINY[cfg])
+    p = dict(wl.params, lambda_mode=1)
+    uh = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    a = O.project(wl.kind, uh, u0, p, backend="dense")
+    b = O.project(wl.kind, uh, u0, p, backend="auto")
+    assert a["status"] == 0 and b["status"] == 0
+    np.testing.assert_allclose(a["u"], b["u"], rtol=0, atol=1e-12)
+    np.testing.assert_allclose(a["lam"], b["lam"], rtol=0, atol=1e-11 * max(1, np.abs(a["lam"]).max()))
+    # one explicit step, written out here: dense KKT solve vs Schur complement by hand
+    keep = O.full_rank_rows(wl.kind, wl.nx, wl.ny, wl.nt)
+    u = uh + 0.01 * np.cos(np.arange(uh.size)).reshape(uh.shape)
+    J = O.jacobian(wl.kind, u, p)[keep].toarray()
+    h = O.residual(wl.kind, u, u0, p)[keep]
+    w = (u - uh).ravel()
+    d, lam = O.solve_kkt_dense_lu(J, w, h)
+    lam_s = np.linalg.solve(J @ J.T, h - J @ w)
+    np.testing.assert_allclose(lam, lam_s, rtol=0, atol=1e-11 * max(1, np.abs(lam).max()))
+    np.testing.assert_allclose(u.ravel() + d, uh.ravel() - J.T @ lam_s, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("cfg", [1, 5])
+def test_p3_redundant_rows_min_norm_equals_pinv(cfg):
+    """R6: rank deficiency as claimed, and the returned multiplier equals (J J^T)^+ r."""
+    wl = _wl(cfg, **TINY[cfg])
+    uh = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    keep = O.full_rank_rows(wl.kind, wl.nx, wl.ny, wl.nt)
+    J = O.jacobian(wl.kind, uh, wl.params).toarray()
+    assert np.linalg.matrix_rank(J) == keep.sum() == np.linalg.matrix_rank(J[keep])
+    out = O.project(wl.kind, uh, u0, wl.params)                       # lambda_mode 0 = min-norm
+    Js = O.jacobian(wl.kind, out["u"], wl.params)
+    h = O.residual(wl.kind, out["u"], u0, wl.params)
+    r = h - Js @ (out["u"] - uh).ravel()
+    lam_pinv = O.solve_schur_pinv(Js, r)
+    np.testing.assert_allclose(out["lam"], lam_pinv, rtol=0, atol=1e-10 * max(1, np.abs(lam_pinv).max()))
+    basic = O.project(wl.kind, uh, u0, dict(wl.params, lambda_mode=1))
+    np.testing.assert_allclose(Js.T @ basic["lam"], Js.T @ out["lam"], rtol=0, atol=1e-11)
+    assert np.linalg.norm(out["lam"]) <= np.linalg.norm(basic["lam"]) + 1e-12
+
+
+def test_min_norm_banded_route_equals_dense_route_and_cg_from_zero():
+    """The two back ends of min_norm_multiplier agree, and both equal what plain CG started from
+    zero converges to on the singular bordered J J^T (the textbook characterisation)."""
+    wl = _wl(5, batch=1, nx=16, nt=12)
+    uh = _np(wl.u_hat[0])
+    J = O.jacobian(wl.kind, uh, wl.params)
+    rng = np.random.default_rng(3)
+    lam_any = rng.standard_normal(J.shape[0])
+    dense = O.min_norm_multiplier(J, lam_any)
+    Nmat = (J.T @ J).tocsr()
+    z = O.solve_schur_banded_cholesky(Nmat, J.T @ lam_any)
+    np.testing.assert_allclose(J @ z, dense, rtol=0, atol=1e-10 * np.abs(dense).max())
+    S = (J @ J.T).tocsr()
+    lam_cg, _ = O.solve_schur_cg(S, S @ lam_any, rtol=1e-14, maxiter=50000)
+    np.testing.assert_allclose(lam_cg, dense, rtol=0, atol=1e-8 * np.abs(dense).max())
+
+
+# ---------------------------------------------------------------------------------- P6
+def test_p6_factor_identity_and_null_space_gram():
+    """Explicit Burgers: J_loc is unit lower triangular in time-major order, so chol(J J^T) = J
+    (zero fill).  With mass rows: border Schur complement = 0 and the analytic left null basis
+    N_k = e_mass,k - dx (1 on IC rows) - dx sum_{j<k} (1 on PDE rows of step j) has
+    N J = 0 and N N^T = I + nx dx^2 (1 1^T + min(k,l))."""
+    wl = _wl(5, **TINY[5])
+    nx, nt, dx = wl.nx, wl.nt, wl.params["dx"]
+    u = _np(wl.u_hat[0])
+    J = O.jacobian(wl.kind, u, wl.params).toarray()
+    n = nx * nt
+    Jl, Jb = J[:n], J[n:]
+    assert np.abs(np.triu(Jl, 1)).max() == 0 and np.all(np.diag(Jl) == 1)
+    assert abs(np.linalg.det(Jl) - 1) < 1e-12
+    np.testing.assert_allclose(np.linalg.cholesky(Jl @ Jl.T), Jl, rtol=0, atol=1e-14)
+    A, Cm, Dm = Jl @ Jl.T, Jb @ Jl.T, Jb @ Jb.T
+    assert np.abs(Dm - Cm @ np.linalg.solve(A, Cm.T)).max() < 1e-13
+    N = np.zeros((nt, n + nt))
+    for k in range(nt):
+        N[k, n + k] = 1.0
+        N[k, :nx * (k + 1)] = -dx
+    assert np.abs(N @ J).max() < 1e-13
+    kk = np.arange(nt)
+    G = np.eye(nt) + nx * dx * dx * (1.0 + np.minimum.outer(kk, kk))
+    np.testing.assert_allclose(N @ N.T, G, rtol=0, atol=1e-13)
+    # N h(u) = 0 identically in u (the rows are *consistently* redundant)
+    h = O.residual(wl.kind, u, _np(wl.cdata[0]), wl.params)
+    assert np.abs(N @ h).max() < 1e-13
+    out = O.project(wl.kind, u, _np(wl.cdata[0]), wl.params)
+    assert np.abs(N @ out["lam"]).max() < 1e-10 * max(1, np.abs(out["lam"]).max())
+
+
+# ---------------------------------------------------------------------------------- P4
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_p4_kkt_invariants(cfg):
+    wl = _wl(cfg, **SMALL[cfg])
+    for b in range(wl.batch):
+        uh = _np(wl.u_hat[b])
+        u0 = _np(wl.cdata[b])
+        out = O.project(wl.kind, uh, u0, wl.params)
+        assert out["status"] == 0
+        h = O.residual(wl.kind, out["u"], u0, wl.params)
+        assert np.abs(h).max() < 1e-12                            # feasibility (L444)
+        J = O.jacobian(wl.kind, out["u"], wl.params)
+        stat = (out["u"] - uh).ravel() + J.T @ out["lam"]         # grad f + J^T lam = 0 (L443)
+        assert np.abs(stat).max() < 1e-11 * max(1.0, np.abs(out["lam"]).max())
+
+
+# ---------------------------------------------------------------------------------- P7
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_p7_feasible_input_and_idempotence(cfg):
+    wl = _wl(cfg, **SMALL[cfg])
+    ut = _np(wl.u_true[0])
+    u0 = _np(wl.cdata[0])
+    out = O.project(wl.kind, ut, u0, wl.params)
+    assert out["steps"] == 0 and out["status"] == 0
+    np.testing.assert_array_equal(out["u"], ut)                   # bit-exact
+    assert np.abs(out["lam"]).max() < 1e-12
+    first = O.project(wl.kind, _np(wl.u_hat[0]), u0, wl.params)
+    again = O.project(wl.kind, first["u"], u0, wl.params)
+    assert again["steps"] == 0
+    np.testing.assert_array_equal(again["u"], first["u"])
+
+
+@pytest.mark.parametrize("cfg", [2, 4, 5])
+def test_p7_periodic_shift_equivariance(cfg):
+    wl = _wl(cfg, **SMALL[cfg])
+    uh = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    a = O.project(wl.kind, uh, u0, wl.params)
+    sh = 5
+    b = O.project(wl.kind, np.roll(uh, sh, -1), np.roll(u0, sh, -1), wl.params)
+    np.testing.assert_allclose(np.roll(a["u"], sh, -1), b["u"], rtol=0, atol=1e-12)
+    loc = wl.n
+    la = a["lam"][:loc].reshape(uh.shape)
+    lb = b["lam"][:loc].reshape(uh.shape)
+    np.testing.assert_allclose(np.roll(la, sh, -1), lb, rtol=0, atol=1e-9 * max(1, np.abs(la).max()))
+
+
+def test_p7_batch_independence():
+    """Block-diagonal batch structure (L106): a sample alone == inside any batch / permutation."""
+    wl = _wl(2, **SMALL[2])
+    uh = _np(wl.u_hat)
+    cd = _np(wl.cdata)
+    full = O.project_batch(wl.kind, uh, cd, wl.params)
+    perm = [2, 0, 1]
+    pb = O.project_batch(wl.kind, uh[perm], cd[perm], wl.params, workers=2)
+    for new, old in enumerate(perm):
+        np.testing.assert_array_equal(pb["u"][new], full["u"][old])
+        np.testing.assert_array_equal(pb["lam"][new], full["lam"][old])
+    one = O.project(wl.kind, uh[1], cd[1], wl.params)
+    np.testing.assert_array_equal(one["u"], full["u"][1])
+
+
+# ---------------------------------------------------------------------------------- R2 / R17
+def test_line_search_backtracks_and_still_reaches_the_same_point():
+    """The Armijo loop is dormant on the benchmark inputs (R17); force it with c1 close to 1 and
+    large noise, and check halving happens and the limit point does not move."""
+    wl = _wl(2, batch=1, nx=24, nt=20, noise=1.0)
+    uh = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    ref = O.project(wl.kind, uh, u0, wl.params)
+    forced = O.project(wl.kind, uh, u0, dict(wl.params, ls_c1=0.99))
+    assert ref["status"] == 0 and forced["status"] == 0
+    assert ref["backtracks"] == 0 and forced["backtracks"] > 0
+    np.testing.assert_allclose(forced["u"], ref["u"], rtol=0, atol=1e-11)
+
+
+def test_nonfinite_direction_reports_status_and_leaves_input(recwarn):
+    """R16: far outside the workloads the linearised propagator overflows; status -3, u* = u_hat."""
+    wl = _wl(2, batch=1, nx=16, nt=200)
+    uh = _np(wl.u_hat[0]) * 1e155
+    out = O.project(wl.kind, uh, _np(wl.cdata[0]), wl.params)
+    assert out["status"] == -3 and out["iters"] == -3
+    np.testing.assert_array_equal(out["u"], uh)
+
+
+def test_residual_norms_per_type():
+    wl = _wl(5, **SMALL[5])
+    u = _np(wl.u_hat[0])
+    u0 = _np(wl.cdata[0])
+    nrm = O.residual_norms(wl.kind, u, u0, wl.params)
+    h = O.residual(wl.kind, u, u0, wl.params)
+    n, nx = wl.n, wl.nx
+    assert nrm[0] == np.abs(h).max()
+    assert math.isclose(nrm[1], np.linalg.norm(h[:nx]), rel_tol=1e-15)
+    assert math.isclose(nrm[2], np.linalg.norm(h[nx:n]), rel_tol=1e-15)
+    assert math.isclose(nrm[3], np.linalg.norm(h[n:]), rel_tol=1e-15)

@@ -1,0 +1,149 @@
+/*
+ * snap.h — C ABI of the B200-native batched constraint projection (SNAP-FM hot path,
+ * arxiv/paper_2607_00095).
+ *
+ *     u* = argmin_u 1/2 ||u - u_hat||^2   s.t.  h(u) = 0        (Eq. 2; Eq. 4)
+ *
+ * solved per sample by Gauss-Newton / Newton-KKT iterations (Eq. 5, Eq. 24 L468 with
+ * W = I): each iteration evaluates the discretised-PDE residual h and its stencil-local Jacobian J
+ * (PAPER.md L98-104), solves the Schur form (J J^T) lam+ = h - J (u - u_hat) of the KKT system
+ * (block diagonal across samples) and takes u <- u + alpha ((u_hat - J^T lam+) - u)
+ * with an l1-merit Armijo line search, until ||h||_inf < tol.  Everything is IEEE fp64.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  Every array argument named below "dev" is a DEVICE pointer owned by
+ *     the caller (e.g. a torch tensor's data_ptr()); "host" pointers are host memory.  The library owns
+ *     only the opaque problem handle and never allocates device memory in snap_project/snap_residual/
+ *     snap_schur_apply (the caller supplies `workspace`); snap_project_host allocates a private
+ *     staging area on first use and frees it in snap_problem_destroy.
+ *   - Layout of a state (time-major, x fastest), dense, fp64:
+ *         u[b][k][j][i]   b < batch, k < nt (time level), j < ny, i < nx      n = nt*ny*nx per sample
+ *   - Layout of constraint rows / multipliers, per sample, m = snap_num_rows(p):
+ *         local block [nt][ny][nx]: level 0 = initial-condition rows u[0] - u0 (Eq. 10, Eq. 14);
+ *                                   level k >= 1 = one-step scheme residual between levels k-1 and k
+ *                                   (PAPER.md L549, L561).  Kind HEAT1D_IC_MASS has level 0 only (nx rows).
+ *         mass block  [nt]        : dx * sum_i u[k][i] - M0,  M0 = dx * sum_i u0[i],
+ *                                   kinds HEAT1D_IC_MASS and BURGERS1D_LF_MASS only.
+ *     (The paper lists IC, mass, flux rows in that order, L374/L499; row order only permutes lam.)
+ *   - Asynchrony: device entry points only enqueue work on `stream` and return; per-sample outcome is in
+ *     device memory (`iters`).  They never synchronise the host.
+ *   - Errors: return value 0 = SNAP_OK, negative = error (see enum).  Non-convergence of an individual
+ *     sample is NOT an error return: it is reported in iters[b] as a negative status.
+ *   - Thread safety: distinct handles may be used concurrently; one handle must not be used from two
+ *     host threads at once with the same workspace.
+ */
+#ifndef SNAP_H_
+#define SNAP_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct snap_problem snap_problem; /* opaque, host side, owned by the library */
+typedef void* snap_stream;                /* a cudaStream_t (NULL = legacy default stream) */
+
+/* Constraint families (BASELINE.json configs 1..5). */
+enum {
+  SNAP_HEAT1D_IC_MASS = 0,    /* IC rows + per-level mass rows; affine (Eq. 10)                    */
+  SNAP_BURGERS1D_LF = 1,      /* IC + finite-volume residual, Lax-Friedrichs flux, explicit viscosity, periodic  */
+  SNAP_FISHER1D_IE = 2,       /* IC + implicit-Euler Fisher-KPP residual, ghost-cell Neumann                     */
+  SNAP_ALLENCAHN2D_IE = 3,    /* IC + implicit-Euler Allen-Cahn residual, 5-point periodic (2D, PCG path)        */
+  SNAP_BURGERS1D_LF_MASS = 4  /* kind 1 + per-level mass rows (dense border rows, all linearly dependent)        */
+};
+
+/* Return codes. */
+enum {
+  SNAP_OK = 0,
+  SNAP_EINVAL = -1,  /* bad kind / size / NULL pointer / ny != 1 for a 1D kind / size above the limits below */
+  SNAP_ECUDA = -2,   /* a CUDA call or launch failed (query cudaGetLastError)                                */
+  SNAP_ENOMEM = -3   /* workspace too small / staging allocation failed                                       */
+};
+
+/* Per-sample status written to iters[b] when negative; iters[b] >= 0 = number of linear (Schur) solves. */
+enum {
+  SNAP_ST_MAXITER = -1,    /* max_iter Gauss-Newton steps without reaching tol; u* = last iterate            */
+  SNAP_ST_LINESEARCH = -2, /* Armijo back-tracking exhausted ls_max halvings; u* = last accepted iterate      */
+  SNAP_ST_NONFINITE = -3,  /* non-finite residual or direction; u* = u_hat, lam = 0          */
+  SNAP_ST_PCG = -4         /* 2D: PCG hit pcg_max without reaching pcg_rtol; u* = last iterate               */
+};
+
+/* Size limits of this implementation (snap_problem_create returns SNAP_EINVAL beyond them):
+ *   1D kinds: 2 <= nx <= 512, ny == 1, 2 <= nt <= 65535;  2D kind: 4 <= nx, ny and nx*ny <= 4096, nt >= 2. */
+
+typedef struct {
+  double dx, dy, dt;  /* grid steps (caller supplied so that oracle and GPU share them bit for bit)           */
+  double nu, alpha;   /* Burgers: viscosity; Lax-Friedrichs dissipation (a constant)           */
+  double D, rho;      /* Fisher-KPP: diffusion, reaction rate                                                 */
+  double eps;         /* Allen-Cahn interface width                                                           */
+  double tol;         /* stop when ||h(u)||_inf < tol                       (default 1e-10)                   */
+  int max_iter;       /* cap on Gauss-Newton steps                          (default 50)                      */
+  int polish;         /* extra full steps once tol is met; skipped when
+                         ||h||_inf <= 1e-3 * tol already                    (default 1)                       */
+  double ls_c1;       /* Armijo sufficient-decrease constant                (default 1e-4)                    */
+  double ls_shrink;   /* step-length reduction factor                       (default 0.5)                     */
+  int ls_max;         /* maximum number of reductions per step              (default 20)                      */
+  double pcg_rtol;    /* 2D: PCG stops at ||r - S lam||_2 <= pcg_rtol ||r||_2 (default 1e-13)  */
+  int pcg_max;        /* 2D: PCG iteration cap per solve                    (default 200)                     */
+  int precond;        /* 2D: 0 none, 1 time-line, 2 time-line x ADI, 3 time-line x exact level solve (default 2) */
+  int lambda_mode;    /* 0 = minimum-norm multiplier, 1 = basic (redundant multipliers = 0)    */
+} snap_params;
+
+/* Fill *p with the defaults listed above (grid steps 1, physical constants 0, alpha = 1). */
+void snap_params_default(snap_params* p);
+
+/* Create a problem handle.  Validates kind/sizes/params, precomputes grid constants (and, for the 2D
+ * kind, the truncated circulant Green's function of the ADI line operator, copied to device memory owned
+ * by the handle).  ny must be 1 for 1D kinds.  *out is set only on success. */
+int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, const snap_params* params);
+int snap_problem_destroy(snap_problem* p);
+
+/* Sizes: unknowns n and constraint rows m per sample (0 for a NULL handle). */
+size_t snap_num_unknowns(const snap_problem* p);
+size_t snap_num_rows(const snap_problem* p);
+
+/* Bytes of device workspace snap_project needs for `batch` samples (256-byte aligned base expected). */
+size_t snap_workspace_bytes(const snap_problem* p, int batch);
+
+/* Batched projection (Eq. 2/4; the whole hot path of SURVEY.md §8(a) a1-a9).
+ *   u_hat   dev [batch][nt][ny][nx]  in   point to project.  May alias u_star (in place).
+ *   cdata   dev [batch][ny][nx]      in   per-sample initial-condition target u0.
+ *   u_star  dev [batch][nt][ny][nx]  out  projected field.
+ *   lambda  dev [batch][m]           in/out  multipliers lam*.  If warm != 0 the incoming values seed the merit
+ *                                         parameter and, for the 2D kind, the PCG initial guess;
+ *                                         the iterate itself always starts at u_hat.
+ *   iters   dev [batch] (int32)      out  number of linear solves performed, or a negative SNAP_ST_* status.
+ *   workspace dev, >= snap_workspace_bytes(p, batch).
+ * Enqueues on `stream`; no host synchronisation. */
+int snap_project(const snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
+                 double* lambda, int* iters, int warm, void* workspace, snap_stream stream);
+
+/* Same computation with HOST buffers (pinned or pageable): copies inputs to a device staging area owned by
+ * the handle, runs snap_project, copies u_star / lambda / iters back, and synchronises `stream` before
+ * returning.  lambda is read only if warm != 0. */
+int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, const double* cdata_host,
+                      double* u_star_host, double* lambda_host, int* iters_host, int warm, snap_stream stream);
+
+/* Constraint residual and the per-type norms of the paper's constraint-error metric
+ * (Eq. 27).
+ *   h      dev [batch][m] or NULL.
+ *   norms  dev [batch][4] or NULL: ||h||_inf, ||h_IC||_2, ||h_PDE||_2, ||h_mass||_2 (0 where a type is absent). */
+int snap_residual(const snap_problem* p, int batch, const double* u, const double* cdata, double* h,
+                  double* norms, snap_stream stream);
+
+/* Matrix-free Schur operator (SURVEY.md §8(a) a2+a4): out = J(u) J(u)^T x for x in the multiplier layout,
+ * the operator is never assembled.  x, out: dev [batch][m]; u: dev [batch][nt][ny][nx].  `workspace` must
+ * hold batch*n doubles.  Used by the PCG path and exported for validation against an assembled J J^T. */
+int snap_schur_apply(const snap_problem* p, int batch, const double* u, const double* x, double* out,
+                     void* workspace, snap_stream stream);
+
+/* Number of kernel launches the library has enqueued through this handle since creation (host counter). */
+long long snap_launch_count(const snap_problem* p);
+
+const char* snap_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SNAP_H_ */

@@ -1,0 +1,315 @@
+// C ABI of libsnap (include/snap.h): validation, handle management, launch configuration.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "kernels_1d.cuh"
+#include "kernels_2d.cuh"
+#include "kernels_misc.cuh"
+#include "snap_internal.h"
+
+using namespace snap;
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool is_1d(int kind) { return kind != SNAP_ALLENCAHN2D_IE; }
+
+// Green's function of the cyclic tridiagonal (-a, 1+2a, -a) of size N, truncated where it drops below
+// 1e-17 of its peak (exact to fp64 rounding); g[t], t = 0..K, applied symmetrically (t = -K..K).
+void circulant_green(double a, int N, std::vector<double>& g) {
+  g.clear();
+  if (a <= 0.0) { g.push_back(1.0); return; }
+  const double b = 1.0 + 2.0 * a;
+  const double disc = sqrt(b * b - 4.0 * a * a);
+  const double rho = (b - disc) / (2.0 * a);
+  const double rhoN = pow(rho, (double)N);
+  const int Kmax = N / 2;
+  for (int t = 0; t <= Kmax; ++t) {
+    const double v = (pow(rho, (double)t) + pow(rho, (double)(N - t))) / ((1.0 - rhoN) * disc);
+    g.push_back(v);
+    if (t > 0 && v < 1e-17 * g[0]) break;
+  }
+  const int K = (int)g.size() - 1;
+  if (2 * K == N) g[K] *= 0.5;  // offset +K and -K are the same point on an even ring
+}
+
+int check_launch(snap_problem* p) {
+  p->launches++;
+  return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+}
+
+struct Plan1d {
+  int q, wpc, nst, nxp, warp_bytes, grid;
+  size_t smem;
+};
+
+bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
+  const int nx = p->dp.nx;
+  pl.q = 1;
+  while (pl.q * 32 < nx) pl.q *= 2;
+  if (pl.q > 16) return false;
+  pl.nxp = (nx + 1) & ~1;
+  const int sms = p->sm_count > 0 ? p->sm_count : 148;
+  int wpc = (batch + sms - 1) / sms;
+  if (wpc < 1) wpc = 1;
+  if (wpc > 8) wpc = 8;
+  const size_t limit = (size_t)p->max_smem_optin;
+  for (;; --wpc) {
+    for (int nst = 4; nst >= 2; --nst) {
+      const size_t wb = align_up((size_t)(3 * nst + 5) * pl.nxp * 8 + (size_t)nst * 8, 128);
+      if (wb * wpc <= limit) {
+        pl.wpc = wpc; pl.nst = nst; pl.warp_bytes = (int)wb; pl.smem = wb * wpc;
+        pl.grid = (batch + wpc - 1) / wpc;
+        return true;
+      }
+    }
+    if (wpc == 1) return false;
+  }
+}
+
+template <int KIND, int Q>
+int launch_1d_t(snap_problem* p, const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  auto kern = project1d_kernel<KIND, Q>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
+    return SNAP_ECUDA;
+  kern<<<pl.grid, pl.wpc * 32, pl.smem, st>>>(a);
+  return check_launch(p);
+}
+
+template <int KIND>
+int launch_1d_k(snap_problem* p, const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  switch (pl.q) {
+    case 1: return launch_1d_t<KIND, 1>(p, a, pl, st);
+    case 2: return launch_1d_t<KIND, 2>(p, a, pl, st);
+    case 4: return launch_1d_t<KIND, 4>(p, a, pl, st);
+    case 8: return launch_1d_t<KIND, 8>(p, a, pl, st);
+    case 16: return launch_1d_t<KIND, 16>(p, a, pl, st);
+  }
+  return SNAP_EINVAL;
+}
+
+bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+void snap_params_default(snap_params* p) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->dx = p->dy = p->dt = 1.0;
+  p->alpha = 1.0;
+  p->tol = 1e-10;
+  p->max_iter = 50;
+  p->polish = 1;
+  p->ls_c1 = 1e-4;
+  p->ls_shrink = 0.5;
+  p->ls_max = 20;
+  p->pcg_rtol = 1e-13;
+  p->pcg_max = 200;
+  p->precond = 2;
+  p->lambda_mode = 0;
+}
+
+int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, const snap_params* prm) {
+  if (!out || !prm) return SNAP_EINVAL;
+  if (kind < SNAP_HEAT1D_IC_MASS || kind > SNAP_BURGERS1D_LF_MASS) return SNAP_EINVAL;
+  if (is_1d(kind)) {
+    if (ny != 1 || nx < 2 || nx > 512 || nt < 2 || nt > 65535) return SNAP_EINVAL;
+  } else {
+    if (nx < 4 || ny < 4 || (long long)nx * ny > 4096 || nt < 2 || nt > 65535) return SNAP_EINVAL;
+  }
+  if (!(prm->dx > 0.0) || !(prm->dt > 0.0) || !(prm->tol > 0.0)) return SNAP_EINVAL;
+  if (!is_1d(kind) && !(prm->dy > 0.0)) return SNAP_EINVAL;
+  if (prm->max_iter < 0 || prm->polish < 0 || prm->ls_max < 0 || prm->pcg_max < 1) return SNAP_EINVAL;
+  if (!(prm->ls_shrink > 0.0 && prm->ls_shrink < 1.0) || !(prm->ls_c1 > 0.0 && prm->ls_c1 < 1.0)) return SNAP_EINVAL;
+  if (prm->precond < 0 || prm->precond > 2 || prm->lambda_mode < 0 || prm->lambda_mode > 1) return SNAP_EINVAL;
+
+  snap_problem* p = new (std::nothrow) snap_problem();
+  if (!p) return SNAP_ENOMEM;
+  memset(p, 0, sizeof(*p));
+  p->params = *prm;
+  DevParams& d = p->dp;
+  d.kind = kind; d.nx = nx; d.ny = ny; d.nt = nt;
+  d.lvl = nx * ny;
+  d.n = d.lvl * nt;
+  d.has_mass = (kind == SNAP_HEAT1D_IC_MASS || kind == SNAP_BURGERS1D_LF_MASS);
+  d.m = (kind == SNAP_HEAT1D_IC_MASS) ? nx + nt : d.n + (d.has_mass ? nt : 0);
+  d.dx = prm->dx; d.dy = prm->dy; d.dt = prm->dt;
+  const double s = prm->dt / prm->dx;
+  d.bs_e = 0.5 * s * prm->alpha + prm->nu * prm->dt / (prm->dx * prm->dx);
+  d.bs_a0 = 1.0 - 2.0 * d.bs_e;
+  d.bs_qs = 0.25 * s;
+  d.bs_hs = 0.5 * s;
+  d.fi_a = prm->dt * prm->D / (prm->dx * prm->dx);
+  d.fi_dtrho = prm->dt * prm->rho;
+  d.ac_ax = prm->dt * prm->eps * prm->eps / (prm->dx * prm->dx);
+  d.ac_ay = is_1d(kind) ? 0.0 : prm->dt * prm->eps * prm->eps / (prm->dy * prm->dy);
+  d.tol = prm->tol; d.ls_c1 = prm->ls_c1; d.ls_shrink = prm->ls_shrink; d.pcg_rtol = prm->pcg_rtol;
+  d.max_iter = prm->max_iter; d.polish = prm->polish; d.ls_max = prm->ls_max; d.pcg_max = prm->pcg_max;
+  d.precond = prm->precond; d.lambda_mode = prm->lambda_mode;
+
+  int dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) {
+    cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  }
+  if (p->sm_count <= 0) p->sm_count = 148;
+  if (p->max_smem_optin <= 0) p->max_smem_optin = 227 * 1024;
+
+  if (kind == SNAP_ALLENCAHN2D_IE) {
+    std::vector<double> gx, gy;
+    circulant_green(d.ac_ax, nx, gx);
+    circulant_green(d.ac_ay, ny, gy);
+    d.gx_K = (int)gx.size() - 1;
+    d.gy_K = (int)gy.size() - 1;
+    const size_t bytes = (gx.size() + gy.size()) * sizeof(double);
+    if (cudaMalloc(&p->d_green, bytes) != cudaSuccess) { delete p; return SNAP_ENOMEM; }
+    std::vector<double> both(gx);
+    both.insert(both.end(), gy.begin(), gy.end());
+    if (cudaMemcpy(p->d_green, both.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+      cudaFree(p->d_green); delete p; return SNAP_ECUDA;
+    }
+    d.gx = p->d_green;
+    d.gy = p->d_green + gx.size();
+  }
+  *out = p;
+  return SNAP_OK;
+}
+
+int snap_problem_destroy(snap_problem* p) {
+  if (!p) return SNAP_EINVAL;
+  if (p->d_green) cudaFree(p->d_green);
+  if (p->stage) cudaFree(p->stage);
+  delete p;
+  return SNAP_OK;
+}
+
+size_t snap_num_unknowns(const snap_problem* p) { return p ? (size_t)p->dp.n : 0; }
+size_t snap_num_rows(const snap_problem* p) { return p ? (size_t)p->dp.m : 0; }
+long long snap_launch_count(const snap_problem* p) { return p ? p->launches : 0; }
+
+size_t snap_workspace_bytes(const snap_problem* p, int batch) {
+  if (!p || batch <= 0) return 0;
+  const size_t n = (size_t)p->dp.n, B = (size_t)batch;
+  if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return 256;
+  if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return align_up(B * n * 8 * kPcgVectors, 256) + 256;
+  return align_up(B * n * 8, 256) * 2 + align_up(B * 2 * (size_t)p->dp.nt * 8, 256) + 256;
+}
+
+int snap_project(const snap_problem* cp, int batch, const double* u_hat, const double* cdata, double* u_star,
+                 double* lambda, int* iters, int warm, void* workspace, snap_stream stream) {
+  snap_problem* p = const_cast<snap_problem*>(cp);
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u_hat || !cdata || !u_star || !lambda || !iters) return SNAP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const DevParams& d = p->dp;
+  if (d.kind == SNAP_HEAT1D_IC_MASS) {
+    const int wpc = 4;
+    heat_project_kernel<<<(batch + wpc - 1) / wpc, wpc * 32, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters);
+    return check_launch(p);
+  }
+  if (!workspace) return SNAP_EINVAL;
+  if (d.kind == SNAP_ALLENCAHN2D_IE)
+    return launch_project2d(p, batch, u_hat, cdata, u_star, lambda, iters, warm, workspace, st);
+
+  Plan1d pl;
+  if (!plan_1d(p, batch, pl)) return SNAP_EINVAL;
+  Proj1dArgs a;
+  a.P = d;
+  a.batch = batch; a.warm = warm;
+  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
+  const size_t field = align_up((size_t)batch * d.n * 8, 256);
+  unsigned char* w = static_cast<unsigned char*>(workspace);
+  w = reinterpret_cast<unsigned char*>(align_up(reinterpret_cast<uintptr_t>(w), 256));
+  a.bufA = reinterpret_cast<double*>(w);
+  a.bufB = reinterpret_cast<double*>(w + field);
+  a.aux = reinterpret_cast<double*>(w + 2 * field);
+  a.nst = pl.nst; a.nxp = pl.nxp; a.warp_bytes = pl.warp_bytes;
+  // bulk (TMA) copies need every row start 16-byte aligned
+  a.tma = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
+          aligned16(lambda) && aligned16(a.bufA);
+  if (d.kind == SNAP_FISHER1D_IE) return launch_1d_k<KF>(p, a, pl, st);
+  return launch_1d_k<KB>(p, a, pl, st);
+}
+
+int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, const double* cdata_host,
+                      double* u_star_host, double* lambda_host, int* iters_host, int warm, snap_stream stream) {
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u_hat_host || !cdata_host || !u_star_host || !lambda_host || !iters_host) return SNAP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const DevParams& d = p->dp;
+  const size_t B = (size_t)batch;
+  const size_t b_u = align_up(B * d.n * 8, 256), b_c = align_up(B * d.lvl * 8, 256), b_l = align_up(B * d.m * 8, 256),
+               b_i = align_up(B * 4, 256), b_w = align_up(snap_workspace_bytes(p, batch), 256);
+  const size_t total = 2 * b_u + b_c + b_l + b_i + b_w;
+  if (p->stage_bytes < total) {
+    if (p->stage) cudaFree(p->stage);
+    p->stage = nullptr;
+    p->stage_bytes = 0;
+    if (cudaMalloc(&p->stage, total) != cudaSuccess) return SNAP_ENOMEM;
+    p->stage_bytes = total;
+  }
+  unsigned char* s = static_cast<unsigned char*>(p->stage);
+  double* d_uh = reinterpret_cast<double*>(s);
+  double* d_us = reinterpret_cast<double*>(s + b_u);
+  double* d_c = reinterpret_cast<double*>(s + 2 * b_u);
+  double* d_l = reinterpret_cast<double*>(s + 2 * b_u + b_c);
+  int* d_i = reinterpret_cast<int*>(s + 2 * b_u + b_c + b_l);
+  void* d_w = s + 2 * b_u + b_c + b_l + b_i;
+  if (cudaMemcpyAsync(d_uh, u_hat_host, B * d.n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return SNAP_ECUDA;
+  if (cudaMemcpyAsync(d_c, cdata_host, B * d.lvl * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return SNAP_ECUDA;
+  if (warm && cudaMemcpyAsync(d_l, lambda_host, B * d.m * 8, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return SNAP_ECUDA;
+  const int rc = snap_project(p, batch, d_uh, d_c, d_us, d_l, d_i, warm, d_w, stream);
+  if (rc != SNAP_OK) return rc;
+  if (cudaMemcpyAsync(u_star_host, d_us, B * d.n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
+  if (cudaMemcpyAsync(lambda_host, d_l, B * d.m * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
+  if (cudaMemcpyAsync(iters_host, d_i, B * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
+  return cudaStreamSynchronize(st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+}
+
+int snap_residual(const snap_problem* cp, int batch, const double* u, const double* cdata, double* h, double* norms,
+                  snap_stream stream) {
+  snap_problem* p = const_cast<snap_problem*>(cp);
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u || !cdata || (!h && !norms)) return SNAP_EINVAL;
+  residual_kernel<<<batch, kMiscThreads, 0, static_cast<cudaStream_t>(stream)>>>(p->dp, batch, u, cdata, h, norms);
+  return check_launch(p);
+}
+
+int snap_schur_apply(const snap_problem* cp, int batch, const double* u, const double* x, double* out, void* workspace,
+                     snap_stream stream) {
+  snap_problem* p = const_cast<snap_problem*>(cp);
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u || !x || !out || !workspace) return SNAP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double* g = static_cast<double*>(workspace);
+  jt_apply_kernel<<<batch, kMiscThreads, 0, st>>>(p->dp, batch, u, x, g);
+  int rc = check_launch(p);
+  if (rc != SNAP_OK) return rc;
+  j_apply_kernel<<<batch, kMiscThreads, 0, st>>>(p->dp, batch, u, g, out);
+  return check_launch(p);
+}
+
+const char* snap_strerror(int code) {
+  switch (code) {
+    case SNAP_OK: return "ok";
+    case SNAP_EINVAL: return "invalid argument (kind, sizes, NULL pointer or size limit)";
+    case SNAP_ECUDA: return "CUDA call or kernel launch failed";
+    case SNAP_ENOMEM: return "workspace too small or allocation failed";
+  }
+  return "unknown error code";
+}
+
+}  // extern "C"

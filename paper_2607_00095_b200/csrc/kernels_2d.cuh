@@ -1,0 +1,447 @@
+// 2D kind (Allen-Cahn, implicit Euler, 5-point periodic): one persistent CTA per sample runs the whole
+// Gauss-Newton loop; the Schur system (J J^T) lam = r is solved by preconditioned conjugate gradients,
+// matrix-free:
+//     S p = J (J^T p)                  two stencil passes fused per level through shared memory
+//     M   = Jt Jt^T,  Jt = J with T_k replaced by the constant ADI operator (I - ax dxx)(I - ay dyy)
+//     M^{-1} r: forward time sweep y_k = Tt^{-1}(r_k + y_{k-1}), backward sweep z_k = Tt^{-1}(y_k + z_{k+1})
+// The cyclic constant-coefficient line solves of Tt^{-1} are applied as truncated circulant convolutions
+// (Green's function of (-a, 1+2a, -a), exact to fp64 rounding) on the level held in shared memory.
+#pragma once
+#include "device_utils.cuh"
+#include "snap_internal.h"
+
+namespace snap {
+
+constexpr int kT2 = 512;          // threads per CTA (one CTA per sample)
+constexpr int kPcgVectors = 8;    // workspace n-vectors per sample: bufA bufB b r z p q y
+
+struct Proj2dArgs {
+  DevParams P;
+  int batch, warm;
+  const double* u_hat;
+  const double* cdata;
+  double* u_star;
+  double* lam;
+  int* iters;
+  double* ws;  // [batch][kPcgVectors][n]
+};
+
+struct Ctx2d {
+  int nx, ny, L, nt;
+  int i, ip, im, jr, rpp;  // this thread's column, its periodic neighbours, first row, rows per pass
+  bool active;
+  double* s0;  // three level buffers in shared memory
+  double* s1;
+  double* s2;
+  double* red;
+  double* gx;
+  double* gy;
+};
+
+__device__ __forceinline__ double blk_sum(const Ctx2d& c, double v) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) c.red[warp] = v;
+  __syncthreads();
+  double r = (lane < (kT2 >> 5)) ? c.red[lane] : 0.0;
+  return warp_sum(r);
+}
+__device__ __forceinline__ double blk_max(const Ctx2d& c, double v) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  v = warp_max(v);
+  __syncthreads();
+  if (lane == 0) c.red[warp] = v;
+  __syncthreads();
+  double r = (lane < (kT2 >> 5)) ? c.red[lane] : 0.0;
+  return warp_max(r);
+}
+
+#define SNAP_FOR_CELLS(c, cell, j) \
+  if ((c).active)                  \
+    for (int j = (c).jr, cell = (c).jr * (c).nx + (c).i; j < (c).ny; j += (c).rpp, cell += (c).rpp * (c).nx)
+
+// T x at one cell, x in shared memory:  x - ax lap_x x - ay lap_y x + dt (3 w^2 - 1) x
+__device__ __forceinline__ double T_apply(const DevParams& P, const Ctx2d& c, const double* x, int j, int cell,
+                                          double w) {
+  const int row = j * c.nx;
+  const int yp = ((j + 1 == c.ny) ? 0 : j + 1) * c.nx + c.i, ym = ((j == 0) ? c.ny - 1 : j - 1) * c.nx + c.i;
+  const double xc = x[cell];
+  return xc - P.ac_ax * ((x[row + c.ip] - xc) + (x[row + c.im] - xc)) - P.ac_ay * ((x[yp] - xc) + (x[ym] - xc)) +
+         P.dt * (3.0 * w * w - 1.0) * xc;
+}
+
+// ---- a1-a3: residual norms and b = h - J (u - u_hat) at the point u --------------------------------
+__device__ void rhs_pass(const DevParams& P, const Ctx2d& c, const double* __restrict__ u,
+                         const double* __restrict__ uh, const double* __restrict__ u0, double* __restrict__ b,
+                         double& hinf, double& h1, double& f, int& bad) {
+  double a_inf = 0.0, a_1 = 0.0, a_f = 0.0;
+  for (int k = 0; k < c.nt; ++k) {
+    const double* uk = u + (size_t)k * c.L;
+    const double* uhk = uh + (size_t)k * c.L;
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double v = uk[cell];
+      c.s0[cell] = v;
+      c.s1[cell] = v - uhk[cell];
+    }
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double v = c.s0[cell], w = c.s1[cell];
+      double h, bb;
+      if (k == 0) {
+        h = v - u0[cell];
+        bb = h - w;
+      } else {
+        const int row = j * c.nx;
+        const int yp = ((j + 1 == c.ny) ? 0 : j + 1) * c.nx + c.i, ym = ((j == 0) ? c.ny - 1 : j - 1) * c.nx + c.i;
+        const double vprev = uk[cell - c.L];
+        const double wprev = vprev - uhk[cell - c.L];
+        h = v - vprev - P.ac_ax * ((c.s0[row + c.ip] - v) + (c.s0[row + c.im] - v)) -
+            P.ac_ay * ((c.s0[yp] - v) + (c.s0[ym] - v)) + P.dt * (v * v * v - v);
+        bb = h - (T_apply(P, c, c.s1, j, cell, v) - wprev);
+      }
+      b[(size_t)k * c.L + cell] = bb;
+      const double ah = fabs(h);
+      if (!finite_d(ah)) a_inf = 1.7976931348623157e308 * 2.0;
+      a_inf = fmax(a_inf, ah);
+      a_1 += ah;
+      a_f = fma(w, w, a_f);
+    }
+  }
+  hinf = blk_max(c, a_inf);
+  h1 = blk_sum(c, a_1);
+  f = 0.5 * blk_sum(c, a_f);
+  bad = !(finite_d(hinf) && finite_d(h1) && finite_d(f));
+}
+
+// ---- a4: q = J (J^T x), never assembled; returns x . q ---------------------------------------------
+//   g_0 = x_0 - x_1 ; g_k = T_k x_k - x_{k+1} ;  q_0 = g_0 ; q_k = T_k g_k - g_{k-1}
+__device__ double schur_apply(const DevParams& P, const Ctx2d& c, const double* __restrict__ u,
+                              const double* __restrict__ x, double* __restrict__ q) {
+  double dot = 0.0;
+  double* gcur = c.s1;
+  double* gprev = c.s2;
+  for (int k = 0; k < c.nt; ++k) {
+    const double* uk = u + (size_t)k * c.L;
+    const double* xk = x + (size_t)k * c.L;
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) c.s0[cell] = xk[cell];
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      double g = (k == 0) ? c.s0[cell] : T_apply(P, c, c.s0, j, cell, uk[cell]);
+      if (k + 1 < c.nt) g -= xk[cell + c.L];
+      gcur[cell] = g;
+    }
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double qq = (k == 0) ? gcur[cell] : T_apply(P, c, gcur, j, cell, uk[cell]) - gprev[cell];
+      q[(size_t)k * c.L + cell] = qq;
+      dot = fma(c.s0[cell], qq, dot);
+    }
+    double* t = gcur; gcur = gprev; gprev = t;
+  }
+  return blk_sum(c, dot);
+}
+
+// Tt^{-1} on the level in `buf` (in place), `tmp` scratch: circulant convolution along x, then along y.
+__device__ void adi_inverse(const DevParams& P, const Ctx2d& c, double* buf, double* tmp) {
+  __syncthreads();
+  SNAP_FOR_CELLS(c, cell, j) {
+    const int row = j * c.nx;
+    double acc = c.gx[0] * buf[cell];
+    for (int t = 1; t <= P.gx_K; ++t) {
+      int a = c.i + t; if (a >= c.nx) a -= c.nx;
+      int d = c.i - t; if (d < 0) d += c.nx;
+      acc = fma(c.gx[t], buf[row + a] + buf[row + d], acc);
+    }
+    tmp[cell] = acc;
+  }
+  __syncthreads();
+  SNAP_FOR_CELLS(c, cell, j) {
+    double acc = c.gy[0] * tmp[cell];
+    for (int t = 1; t <= P.gy_K; ++t) {
+      int a = j + t; if (a >= c.ny) a -= c.ny;
+      int d = j - t; if (d < 0) d += c.ny;
+      acc = fma(c.gy[t], tmp[a * c.nx + c.i] + tmp[d * c.nx + c.i], acc);
+    }
+    buf[cell] = acc;
+  }
+  __syncthreads();
+}
+
+// ---- preconditioner z = M^{-1} r ; returns r . z -----------------------------------------------------
+__device__ double precond_apply(const DevParams& P, const Ctx2d& c, const double* __restrict__ r,
+                                double* __restrict__ z, double* __restrict__ y) {
+  double dot = 0.0;
+  if (P.precond == 0) {
+    for (int k = 0; k < c.nt; ++k) SNAP_FOR_CELLS(c, cell, j) {
+      const double v = r[(size_t)k * c.L + cell];
+      z[(size_t)k * c.L + cell] = v;
+      dot = fma(v, v, dot);
+    }
+    return blk_sum(c, dot);
+  }
+  // forward: y_0 = r_0 ; y_k = Tt^{-1} (r_k + y_{k-1})      (level kept in s0)
+  for (int k = 0; k < c.nt; ++k) {
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double v = r[(size_t)k * c.L + cell];
+      c.s0[cell] = (k == 0) ? v : v + c.s0[cell];
+    }
+    if (k > 0 && P.precond == 2) adi_inverse(P, c, c.s0, c.s1);
+    SNAP_FOR_CELLS(c, cell, j) y[(size_t)k * c.L + cell] = c.s0[cell];
+  }
+  // backward: z_k = Tt^{-1} (y_k + z_{k+1}) ; z_0 = y_0 + z_1
+  for (int k = c.nt - 1; k >= 0; --k) {
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double v = y[(size_t)k * c.L + cell];
+      c.s0[cell] = (k == c.nt - 1) ? v : v + c.s0[cell];
+    }
+    if (k > 0 && P.precond == 2) adi_inverse(P, c, c.s0, c.s1);
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double zz = c.s0[cell];
+      z[(size_t)k * c.L + cell] = zz;
+      dot = fma(r[(size_t)k * c.L + cell], zz, dot);
+    }
+  }
+  return blk_sum(c, dot);
+}
+
+// ---- a8: trial = u_hat - J^T lam ; returns ||lam||_inf and (u - u_hat)^T (trial - u) ------------------
+__device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __restrict__ u,
+                          const double* __restrict__ uh, const double* __restrict__ lam, double* __restrict__ trial,
+                          double& linf, double& wd) {
+  double a_inf = 0.0, a_wd = 0.0;
+  for (int k = 0; k < c.nt; ++k) {
+    const double* uk = u + (size_t)k * c.L;
+    const double* lk = lam + (size_t)k * c.L;
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) c.s0[cell] = lk[cell];
+    __syncthreads();
+    SNAP_FOR_CELLS(c, cell, j) {
+      const double v = uk[cell], hh = uh[(size_t)k * c.L + cell];
+      double g = (k == 0) ? c.s0[cell] : T_apply(P, c, c.s0, j, cell, v);
+      if (k + 1 < c.nt) g -= lk[cell + c.L];
+      const double tr = hh - g;
+      trial[(size_t)k * c.L + cell] = tr;
+      a_wd = fma(v - hh, tr - v, a_wd);
+      const double al = fabs(c.s0[cell]);
+      if (!finite_d(al)) a_inf = 1.7976931348623157e308 * 2.0;
+      a_inf = fmax(a_inf, al);
+    }
+  }
+  linf = blk_max(c, a_inf);
+  wd = blk_sum(c, a_wd);
+}
+
+// ---- a6: PCG on S lam = b.  Returns 0 on success, 1 if pcg_max was hit ----------------------------------
+__device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __restrict__ u, const double* __restrict__ b,
+                         double* __restrict__ x, double* r, double* z, double* p, double* q, double* y, bool warm,
+                         size_t n) {
+  const int tid = threadIdx.x;
+  double bb = 0.0;
+  for (size_t i = tid; i < n; i += kT2) bb = fma(b[i], b[i], bb);
+  bb = blk_sum(c, bb);
+  const double bnorm = sqrt(bb);
+  if (bnorm == 0.0) {
+    for (size_t i = tid; i < n; i += kT2) x[i] = 0.0;
+    return 0;
+  }
+  if (warm) {
+    schur_apply(P, c, u, x, q);
+    __syncthreads();
+    for (size_t i = tid; i < n; i += kT2) r[i] = b[i] - q[i];
+  } else {
+    for (size_t i = tid; i < n; i += kT2) { x[i] = 0.0; r[i] = b[i]; }
+  }
+  __syncthreads();
+  double rz = precond_apply(P, c, r, z, y);
+  __syncthreads();
+  for (size_t i = tid; i < n; i += kT2) p[i] = z[i];
+  for (int it = 0; it < P.pcg_max; ++it) {
+    __syncthreads();
+    const double pq = schur_apply(P, c, u, p, q);
+    const double alpha = rz / pq;
+    __syncthreads();
+    double rr = 0.0;
+    for (size_t i = tid; i < n; i += kT2) {
+      x[i] = fma(alpha, p[i], x[i]);
+      const double rn = fma(-alpha, q[i], r[i]);
+      r[i] = rn;
+      rr = fma(rn, rn, rr);
+    }
+    rr = blk_sum(c, rr);
+    if (!finite_d(rr)) return 2;
+    if (sqrt(rr) <= P.pcg_rtol * bnorm) {
+      // exit test on the true residual, recomputed
+      __syncthreads();
+      schur_apply(P, c, u, x, q);
+      __syncthreads();
+      double tr = 0.0;
+      for (size_t i = tid; i < n; i += kT2) {
+        const double rn = b[i] - q[i];
+        r[i] = rn;
+        tr = fma(rn, rn, tr);
+      }
+      tr = blk_sum(c, tr);
+      if (sqrt(tr) <= P.pcg_rtol * bnorm) return 0;
+    }
+    __syncthreads();
+    const double rz_new = precond_apply(P, c, r, z, y);
+    const double beta = rz_new / rz;
+    rz = rz_new;
+    __syncthreads();
+    for (size_t i = tid; i < n; i += kT2) p[i] = fma(beta, p[i], z[i]);
+  }
+  return 1;
+}
+
+__global__ void __launch_bounds__(kT2) project2d_kernel(const __grid_constant__ Proj2dArgs A) {
+  extern __shared__ __align__(16) unsigned char smem2[];
+  const DevParams& P = A.P;
+  const int b = blockIdx.x;
+  if (b >= A.batch) return;
+  Ctx2d c;
+  c.nx = P.nx; c.ny = P.ny; c.L = P.lvl; c.nt = P.nt;
+  c.s0 = reinterpret_cast<double*>(smem2);
+  c.s1 = c.s0 + c.L;
+  c.s2 = c.s1 + c.L;
+  c.red = c.s2 + c.L;
+  c.gx = c.red + 32;
+  c.gy = c.gx + (P.gx_K + 1);
+  c.rpp = kT2 / c.nx;
+  c.i = threadIdx.x % c.nx;
+  c.jr = threadIdx.x / c.nx;
+  c.active = c.jr < c.rpp;
+  c.ip = (c.i + 1 == c.nx) ? 0 : c.i + 1;
+  c.im = (c.i == 0) ? c.nx - 1 : c.i - 1;
+  for (int t = threadIdx.x; t <= P.gx_K; t += kT2) c.gx[t] = P.gx[t];
+  for (int t = threadIdx.x; t <= P.gy_K; t += kT2) c.gy[t] = P.gy[t];
+  __syncthreads();
+
+  const size_t n = (size_t)P.n;
+  const int tid = threadIdx.x;
+  const double* uh = A.u_hat + (size_t)b * n;
+  const double* u0 = A.cdata + (size_t)b * c.L;
+  double* ustar = A.u_star + (size_t)b * n;
+  double* lam = A.lam + (size_t)b * n;
+  double* ws = A.ws + (size_t)b * kPcgVectors * n;
+  double* bufA = ws;
+  double* bufB = ws + n;
+  double* bv = ws + 2 * n;
+  double* rv = ws + 3 * n;
+  double* zv = ws + 4 * n;
+  double* pv = ws + 5 * n;
+  double* qv = ws + 6 * n;
+  double* yv = ws + 7 * n;
+
+  double mu = 0.0;
+  bool have_lam = A.warm != 0;
+  if (have_lam) {
+    double li = 0.0;
+    for (size_t i = tid; i < n; i += kT2) {
+      const double v = fabs(lam[i]);
+      li = fmax(li, finite_d(v) ? v : 1.7976931348623157e308 * 2.0);
+    }
+    li = blk_max(c, li);
+    if (finite_d(li)) mu = 1.1 * li + 1e-3; else have_lam = false;
+  }
+
+  const double* cur = uh;
+  double* trial = bufA;
+  bool have_trial = false, polishing = false;
+  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0;
+  double alpha = 1.0, phi_cur = 0.0, Dphi = 0.0;
+  double hinf = 0.0, h1 = 0.0, f = 0.0;
+  int bad = 0;
+
+  while (true) {
+    const double* pt = have_trial ? trial : cur;
+    __syncthreads();
+    rhs_pass(P, c, pt, uh, u0, bv, hinf, h1, f, bad);
+    if (have_trial) {
+      if (!polishing) {
+        const double phi_t = f + mu * h1;
+        const bool ok = !bad && finite_d(phi_t) && (phi_t <= phi_cur + P.ls_c1 * alpha * Dphi);
+        if (!ok) {
+          if (++tries > P.ls_max) { status = SNAP_ST_LINESEARCH; break; }
+          __syncthreads();
+          for (size_t i = tid; i < n; i += kT2) trial[i] = fma(P.ls_shrink, trial[i] - cur[i], cur[i]);
+          alpha *= P.ls_shrink;
+          continue;
+        }
+        ++steps;
+      }
+      cur = trial;
+      trial = (trial == bufA) ? bufB : bufA;
+      have_trial = false;
+    } else if (bad) {
+      status = SNAP_ST_NONFINITE;
+      break;
+    }
+    ++solves;
+    __syncthreads();
+    const int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n);
+    have_lam = true;
+    __syncthreads();
+    if (prc == 2) { status = SNAP_ST_NONFINITE; break; }
+    if (prc == 1) { status = SNAP_ST_PCG; break; }
+    const bool conv = hinf < P.tol;
+    bool final_solve = false;
+    if (polishing) {
+      final_solve = (polish_left == 0);
+    } else if (conv) {
+      polishing = true;
+      polish_left = (hinf > kPolishSkip * P.tol) ? P.polish : 0;
+      final_solve = (polish_left == 0);
+    } else if (steps >= P.max_iter) {
+      status = SNAP_ST_MAXITER;
+      final_solve = true;
+    }
+    if (final_solve) break;
+    double linf, wd;
+    step_pass(P, c, cur, uh, lam, trial, linf, wd);
+    if (!finite_d(linf) || !finite_d(wd)) { status = SNAP_ST_NONFINITE; break; }
+    if (polishing) {
+      --polish_left;
+    } else {
+      mu = fmax(mu, 1.1 * linf + 1e-3);
+      phi_cur = f + mu * h1;
+      Dphi = wd - mu * h1;
+      alpha = 1.0;
+      tries = 0;
+    }
+    have_trial = true;
+  }
+  __syncthreads();
+  if (status == SNAP_ST_NONFINITE) {
+    if (ustar != uh)
+      for (size_t i = tid; i < n; i += kT2) ustar[i] = uh[i];
+    for (size_t i = tid; i < n; i += kT2) lam[i] = 0.0;
+  } else if (ustar != cur) {
+    for (size_t i = tid; i < n; i += kT2) ustar[i] = cur[i];
+  }
+  if (tid == 0) A.iters[b] = (status == 0) ? solves : status;
+}
+
+inline int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
+                            double* lambda, int* iters, int warm, void* workspace, cudaStream_t st) {
+  const DevParams& d = p->dp;
+  if (d.nx > kT2) return SNAP_EINVAL;
+  Proj2dArgs a;
+  a.P = d;
+  a.batch = batch; a.warm = warm;
+  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
+  a.ws = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~(uintptr_t)255);
+  const size_t smem = ((size_t)3 * d.lvl + 32 + d.gx_K + 1 + d.gy_K + 1) * sizeof(double);
+  if (smem > (size_t)p->max_smem_optin) return SNAP_EINVAL;
+  if (cudaFuncSetAttribute(project2d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return SNAP_ECUDA;
+  project2d_kernel<<<batch, kT2, smem, st>>>(a);
+  p->launches++;
+  return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+}
+
+}  // namespace snap

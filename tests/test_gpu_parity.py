@@ -1,0 +1,299 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle, element by element on
+the same seeded inputs (SURVEY.md §8(c) "Parity metric"):
+    rel_u = ||u*_gpu - u*_orc||_inf / ||u*_orc||_inf <= 1e-9      (north_star)
+    rel_l = ||lam_gpu - lam_orc||_inf / ||lam_orc||_inf <= 1e-8   (absolute 1e-12 where lam = 0)
+plus ||h(u*)||_inf < 1e-10 on every sample."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_U, TOL_L = 1e-9, 1e-8
+
+
+@pytest.fixture(scope="module")
+def S():
+    import paper_2607_00095_b200 as S
+    S.load_library()
+    return S
+
+
+def gpu_project(S, wl, u_hat, params=None, warm=False, lam0=None, in_place=False):
+    dev = torch.device("cuda:0")
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, dict(wl.params, **(params or {})))
+    B = u_hat.shape[0]
+    uh = u_hat.to(dev).contiguous()
+    cd = wl.cdata[:B].to(dev).contiguous()
+    us = uh if in_place else torch.full_like(uh, float("nan"))
+    lam = torch.full((B, p.m), float("nan"), dtype=torch.float64, device=dev)
+    if lam0 is not None:
+        lam.copy_(lam0.to(dev))
+    it = torch.full((B,), -99, dtype=torch.int32, device=dev)
+    S.snap_project(p, B, uh, cd, us, lam, it, warm=warm)
+    norms = torch.empty(B, 4, dtype=torch.float64, device=dev)
+    S.snap_residual(p, B, us, cd, None, norms)
+    torch.cuda.synchronize()
+    out = dict(u=us.cpu().numpy(), lam=lam.cpu().numpy(), iters=it.cpu().numpy(), norms=norms.cpu().numpy(),
+               launches=p.launch_count())
+    p.destroy()
+    return out
+
+
+def check_against_oracle(wl, u_hat, g, samples, params=None, tol_u=TOL_U, tol_l=TOL_L):
+    p = dict(wl.params, **(params or {}))
+    worst_u = worst_l = 0.0
+    for b in samples:
+        o = O.project(wl.kind, u_hat[b].numpy(), wl.cdata[b].numpy(), p)
+        assert o["status"] == 0
+        assert g["iters"][b] > 0, f"sample {b}: status {g['iters'][b]}"
+        ru = np.abs(g["u"][b] - o["u"]).max() / np.abs(o["u"]).max()
+        ln = np.abs(o["lam"]).max()
+        rl = np.abs(g["lam"][b] - o["lam"]).max() / ln if ln > 1e-9 else np.abs(g["lam"][b] - o["lam"]).max() * 1e4
+        worst_u, worst_l = max(worst_u, ru), max(worst_l, rl)
+        assert ru <= tol_u, f"sample {b}: rel_u {ru:.2e}"
+        assert rl <= tol_l, f"sample {b}: rel_lam {rl:.2e}"
+        assert abs(int(g["iters"][b]) - int(o["iters"])) <= 1
+    return worst_u, worst_l
+
+
+# ------------------------------------------------------------------------------------------------
+# a1 / a2+a4: residual and matrix-free Schur operator
+# ------------------------------------------------------------------------------------------------
+SHAPES = {
+    1: [dict(batch=3, nx=20, nt=12), dict(batch=2, nx=65, nt=7)],
+    2: [dict(batch=3, nx=24, nt=20), dict(batch=2, nx=101, nt=9), dict(batch=2, nx=128, nt=40)],
+    3: [dict(batch=3, nx=24, nt=20), dict(batch=2, nx=77, nt=9)],
+    4: [dict(batch=2, nx=12, ny=10, nt=6), dict(batch=2, nx=64, ny=64, nt=4)],
+    5: [dict(batch=3, nx=24, nt=20), dict(batch=2, nx=101, nt=9)],
+}
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_residual_and_schur_operator(S, cfg):
+    dev = torch.device("cuda:0")
+    for kw in SHAPES[cfg]:
+        wl = W.make_workload(cfg, **kw)
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        B = wl.batch
+        u = wl.u_hat.to(dev)
+        cd = wl.cdata.to(dev)
+        h = torch.empty(B, p.m, dtype=torch.float64, device=dev)
+        norms = torch.empty(B, 4, dtype=torch.float64, device=dev)
+        S.snap_residual(p, B, u, cd, h, norms)
+        g = torch.Generator().manual_seed(7)
+        x = torch.randn(B, p.m, generator=g, dtype=torch.float64)
+        out = torch.empty(B, p.m, dtype=torch.float64, device=dev)
+        ws = torch.empty(B * p.n, dtype=torch.float64, device=dev)
+        S.snap_schur_apply(p, B, u, x.to(dev), out, ws)
+        torch.cuda.synchronize()
+        for b in range(B):
+            ub, u0 = wl.u_hat[b].numpy(), wl.cdata[b].numpy()
+            h_ref = O.residual(wl.kind, ub, u0, wl.params)
+            np.testing.assert_allclose(h[b].cpu().numpy(), h_ref, rtol=0, atol=2e-14 * max(1, np.abs(h_ref).max()))
+            n_ref = O.residual_norms(wl.kind, ub, u0, wl.params)
+            np.testing.assert_allclose(norms[b].cpu().numpy(), n_ref, rtol=1e-13, atol=1e-15)
+            J = O.jacobian(wl.kind, ub, wl.params)
+            s_ref = J @ (J.T @ x[b].numpy())
+            np.testing.assert_allclose(out[b].cpu().numpy(), s_ref, rtol=0, atol=1e-13 * max(1, np.abs(s_ref).max()))
+        p.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# whole path, small sizes: several tiles, ragged tails, odd nx (non-bulk path), every sample
+# ------------------------------------------------------------------------------------------------
+SMALL = {
+    1: [dict(batch=4), dict(batch=3, nx=20, nt=12), dict(batch=5, nx=65, nt=7)],
+    2: [dict(batch=3, nx=24, nt=20), dict(batch=9, nx=32, nt=33), dict(batch=2, nx=101, nt=9),
+        dict(batch=3, nx=70, nt=26), dict(batch=2, nx=128, nt=128)],
+    3: [dict(batch=3, nx=24, nt=20), dict(batch=9, nx=64, nt=17), dict(batch=2, nx=77, nt=9),
+        dict(batch=2, nx=128, nt=128), dict(batch=2, nx=6, nt=5)],
+    4: [dict(batch=2, nx=12, ny=10, nt=6), dict(batch=2, nx=32, ny=16, nt=5)],
+    5: [dict(batch=3, nx=24, nt=20), dict(batch=9, nx=32, nt=33), dict(batch=2, nx=101, nt=9),
+        dict(batch=2, nx=64, nt=63), dict(batch=2, nx=256, nt=24)],
+}
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_project_parity_small(S, cfg):
+    for kw in SMALL[cfg]:
+        wl = W.make_workload(cfg, **kw)
+        g = gpu_project(S, wl, wl.u_hat)
+        assert g["norms"][:, 0].max() < 1e-10, kw
+        assert g["launches"] >= 1
+        wu, wl_ = check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
+        print(f"cfg{cfg} {kw}: rel_u {wu:.1e} rel_lam {wl_:.1e} iters {g['iters'].tolist()}")
+
+
+def test_basic_multiplier_mode(S):
+    """lambda_mode = 1: redundant multipliers pinned to 0 (R6); J^T lam is the same in both modes."""
+    for cfg in (1, 5):
+        wl = W.make_workload(cfg, **SMALL[cfg][1])
+        g = gpu_project(S, wl, wl.u_hat, params=dict(lambda_mode=1))
+        check_against_oracle(wl, wl.u_hat, g, range(wl.batch), params=dict(lambda_mode=1))
+        g0 = gpu_project(S, wl, wl.u_hat)
+        for b in range(wl.batch):
+            J = O.jacobian(wl.kind, g["u"][b], wl.params)
+            np.testing.assert_allclose(J.T @ g["lam"][b], J.T @ g0["lam"][b], rtol=0,
+                                       atol=1e-10 * max(1, np.abs(g["lam"][b]).max()))
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json sizes, launch configuration of bench.py; oracle on sampled problems, P2 on every sample
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,samples", [(2, [0, 13, 31]), (3, [0, 100, 255]), (4, [5])])
+def test_project_parity_full_size(S, cfg, samples):
+    wl = W.make_workload(cfg)
+    g = gpu_project(S, wl, wl.u_hat)
+    assert (g["iters"] > 0).all()
+    assert g["norms"][:, 0].max() < 1e-10
+    # forward-solve identity (oracle pin P2) on every sample: O(n) check, no oracle solve needed
+    err = np.abs(g["u"] - wl.u_true.numpy()).reshape(wl.batch, -1).max(1)
+    assert err.max() < 1e-10, err.max()
+    wu, wl_ = check_against_oracle(wl, wl.u_hat, g, samples)
+    print(f"cfg{cfg} full: rel_u {wu:.1e} rel_lam {wl_:.1e} iters {np.bincount(g['iters'])}")
+
+
+def test_project_parity_cfg5_full_size_tau_sequence(S):
+    """Config 5 at 256x256, batch 1024, three flow times incl. the hardest (tau = 0.02) with the
+    multiplier warm start carried between calls; oracle on one sampled problem per tau."""
+    wl = W.make_workload(5, with_u_hat=False)
+    dev = torch.device("cuda:0")
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    B = wl.batch
+    cd = wl.cdata.to(dev)
+    ut = wl.u_true.to(dev)
+    us = torch.empty(B, wl.n, dtype=torch.float64, device=dev)
+    lam = torch.zeros(B, p.m, dtype=torch.float64, device=dev)
+    it = torch.empty(B, dtype=torch.int32, device=dev)
+    ws = torch.empty(S.snap_workspace_bytes(p, B), dtype=torch.uint8, device=dev)
+    norms = torch.empty(B, 4, dtype=torch.float64, device=dev)
+    for n_call, (j, b) in enumerate([(1, 17), (25, 600), (50, 1023)]):
+        uh_cpu = W.burgers_tau_input(wl, j)
+        uh = uh_cpu.to(dev)
+        S.snap_project(p, B, uh, cd, us, lam, it, warm=n_call > 0, workspace=ws)
+        S.snap_residual(p, B, us, cd, None, norms)
+        torch.cuda.synchronize()
+        assert (it > 0).all()
+        assert float(norms[:, 0].max()) < 1e-10
+        assert float((us.view_as(ut) - ut).abs().max()) < 1e-9          # P2 on all 1024 samples
+        o = O.project(wl.kind, uh_cpu[b].numpy(), wl.cdata[b].numpy(), wl.params)
+        gu, gl = us[b].cpu().numpy().reshape(o["u"].shape), lam[b].cpu().numpy()
+        ru = np.abs(gu - o["u"]).max() / np.abs(o["u"]).max()
+        ln = np.abs(o["lam"]).max()
+        rl = np.abs(gl - o["lam"]).max() / ln if ln > 1e-9 else np.abs(gl - o["lam"]).max() * 1e4
+        print(f"cfg5 tau={j}/50 sample {b}: rel_u {ru:.1e} rel_lam {rl:.1e} iters {np.bincount(it.cpu().numpy())}")
+        assert ru <= TOL_U and rl <= TOL_L
+        if j == 50:                                                     # P7: feasible input
+            assert torch.equal(us.view_as(uh), uh)
+    p.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases
+# ------------------------------------------------------------------------------------------------
+def test_empty_batch_and_bad_arguments(S):
+    wl = W.make_workload(2, batch=1, nx=24, nt=8)
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    dev = torch.device("cuda:0")
+    e = torch.empty(0, dtype=torch.float64, device=dev)
+    S.snap_project(p, 0, e, e, e, e, torch.empty(0, dtype=torch.int32, device=dev))
+    with pytest.raises(S.SnapError):
+        S.snap_project(p, 1, wl.u_hat, wl.cdata, wl.u_hat, wl.u_hat, torch.empty(1, dtype=torch.int32))  # host tensors
+    with pytest.raises(S.SnapError):
+        S.snap_project(p, 1, wl.u_hat.to(dev), wl.cdata.to(dev), wl.u_hat.to(dev),
+                       torch.empty(p.m, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.int32, device=dev),
+                       workspace=torch.empty(16, dtype=torch.uint8, device=dev))
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_in_place_and_batch_independence(S, cfg):
+    wl = W.make_workload(cfg, **SMALL[cfg][0])
+    ref = gpu_project(S, wl, wl.u_hat)
+    inp = gpu_project(S, wl, wl.u_hat.clone(), in_place=True)
+    np.testing.assert_array_equal(inp["u"], ref["u"])
+    np.testing.assert_array_equal(inp["lam"], ref["lam"])
+    one = gpu_project(S, wl, wl.u_hat[1:2].clone())                    # sample alone == inside the batch (L106)
+    wl1 = one["u"][0]
+    if cfg == 4:
+        np.testing.assert_allclose(wl1, ref["u"][1], rtol=0, atol=1e-12)
+    else:
+        np.testing.assert_array_equal(wl1, ref["u"][1])
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_feasible_input_is_returned_bit_exact(S, cfg):
+    wl = W.make_workload(cfg, **SMALL[cfg][0])
+    g = gpu_project(S, wl, wl.u_true)
+    np.testing.assert_array_equal(g["u"], wl.u_true.numpy())
+    assert (g["iters"] == 1).all()
+    assert np.abs(g["lam"]).max() < 1e-12
+    first = gpu_project(S, wl, wl.u_hat)
+    again = gpu_project(S, wl, torch.from_numpy(first["u"]))
+    np.testing.assert_array_equal(again["u"], first["u"])              # idempotence
+
+
+def test_warm_start_does_not_change_the_result_1d(S):
+    wl = W.make_workload(5, **SMALL[5][1])
+    cold = gpu_project(S, wl, wl.u_hat)
+    lam0 = torch.from_numpy(cold["lam"]) * 3.0
+    warm = gpu_project(S, wl, wl.u_hat, warm=True, lam0=lam0)
+    np.testing.assert_array_equal(warm["u"], cold["u"])
+    np.testing.assert_array_equal(warm["lam"], cold["lam"])
+
+
+def test_warm_start_2d_reaches_the_same_point(S):
+    wl = W.make_workload(4, **SMALL[4][0])
+    cold = gpu_project(S, wl, wl.u_hat)
+    warm = gpu_project(S, wl, wl.u_hat, warm=True, lam0=torch.from_numpy(cold["lam"]))
+    np.testing.assert_allclose(warm["u"], cold["u"], rtol=0, atol=1e-11)
+    np.testing.assert_allclose(warm["lam"], cold["lam"], rtol=0, atol=1e-9 * np.abs(cold["lam"]).max())
+
+
+@pytest.mark.parametrize("precond", [0, 1, 2])
+def test_pcg_preconditioners_agree(S, precond):
+    wl = W.make_workload(4, **SMALL[4][0])
+    g = gpu_project(S, wl, wl.u_hat, params=dict(precond=precond, pcg_max=2000))
+    check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
+
+
+def test_line_search_backtracking_on_gpu(S):
+    """R17: force Armijo halving (c1 close to 1, noise 1.0); the limit point must not move."""
+    wl = W.make_workload(2, batch=2, nx=24, nt=20, noise=1.0)
+    ref = gpu_project(S, wl, wl.u_hat)
+    forced = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.99))
+    assert (forced["iters"] > ref["iters"]).all()
+    np.testing.assert_allclose(forced["u"], ref["u"], rtol=0, atol=1e-11)
+    check_against_oracle(wl, wl.u_hat, forced, range(wl.batch), params=dict(ls_c1=0.99))
+    stuck = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.99, ls_max=0))
+    assert (stuck["iters"] == -2).all()
+
+
+def test_status_codes(S):
+    wl = W.make_workload(2, batch=2, nx=16, nt=200)
+    big = wl.u_hat * 1e155
+    g = gpu_project(S, wl, big)
+    assert (g["iters"] == -3).all()                                     # R16
+    np.testing.assert_array_equal(g["u"], big.numpy())
+    assert np.all(g["lam"] == 0)
+    wl = W.make_workload(2, **SMALL[2][0])
+    g = gpu_project(S, wl, wl.u_hat, params=dict(max_iter=1))
+    assert (g["iters"] == -1).all()
+
+
+def test_host_buffer_entry_point(S):
+    wl = W.make_workload(5, **SMALL[5][1])
+    ref = gpu_project(S, wl, wl.u_hat)
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    uh = wl.u_hat.contiguous().pin_memory()
+    us = torch.empty_like(uh).pin_memory()
+    lam = torch.empty(wl.batch, p.m, dtype=torch.float64).pin_memory()
+    it = torch.empty(wl.batch, dtype=torch.int32).pin_memory()
+    S.snap_project_host(p, wl.batch, uh, wl.cdata.contiguous(), us, lam, it)
+    np.testing.assert_array_equal(us.numpy(), ref["u"])
+    np.testing.assert_array_equal(lam.numpy(), ref["lam"])
+    np.testing.assert_array_equal(it.numpy(), ref["iters"])
+    p.destroy()

@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py — projected samples/s to ||h||_inf < 1e-10 (fp64) and achieved fraction of the HBM roofline.
+
+Headline workload (BASELINE.json configs[4], "cfg5"): 1D Burgers at scale — batch 1024, 256x256,
+Lax-Friedrichs finite-volume rows + IC rows + per-level mass border rows, projected at 50 interleaved
+flow-matching times tau_j = j/50 with the multiplier warm start carried from tau to tau.
+One "step" = that whole 50-call sequence = 51 200 projections.  All 50 inputs (25.6 GB) are resident in
+HBM before the timed region, so the working set is far larger than L2 and no L2 flush is needed.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg1..cfg4] [--impl reference]
+
+Multi-GPU (torchrun): samples are independent blocks, so each rank projects its own
+batch of the same size with no data-path collective ("scaling": "weak"); NCCL carries only the barrier
+and the max-over-ranks of the device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "projected samples/sec to ||h||inf<1e-10 (fp64, 1 B200); % of HBM roofline"
+UNIT = "projections/s"
+N_TAU = 50
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            pk = json.load(f)
+        return float(pk["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def a_solve_bytes(n: int, m: int) -> int:
+    """Algorithmic bytes of one Gauss-Newton linear solve per sample:
+    forward sweep reads u, u_hat (16 n) and writes y (8 m); backward sweep reads y, u, u_hat (8 m + 16 n)
+    and writes lam, u+ (8 m + 8 n)  =>  40 n + 24 m."""
+    return 40 * n + 24 * m
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [x.strip() for x in r.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------------
+# reference arm = the oracle, as it stands, on the host cores (bounded sample)
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg: int, n_samples: int, workers: int, tau_j: int = 25):
+    """Time the CPU oracle on `n_samples` problems of workload `cfg`; returns (projections/s, seconds, desc)."""
+    import oracle as O
+    if cfg == 5:
+        wl = W.make_workload(5, batch=n_samples, with_u_hat=False)
+        uh = W.burgers_tau_input(wl, tau_j)
+        desc = f"{n_samples} samples of cfg5 (256x256, Burgers-LF + mass rows) at tau={tau_j}/{N_TAU}"
+    else:
+        wl = W.make_workload(cfg, batch=n_samples)
+        uh = wl.u_hat
+        desc = f"{n_samples} samples of cfg{cfg}"
+    t0 = time.perf_counter()
+    out = O.project_batch(wl.kind, uh.numpy(), wl.cdata.numpy(), wl.params, workers=workers)
+    dt = time.perf_counter() - t0
+    ok = bool((out["iters"] > 0).all())
+    return n_samples / dt, dt, desc + ("" if ok else " [oracle reported non-convergence]"), out["workers"]
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = int(args.workload[3:])
+    cores = os.cpu_count() or 1
+    workers = min(cores, 16)
+    n_samples = workers if cfg in (4, 5) else max(workers, 16)
+    times = []
+    desc = ""
+    for s in range(args.warmup + args.steps):
+        v, dt, desc, used = oracle_sample(cfg, n_samples, workers, tau_j=25)
+        if s >= args.warmup:
+            times.append(dt)
+    total = sum(times)
+    value = n_samples * len(times) / total
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "reference": "CPU oracle (oracle/, numpy/scipy), one step = a bounded sample"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": desc + " per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg: int) -> str:
+    return {
+        1: "cfg1: 1D heat IC+mass projection, batch 4, 64x64 (linear)",
+        2: "cfg2: 1D viscous Burgers LF projection, batch 32, 128x128",
+        3: "cfg3: 1D Fisher-KPP implicit projection, batch 256, 128x128",
+        4: "cfg4: 2D Allen-Cahn implicit projection, batch 64, 64x64x32 (PCG)",
+        5: "cfg5: 1D Burgers LF + mass rows at scale, batch 1024, 256x256, 50 flow times tau=j/50, warm-started",
+    }[cfg]
+
+
+# ------------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------------
+class GpuRun:
+    """One workload resident on the device, ready to be stepped."""
+
+    def __init__(self, S, cfg: int, dev, seed_offset: int = 0):
+        self.S, self.cfg, self.dev = S, cfg, dev
+        kind, B, nx, ny, nt, seed = W.CONFIG_SHAPES[cfg]
+        self.wl = W.make_workload(cfg, device=dev, with_u_hat=(cfg != 5), seed=seed + 1000 * seed_offset)
+        wl = self.wl
+        self.p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        self.B = wl.batch
+        if cfg == 5:
+            self.inputs = [W.burgers_tau_input(wl, j) for j in range(1, N_TAU + 1)]
+        else:
+            self.inputs = [wl.u_hat]
+        self.calls = len(self.inputs)
+        self.cdata = wl.cdata.contiguous()
+        self.u_star = torch.empty(self.B, wl.n, dtype=torch.float64, device=dev)
+        self.lam = torch.zeros(self.B, self.p.m, dtype=torch.float64, device=dev)
+        self.iters = torch.zeros(self.calls, self.B, dtype=torch.int32, device=dev)
+        self.ws = torch.empty(S.snap_workspace_bytes(self.p, self.B), dtype=torch.uint8, device=dev)
+        self.norms = torch.empty(self.B, 4, dtype=torch.float64, device=dev)
+
+    def step(self, events=None):
+        """The whole hot path over one batch of input: `calls` back-to-back snap_project launches."""
+        for c, uh in enumerate(self.inputs):
+            if events is not None:
+                events[c][0].record()
+            self.S.snap_project(self.p, self.B, uh, self.cdata, self.u_star, self.lam, self.iters[c],
+                                warm=(self.cfg == 5 and c > 0), workspace=self.ws)
+            if events is not None:
+                events[c][1].record()
+
+    def check(self):
+        """Every sample converged and the last call's output is feasible."""
+        it = self.iters.cpu()
+        self.S.snap_residual(self.p, self.B, self.u_star, self.cdata, None, self.norms)
+        hmax = float(self.norms[:, 0].max())
+        return bool((it > 0).all()), hmax, it
+
+    def projections_per_step(self):
+        return self.B * self.calls
+
+
+def time_steps(run: GpuRun, steps: int, warmup: int, dist):
+    for _ in range(warmup):
+        run.step()
+    ev = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(run.calls)]
+          for _ in range(steps)]
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    l0 = run.p.launch_count()
+    t0 = torch.cuda.Event(enable_timing=True)
+    t1 = torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for s in range(steps):
+        run.step(ev[s])
+    t1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    total_ms = t0.elapsed_time(t1)
+    launches = run.p.launch_count() - l0
+    kern_ms = [[a.elapsed_time(b) for a, b in evs] for evs in ev]
+    return total_ms, kern_ms, launches
+
+
+def e2e_steps(run: GpuRun, steps: int, warmup: int):
+    """Same metric through the host-buffer C-ABI entry: every call copies its input from pinned host memory
+    and reads u*, lam, iters back, inside the timed region."""
+    S, wl, p, B = run.S, run.wl, run.p, run.B
+    host_in = [x.cpu().pin_memory() for x in run.inputs]
+    cd = run.cdata.cpu().pin_memory()
+    us = torch.empty(B, wl.n, dtype=torch.float64).pin_memory()
+    lam = torch.zeros(B, p.m, dtype=torch.float64).pin_memory()
+    it = torch.empty(B, dtype=torch.int32).pin_memory()
+
+    def one():
+        for c, uh in enumerate(host_in):
+            S.snap_project_host(p, B, uh, cd, us, lam, it, warm=(run.cfg == 5 and c > 0))
+
+    for _ in range(warmup):
+        one()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    warm_calls = (run.calls - 1) if run.cfg == 5 else 0
+    h2d = run.calls * (B * wl.n * 8 + B * wl.nx * wl.ny * 8) + warm_calls * B * p.m * 8
+    d2h = run.calls * (B * wl.n * 8 + B * p.m * 8 + B * 4)
+    ok = bool((it > 0).all())
+    return run.projections_per_step() * steps / dt, h2d, d2h, ok
+
+
+def run_gpu(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group(backend="nccl")
+        dist = dist_mod
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    import paper_2607_00095_b200 as S
+    S.load_library()          # fails loudly if libsnap.so is missing: there is no fallback path
+
+    cfg = int(args.workload[3:])
+    run = GpuRun(S, cfg, dev, seed_offset=rank)
+    wl, p = run.wl, run.p
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    total_ms, kern_ms, launches = time_steps(run, args.steps, args.warmup, dist)
+    clocks = sampler.stop() if rank == 0 else None
+    ok, hmax, iters = run.check()
+
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t[0])
+    value = world * run.projections_per_step() * args.steps / (total_ms * 1e-3)
+
+    # roofline of the dominant kernel (the persistent projection kernel), live CUDA-event durations
+    peak, peak_src = load_peaks()
+    solves = iters.clamp(min=0).sum(dim=1).to(torch.float64)        # per call, over the batch
+    alg_bytes_call = (solves * a_solve_bytes(wl.n, p.m)).tolist()
+    if cfg == 1:
+        alg_bytes_call = [float(run.B * (16 * wl.n + 8 * p.m))]
+    kern_s = sum(sum(k) for k in kern_ms) * 1e-3
+    alg_total = sum(alg_bytes_call) * args.steps
+    achieved = alg_total / kern_s / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "batch_per_gpu": run.B, "nx": wl.nx, "ny": wl.ny, "nt": wl.nt,
+                   "calls_per_step": run.calls, "projections_per_step": world * run.projections_per_step(),
+                   "l2": "inputs (25.6 GB resident) exceed L2; no flush" if cfg == 5 else
+                         "working set smaller than L2 (latency-bound config; see DESIGN.md)",
+                   "tol": wl.params["tol"], "converged_all": ok, "max_hinf_last_call": hmax,
+                   "mean_solves_per_projection": float(solves.sum() / (run.B * run.calls))},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": args.traffic, "kernel": "project1d_kernel" if cfg != 4 else "project2d_kernel",
+                     "peak_source": peak_src, "alg_bytes_per_launch_mean": alg_total / (args.steps * run.calls),
+                     "launch_ms_mean": 1e3 * kern_s / (args.steps * run.calls),
+                     "frac_of_8TBs_spec": achieved / 8000.0},
+        "gpu_launches": launches,
+        "clocks": clocks,
+    }
+    if rank == 0 and not args.no_e2e:
+        e_val, h2d, d2h, e_ok = e2e_steps(run, max(1, min(args.steps, 2)), 1)
+        line["e2e"] = {"value": e_val * world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "converged_all": e_ok, "note": "snap_project_host: pinned host buffers, copies inside the timed region"}
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cores = os.cpu_count() or 1
+        workers = min(cores, 16)
+        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5) else max(workers, 16), workers)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle", "sample": desc,
+                                "seconds": dt}
+    if rank == 0 and world == 1 and args.others and cfg == 5:
+        others = {}
+        for c in (1, 2, 3, 4):
+            r = GpuRun(S, c, dev)
+            ms, km, _ = time_steps(r, 5, 3, None)
+            okc, hm, itc = r.check()
+            sol = float(itc.clamp(min=0).sum())
+            ab = sol * a_solve_bytes(r.wl.n, r.p.m) if c != 1 else r.B * (16 * r.wl.n + 8 * r.p.m)
+            others[f"cfg{c}"] = {"projections_per_s": r.B * 5 / (ms * 1e-3), "ms_per_call": ms / 5, "converged_all": okc,
+                                 "max_hinf": hm, "model_GBs": ab * 5 / (ms * 1e-3) / 1e9,
+                                 "note": "not HBM-resident (fits L2) / latency-bound" if c != 4 else "PCG path"}
+            del r
+        line["other_workloads"] = others
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--impl", default="snap", choices=["snap", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-others", dest="others", action="store_false")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture (profiles/)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

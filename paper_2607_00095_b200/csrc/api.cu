@@ -7,9 +7,8 @@
 #include <new>
 #include <vector>
 
-#include "kernels_1d.cuh"
-#include "kernels_2d.cuh"
 #include "kernels_misc.cuh"
+#include "launch.h"
 #include "snap_internal.h"
 
 using namespace snap;
@@ -44,17 +43,13 @@ int check_launch(snap_problem* p) {
   return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
 }
 
-struct Plan1d {
-  int q, wpc, nst, nxp, warp_bytes, grid;
-  size_t smem;
-};
-
 bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
   const int nx = p->dp.nx;
   pl.q = 1;
   while (pl.q * 32 < nx) pl.q *= 2;
   if (pl.q > 16) return false;
-  pl.nxp = (nx + 1) & ~1;
+  pl.full = (pl.q * 32 == nx);
+  pl.rp = ((nx + 1) & ~1) + 4;  // [pad, halo, data(nx), halo, pad], data start 16-byte aligned
   const int sms = p->sm_count > 0 ? p->sm_count : 148;
   int wpc = (batch + sms - 1) / sms;
   if (wpc < 1) wpc = 1;
@@ -62,7 +57,7 @@ bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
   const size_t limit = (size_t)p->max_smem_optin;
   for (;; --wpc) {
     for (int nst = 4; nst >= 2; --nst) {
-      const size_t wb = align_up((size_t)(3 * nst + 5) * pl.nxp * 8 + (size_t)nst * 8, 128);
+      const size_t wb = align_up((size_t)(3 * nst + 5) * pl.rp * 8 + (size_t)nst * 8, 128);
       if (wb * wpc <= limit) {
         pl.wpc = wpc; pl.nst = nst; pl.warp_bytes = (int)wb; pl.smem = wb * wpc;
         pl.grid = (batch + wpc - 1) / wpc;
@@ -71,27 +66,6 @@ bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
     }
     if (wpc == 1) return false;
   }
-}
-
-template <int KIND, int Q>
-int launch_1d_t(snap_problem* p, const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
-  auto kern = project1d_kernel<KIND, Q>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
-    return SNAP_ECUDA;
-  kern<<<pl.grid, pl.wpc * 32, pl.smem, st>>>(a);
-  return check_launch(p);
-}
-
-template <int KIND>
-int launch_1d_k(snap_problem* p, const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
-  switch (pl.q) {
-    case 1: return launch_1d_t<KIND, 1>(p, a, pl, st);
-    case 2: return launch_1d_t<KIND, 2>(p, a, pl, st);
-    case 4: return launch_1d_t<KIND, 4>(p, a, pl, st);
-    case 8: return launch_1d_t<KIND, 8>(p, a, pl, st);
-    case 16: return launch_1d_t<KIND, 16>(p, a, pl, st);
-  }
-  return SNAP_EINVAL;
 }
 
 bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
@@ -232,12 +206,14 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   a.bufA = reinterpret_cast<double*>(w);
   a.bufB = reinterpret_cast<double*>(w + field);
   a.aux = reinterpret_cast<double*>(w + 2 * field);
-  a.nst = pl.nst; a.nxp = pl.nxp; a.warp_bytes = pl.warp_bytes;
+  a.nst = pl.nst; a.rp = pl.rp; a.warp_bytes = pl.warp_bytes;
   // bulk (TMA) copies need every row start 16-byte aligned
-  a.tma = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
-          aligned16(lambda) && aligned16(a.bufA);
-  if (d.kind == SNAP_FISHER1D_IE) return launch_1d_k<KF>(p, a, pl, st);
-  return launch_1d_k<KB>(p, a, pl, st);
+  pl.tma = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
+           aligned16(lambda) && aligned16(a.bufA);
+  if (!pl.tma) pl.full = false;  // the plain-load path is only instantiated with bounds checks
+  p->launches++;
+  if (d.kind == SNAP_FISHER1D_IE) return launch_project1d_fisher(a, pl, st);
+  return launch_project1d_burgers(a, pl, st);
 }
 
 int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, const double* cdata_host,

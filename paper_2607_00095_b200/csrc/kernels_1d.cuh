@@ -12,6 +12,7 @@
 // from the shared-memory rows (halo staging), reductions are fixed-order warp shuffles.
 #pragma once
 #include "device_utils.cuh"
+#include "launch.h"
 #include "snap_internal.h"
 
 namespace snap {
@@ -19,42 +20,31 @@ namespace snap {
 constexpr int KB = 1;  // Burgers family: lane owns cells lane + 32 j   (conflict-free shared-memory access)
 constexpr int KF = 2;  // Fisher family:  lane owns cells lane*Q + j    (contiguous, for the warp tridiagonal solve)
 
-struct Proj1dArgs {
-  DevParams P;
-  int batch, warm;
-  const double* u_hat;
-  const double* cdata;
-  double* u_star;
-  double* lam;
-  int* iters;
-  double* bufA;  // [batch][n]  trial / iterate ping-pong
-  double* bufB;  // [batch][n]
-  double* aux;   // [batch][2*nt]  level sums and null-space coefficients (min-norm multiplier, kind 4)
-  int nst;       // ring depth (levels in flight per warp)
-  int nxp;       // row pitch in doubles (nx rounded up to even)
-  int tma;       // 1: rows are 16-byte aligned -> bulk copies; 0: plain loads/stores
-  int warp_bytes;
-};
 
 // ------------------------------------------------------------------------------------------------
-// per-warp row pipeline
+// per-warp row pipeline.  A row buffer is [pad, halo_left, data[0..nx), halo_right, pad] with the data
+// start 16-byte aligned (bulk-copy destination); the halo cells hold the periodic (Burgers) or mirrored
+// (Fisher, Neumann) neighbours so that every stencil access is base[i +- 1] with no index arithmetic.
 // ------------------------------------------------------------------------------------------------
+constexpr int kHalo = 2;  // doubles in front of the data start
+
+template <bool TMA>
 struct Pipe {
-  double* stage;   // [nst][3][nxp]
-  double* srow;    // [5][nxp]
+  double* stage;   // [nst][3][rp]
+  double* srow;    // [5][rp]
   uint32_t bar0;   // shared address of mbarrier 0
   uint32_t phase;  // parity to wait for, one bit per stage
-  int nst, nxp, nx, tma, lane;
+  int nst, rp, nx, lane;
 
-  __device__ __forceinline__ double* row(int s, int r) const { return stage + (size_t)(s * 3 + r) * nxp; }
-  __device__ __forceinline__ double* out(int r) const { return srow + (size_t)r * nxp; }
+  __device__ __forceinline__ double* row(int s, int r) const { return stage + (size_t)(s * 3 + r) * rp + kHalo; }
+  __device__ __forceinline__ double* out(int r) const { return srow + (size_t)r * rp + kHalo; }
 
   // Load up to three global rows of nx doubles into stage s.  Called by the whole (converged) warp after
   // every lane has finished reading the previous contents of the stage.
   __device__ __forceinline__ void issue(int s, const double* g0, const double* g1, const double* g2) {
     __syncwarp();
     const uint32_t bar = bar0 + 8u * s;
-    if (tma) {
+    if (TMA) {
       if (lane == 0) {
         const uint32_t rb = (uint32_t)nx * 8u;
         mbar_expect_tx(bar, rb * (g2 ? 3u : 2u));
@@ -79,21 +69,29 @@ struct Pipe {
     mbar_wait(bar0 + 8u * s, (phase >> s) & 1u);
     phase ^= (1u << s);
   }
-  // make the shared-memory output rows written >= 2 steps ago reusable
-  __device__ __forceinline__ void out_reuse() {
-    if (tma && lane == 0) bulk_wait_read<1>();
+  // After wait(): fill the halo of a freshly landed row (periodic or mirror) and make the shared-memory
+  // output rows written >= 2 steps ago reusable; ends with a warp barrier.
+  template <bool PERIODIC>
+  __device__ __forceinline__ void ready(double* halo_row) {
+    if (lane == 0) {
+      if (halo_row) {
+        halo_row[-1] = PERIODIC ? halo_row[nx - 1] : halo_row[0];
+        halo_row[nx] = PERIODIC ? halo_row[0] : halo_row[nx - 1];
+      }
+      if (TMA) bulk_wait_read<1>();
+    }
     __syncwarp();
   }
   // lanes have written an output row with generic stores; hand it to the bulk-store engine
   __device__ __forceinline__ void store_row(double* g, const double* s_row) {
-    if (tma && lane == 0) bulk_s2g(g, smem_u32(s_row), (uint32_t)nx * 8u);
+    if (TMA && lane == 0) bulk_s2g(g, smem_u32(s_row), (uint32_t)nx * 8u);
   }
   __device__ __forceinline__ void commit() {
-    if (tma && lane == 0) bulk_commit();
+    if (TMA && lane == 0) bulk_commit();
   }
   // all outstanding bulk stores of this warp are complete and visible to later loads
   __device__ __forceinline__ void drain() {
-    if (tma) {
+    if (TMA) {
       if (lane == 0) {
         bulk_wait_all<0>();
         fence_proxy_async_all();
@@ -109,11 +107,6 @@ struct SweepNorms {
   double hinf, h1, f;  // ||h||_inf, ||h||_1, 1/2 ||u - u_hat||^2
   int bad;             // non-finite residual seen
 };
-
-template <int KIND, int Q>
-__device__ __forceinline__ int cell(int lane, int j) {
-  return KIND == KB ? lane + 32 * j : lane * Q + j;
-}
 
 // ------------------------------------------------------------------------------------------------
 // warp tridiagonal solve (Fisher): rows owned contiguously, Q per lane; partition method —
@@ -219,108 +212,74 @@ __device__ __forceinline__ void fisher_matrix(const DevParams& P, const double (
 // ------------------------------------------------------------------------------------------------
 // forward sweep: residual h (a1), Jacobian coefficients (a2), rhs (a3) and L y = r (a5), level by level.
 // Reads u (point of linearisation) and u_hat rows, writes y into the multiplier buffer.
+//
+// Burgers family (lane owns cells lane + 32 j).  With q = y + (u - u_hat) the recurrence L y = r reads
+//     q_0 = h_0 ,   q_k = h_k + A_{k-1} q_{k-1} ,   h_k = u[k] - Phi(u[k-1]) ,   y_k = q_k - (u[k] - u_hat[k])
+// Phi(u[k-1])_i and the two off-diagonal coefficients of A_{k-1} are computed while level k-1 is in shared
+// memory and carried in registers, so a stage is free for refill as soon as its level has been processed.
 // ------------------------------------------------------------------------------------------------
-template <int KIND, int Q>
-__device__ void fwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict__ u, const double* __restrict__ uh,
-                          const double* __restrict__ u0, double* __restrict__ y, double M0, SweepNorms& out) {
+template <int Q, bool FULL, bool TMA>
+__device__ void fwd_sweep_b(const DevParams& P, Pipe<TMA>& pp, const double* __restrict__ u,
+                            const double* __restrict__ uh, const double* __restrict__ u0, double* __restrict__ y,
+                            double M0, SweepNorms& out) {
   const int nx = P.nx, nt = P.nt, lane = pp.lane, nst = pp.nst;
+  const double a0 = P.bs_a0, e = P.bs_e, qs = P.bs_qs, hs = P.bs_hs;
   double hinf = 0.0, h1 = 0.0, f2 = 0.0, minf = 0.0, m1 = 0.0;
-  int bad = 0;
-  double u0r[Q], qo[Q];
-  double phi[Q], cpj[Q], cmj[Q];  // Burgers: Phi(u[k-1])_i and dPhi_i/du_{i+-1}, carried one level
-  double upr[Q];                  // Fisher: u[k-1] own cells
+  double qo[Q], phi[Q], cpj[Q], cmj[Q];
 #pragma unroll
   for (int j = 0; j < Q; ++j) {
-    const int i = cell<KIND, Q>(lane, j);
-    u0r[j] = (i < nx) ? u0[i] : 0.0;
-    qo[j] = 0.0; phi[j] = 0.0; cpj[j] = 0.0; cmj[j] = 0.0; upr[j] = 0.0;
+    const int i = lane + 32 * j;
+    phi[j] = (FULL || i < nx) ? u0[i] : 0.0;  // level 0: h_0 = u[0] - u0
+    qo[j] = 0.0; cpj[j] = 0.0; cmj[j] = 0.0;
   }
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, u + (size_t)k * nx, uh + (size_t)k * nx, nullptr);
+  // q_{-1} = 0: level 0 runs the general recurrence with zero coefficients, so the slot it reads must be finite
+  {
+    double* z = pp.out(3) - 1;
+    for (int i = lane; i < nx + 2; i += 32) z[i] = 0.0;
+  }
   int s = 0;
   for (int k = 0; k < nt; ++k) {
     pp.wait(s);
-    pp.out_reuse();
-    const double* su = pp.row(s, 0);
-    const double* sh = pp.row(s, 1);
-    double* yo = pp.out(k & 1);
-    double* qc = pp.out(2 + (k & 1));
-    const double* qp = pp.out(2 + ((k + 1) & 1));
+    double* su0 = pp.row(s, 0);
+    pp.template ready<true>(su0);
+    const double* su = su0 + lane;
+    const double* sh = pp.row(s, 1) + lane;
+    double* yo0 = pp.out(k & 1);
+    double* qc0 = pp.out(2 + (k & 1));
+    double* yo = yo0 + lane;
+    double* qc = qc0 + lane;
+    const double* qp = pp.out(2 + ((k + 1) & 1)) + lane;   // q_{k-1} (zero coefficients at k = 0)
     double* yg = y + (size_t)k * nx;
     double msum = 0.0;
-    if (KIND == KB) {
 #pragma unroll
-      for (int j = 0; j < Q; ++j) {
-        const int i = lane + 32 * j;
-        if (i < nx) {
-          const int ip = (i + 1 == nx) ? 0 : i + 1;
-          const int im = (i == 0) ? nx - 1 : i - 1;
-          const double uk = su[i], uhk = sh[i], up = su[ip], um = su[im];
-          double h, q;
-          if (k == 0) {
-            h = uk - u0r[j];
-            q = h;
-          } else {
-            h = uk - phi[j];
-            q = fma(cpj[j], qp[ip], fma(cmj[j], qp[im], fma(P.bs_a0, qo[j], h)));
-          }
-          const double w = uk - uhk;
-          const double yv = q - w;
-          qc[i] = q;
-          if (pp.tma) yo[i] = yv; else yg[i] = yv;
-          const double ah = fabs(h);
-          bad |= !finite_d(ah) | !finite_d(q);
-          hinf = fmax(hinf, ah);
-          h1 += ah;
-          f2 = fma(w, w, f2);
-          msum += uk;
-          phi[j] = fma(P.bs_a0, uk, (up + um) * fma(-P.bs_qs, up - um, P.bs_e));
-          cpj[j] = fma(-P.bs_hs, up, P.bs_e);
-          cmj[j] = fma(P.bs_hs, um, P.bs_e);
-          qo[j] = q;
-        }
-      }
-    } else {
-      double uk[Q], uhk[Q], rhs[Q], a[Q], b[Q], c[Q], hv[Q];
-#pragma unroll
-      for (int j = 0; j < Q; ++j) {
-        const int i = lane * Q + j;
-        if (i < nx) {
-          uk[j] = su[i];
-          uhk[j] = sh[i];
-          if (k == 0) {
-            hv[j] = uk[j] - u0r[j];
-          } else {
-            const double ul = (i > 0) ? su[i - 1] : uk[j];
-            const double ur = (i < nx - 1) ? su[i + 1] : uk[j];
-            // h = u[k] - u[k-1] - dt (D Lap u[k] + rho u[k](1-u[k]))
-            hv[j] = uk[j] - upr[j] - P.fi_a * ((ul - uk[j]) + (ur - uk[j])) - P.fi_dtrho * uk[j] * (1.0 - uk[j]);
-          }
-          rhs[j] = hv[j] + qo[j];
+    for (int j = 0; j < Q; ++j) {
+      const int o = 32 * j;
+      if (FULL || lane + o < nx) {
+        const double uk = su[o], uhk = sh[o], up = su[o + 1], um = su[o - 1];
+        const double h = uk - phi[j];
+        const double q = fma(cpj[j], qp[o + 1], fma(cmj[j], qp[o - 1], fma(a0, qo[j], h)));
+        const double w = uk - uhk;
+        const double yv = q - w;
+        qc[o] = q;
+        if (FULL) {
+          if (j == 0 && lane == 0) qc0[nx] = q;
+          if (j == Q - 1 && lane == 31) qc0[-1] = q;
         } else {
-          uk[j] = 0.0; uhk[j] = 0.0; hv[j] = 0.0; rhs[j] = 0.0;
+          if (lane + o == 0) qc0[nx] = q;
+          if (lane + o == nx - 1) qc0[-1] = q;
         }
-      }
-      if (k > 0) {
-        fisher_matrix<Q>(P, uk, lane, a, b, c);
-        warp_tridiag<Q>(a, b, c, rhs, lane);
-      }
-#pragma unroll
-      for (int j = 0; j < Q; ++j) {
-        const int i = lane * Q + j;
-        if (i < nx) {
-          const double q = rhs[j];
-          const double w = uk[j] - uhk[j];
-          const double yv = q - w;
-          if (pp.tma) yo[i] = yv; else yg[i] = yv;
-          const double ah = fabs(hv[j]);
-          bad |= !finite_d(ah) | !finite_d(q);
-          hinf = fmax(hinf, ah);
-          h1 += ah;
-          f2 = fma(w, w, f2);
-          qo[j] = q;
-          upr[j] = uk[j];
-        }
+        if (TMA) yo[o] = yv; else yg[lane + o] = yv;
+        const double ah = fabs(h);
+        hinf = fmax(hinf, ah);
+        h1 += ah;
+        f2 = fma(w, w, f2);
+        msum += uk;
+        phi[j] = fma(a0, uk, (up + um) * fma(-qs, up - um, e));
+        cpj[j] = fma(-hs, up, e);
+        cmj[j] = fma(hs, um, e);
+        qo[j] = q;
       }
     }
     if (P.has_mass) {
@@ -328,7 +287,91 @@ __device__ void fwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict
       minf = fmax(minf, hm);
       m1 += hm;
     }
-    if (pp.tma) fence_proxy_async_smem();
+    if (TMA) fence_proxy_async_smem();
+    __syncwarp();
+    pp.store_row(yg, yo0);
+    pp.commit();
+    if (k + nst < nt) pp.issue(s, u + (size_t)(k + nst) * nx, uh + (size_t)(k + nst) * nx, nullptr);
+    if (++s == nst) s = 0;
+  }
+  pp.drain();
+  hinf = warp_max(hinf);
+  h1 = warp_sum(h1);
+  f2 = warp_sum(f2);
+  if (P.has_mass) {
+    hinf = fmax(hinf, minf);
+    h1 += m1;
+  }
+  out.hinf = hinf;
+  out.h1 = h1;
+  out.f = 0.5 * f2;
+  // fmax drops NaN; the sums do not: a non-finite residual or iterate shows up in h1 / f2
+  out.bad = !finite_d(hinf) | !finite_d(h1) | !finite_d(f2);
+}
+
+// Fisher family (lane owns cells lane*Q + j):  q_0 = h_0 ,  T_k q_k = h_k + q_{k-1} ,  y_k = q_k - (u[k]-u_hat[k]).
+template <int Q, bool TMA>
+__device__ void fwd_sweep_f(const DevParams& P, Pipe<TMA>& pp, const double* __restrict__ u,
+                            const double* __restrict__ uh, const double* __restrict__ u0, double* __restrict__ y,
+                            SweepNorms& out) {
+  const int nx = P.nx, nt = P.nt, lane = pp.lane, nst = pp.nst;
+  double hinf = 0.0, h1 = 0.0, f2 = 0.0;
+  double u0r[Q], qo[Q], upr[Q];
+#pragma unroll
+  for (int j = 0; j < Q; ++j) {
+    const int i = lane * Q + j;
+    u0r[j] = (i < nx) ? u0[i] : 0.0;
+    qo[j] = 0.0; upr[j] = 0.0;
+  }
+  const int npro = nst < nt ? nst : nt;
+  for (int k = 0; k < npro; ++k) pp.issue(k, u + (size_t)k * nx, uh + (size_t)k * nx, nullptr);
+  int s = 0;
+  for (int k = 0; k < nt; ++k) {
+    pp.wait(s);
+    double* su = pp.row(s, 0);
+    pp.template ready<false>(su);
+    const double* sh = pp.row(s, 1);
+    double* yo = pp.out(k & 1);
+    double* yg = y + (size_t)k * nx;
+    double uk[Q], uhk[Q], rhs[Q], a[Q], b[Q], c[Q], hv[Q];
+#pragma unroll
+    for (int j = 0; j < Q; ++j) {
+      const int i = lane * Q + j;
+      if (i < nx) {
+        uk[j] = su[i];
+        uhk[j] = sh[i];
+        if (k == 0) {
+          hv[j] = uk[j] - u0r[j];
+        } else {  // h = u[k] - u[k-1] - dt (D Lap u[k] + rho u[k](1-u[k])); mirrored halo = Neumann ghost cells
+          hv[j] = uk[j] - upr[j] - P.fi_a * ((su[i - 1] - uk[j]) + (su[i + 1] - uk[j])) -
+                  P.fi_dtrho * uk[j] * (1.0 - uk[j]);
+        }
+        rhs[j] = hv[j] + qo[j];
+      } else {
+        uk[j] = 0.0; uhk[j] = 0.0; hv[j] = 0.0; rhs[j] = 0.0;
+      }
+    }
+    if (k > 0) {
+      fisher_matrix<Q>(P, uk, lane, a, b, c);
+      warp_tridiag<Q>(a, b, c, rhs, lane);
+    }
+#pragma unroll
+    for (int j = 0; j < Q; ++j) {
+      const int i = lane * Q + j;
+      if (i < nx) {
+        const double q = rhs[j];
+        const double w = uk[j] - uhk[j];
+        const double yv = q - w;
+        if (TMA) yo[i] = yv; else yg[i] = yv;
+        const double ah = fabs(hv[j]);
+        hinf = fmax(hinf, ah);
+        h1 += ah;
+        f2 = fma(w, w, f2);
+        qo[j] = q;
+        upr[j] = uk[j];
+      }
+    }
+    if (TMA) fence_proxy_async_smem();
     __syncwarp();
     pp.store_row(yg, yo);
     pp.commit();
@@ -339,29 +382,25 @@ __device__ void fwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict
   hinf = warp_max(hinf);
   h1 = warp_sum(h1);
   f2 = warp_sum(f2);
-  bad = warp_or(bad);
-  if (P.has_mass) {
-    bad |= !finite_d(minf);
-    hinf = fmax(hinf, minf);
-    h1 += m1;
-  }
   out.hinf = hinf;
   out.h1 = h1;
   out.f = 0.5 * f2;
-  out.bad = bad | !finite_d(hinf) | !finite_d(h1) | !finite_d(f2);
+  out.bad = !finite_d(hinf) | !finite_d(h1) | !finite_d(f2);
 }
 
 // ------------------------------------------------------------------------------------------------
 // backward sweep: L^T lam = y (a5) and the step u+ = u_hat - J^T lam = u_hat - y (a8).
 //   mode 0: write the trial point u+ to `unew`;  mode 1 (final solve): write the current iterate u to
 //   `unew` (= u_star), lam only.  sig != nullptr: also store the level sums of lam (min-norm correction).
-// Returns ||lam||_inf and (u - u_hat)^T d, d = u+ - u.
+// Returns ||lam||_inf (NaN if anything was non-finite) and (u - u_hat)^T d, d = u+ - u.
+// Burgers:  lam_{nt-1} = y_{nt-1} ,  lam_k = y_k + A_k^T lam_{k+1}   (A_k^T needs only u[k] at the own cell).
 // ------------------------------------------------------------------------------------------------
-template <int KIND, int Q>
-__device__ void bwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict__ u, const double* __restrict__ uh,
-                          double* __restrict__ lam, double* __restrict__ unew, int mode, double* __restrict__ sig,
-                          double& linf_out, double& wd_out) {
+template <int Q, bool FULL, bool TMA>
+__device__ void bwd_sweep_b(const DevParams& P, Pipe<TMA>& pp, const double* __restrict__ u,
+                            const double* __restrict__ uh, double* __restrict__ lam, double* __restrict__ unew,
+                            int mode, double* __restrict__ sig, double& linf_out, double& wd_out) {
   const int nx = P.nx, nt = P.nt, lane = pp.lane, nst = pp.nst;
+  const double a0 = P.bs_a0, e = P.bs_e, hs = P.bs_hs;
   double linf = 0.0, wd = 0.0;
   double lo[Q];
 #pragma unroll
@@ -371,80 +410,58 @@ __device__ void bwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict
     const size_t o = (size_t)(nt - 1 - t) * nx;
     pp.issue(t, lam + o, u + o, uh + o);
   }
+  // lam_{nt} = 0: clear the ring slot the first step reads its neighbours from
+  {
+    double* z = pp.out(2) - 1;
+    for (int i = lane; i < nx + 2; i += 32) z[i] = 0.0;
+  }
   int s = 0, r3 = 0;
   for (int t = 0; t < nt; ++t) {
     const int k = nt - 1 - t;
     pp.wait(s);
-    pp.out_reuse();
-    const double* sy = pp.row(s, 0);
-    const double* su = pp.row(s, 1);
-    const double* sh = pp.row(s, 2);
-    double* lc = pp.out(r3);
-    const double* lp = pp.out(r3 == 0 ? 2 : r3 - 1);
-    double* uo = pp.out(3 + (t & 1));
+    pp.template ready<true>(nullptr);
+    const double* sy = pp.row(s, 0) + lane;
+    const double* su = pp.row(s, 1) + lane;
+    const double* sh = pp.row(s, 2) + lane;
+    double* lc0 = pp.out(r3);
+    double* lc = lc0 + lane;
+    const double* lp = pp.out(r3 == 0 ? 2 : r3 - 1) + lane;
+    double* uo0 = pp.out(3 + (t & 1));
+    double* uo = uo0 + lane;
     double* lg = lam + (size_t)k * nx;
     double* ug = unew + (size_t)k * nx;
     double lsum = 0.0;
-    if (KIND == KB) {
 #pragma unroll
-      for (int j = 0; j < Q; ++j) {
-        const int i = lane + 32 * j;
-        if (i < nx) {
-          const int ip = (i + 1 == nx) ? 0 : i + 1;
-          const int im = (i == 0) ? nx - 1 : i - 1;
-          const double yv = sy[i], v = su[i], uhk = sh[i];
-          double l = yv;
-          if (t > 0)  // lam_k = y_k + A_k^T lam_{k+1}
-            l = fma(fma(-P.bs_hs, v, P.bs_e), lp[im], fma(fma(P.bs_hs, v, P.bs_e), lp[ip], fma(P.bs_a0, lo[j], yv)));
-          lc[i] = l;
-          const double un = (mode == 0) ? (uhk - yv) : v;
-          if (pp.tma) uo[i] = un; else { lg[i] = l; ug[i] = un; }
-          const double w = v - uhk;
-          wd = fma(w, (uhk - yv) - v, wd);
-          linf = fmax(linf, fabs(l));
-          lsum += l;
-          lo[j] = l;
-        }
-      }
-    } else {
-      double uk[Q], yv[Q], uhk[Q], rhs[Q], a[Q], b[Q], c[Q];
-#pragma unroll
-      for (int j = 0; j < Q; ++j) {
-        const int i = lane * Q + j;
-        if (i < nx) {
-          yv[j] = sy[i]; uk[j] = su[i]; uhk[j] = sh[i];
-          rhs[j] = yv[j] + lo[j];
+    for (int j = 0; j < Q; ++j) {
+      const int o = 32 * j;
+      if (FULL || lane + o < nx) {
+        const double yv = sy[o], v = su[o], uhk = sh[o];
+        const double l = fma(fma(-hs, v, e), lp[o - 1], fma(fma(hs, v, e), lp[o + 1], fma(a0, lo[j], yv)));
+        lc[o] = l;
+        if (FULL) {
+          if (j == 0 && lane == 0) lc0[nx] = l;
+          if (j == Q - 1 && lane == 31) lc0[-1] = l;
         } else {
-          yv[j] = 0.0; uk[j] = 0.0; uhk[j] = 0.0; rhs[j] = 0.0;
+          if (lane + o == 0) lc0[nx] = l;
+          if (lane + o == nx - 1) lc0[-1] = l;
         }
-      }
-      if (k > 0) {  // T_k lam_k = y_k + lam_{k+1}   (level 0: identity block)
-        fisher_matrix<Q>(P, uk, lane, a, b, c);
-        warp_tridiag<Q>(a, b, c, rhs, lane);
-      }
-#pragma unroll
-      for (int j = 0; j < Q; ++j) {
-        const int i = lane * Q + j;
-        if (i < nx) {
-          const double l = rhs[j];
-          const double un = (mode == 0) ? (uhk[j] - yv[j]) : uk[j];
-          if (pp.tma) { lc[i] = l; uo[i] = un; } else { lg[i] = l; ug[i] = un; }
-          const double w = uk[j] - uhk[j];
-          wd = fma(w, (uhk[j] - yv[j]) - uk[j], wd);
-          linf = fmax(linf, fabs(l));
-          lsum += l;
-          lo[j] = l;
-        }
+        const double step = uhk - yv;
+        const double un = (mode == 0) ? step : v;
+        if (TMA) uo[o] = un; else { lg[lane + o] = l; ug[lane + o] = un; }
+        wd = fma(v - uhk, step - v, wd);
+        linf = fmax(linf, fabs(l));
+        lsum += l;
+        lo[j] = l;
       }
     }
     if (sig) {
       const double sk = warp_sum(lsum);
       if (lane == 0) sig[k] = sk;
     }
-    if (pp.tma) fence_proxy_async_smem();
+    if (TMA) fence_proxy_async_smem();
     __syncwarp();
-    pp.store_row(lg, lc);
-    pp.store_row(ug, uo);
+    pp.store_row(lg, lc0);
+    pp.store_row(ug, uo0);
     pp.commit();
     if (t + nst < nt) {
       const size_t o = (size_t)(k - nst) * nx;
@@ -456,7 +473,80 @@ __device__ void bwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict
   pp.drain();
   linf = warp_max(linf);
   wd = warp_sum(wd);
-  // fmax drops NaN: detect a non-finite multiplier through the sum as well
+  // fmax drops NaN: detect a non-finite multiplier / step through the sum as well
+  linf_out = finite_d(wd) ? linf : __longlong_as_double(0x7ff8000000000000LL);
+  wd_out = wd;
+}
+
+// Fisher:  T_k lam_k = y_k + lam_{k+1}  (k >= 1, T symmetric) ,  lam_0 = y_0 + lam_1.
+template <int Q, bool TMA>
+__device__ void bwd_sweep_f(const DevParams& P, Pipe<TMA>& pp, const double* __restrict__ u,
+                            const double* __restrict__ uh, double* __restrict__ lam, double* __restrict__ unew,
+                            int mode, double& linf_out, double& wd_out) {
+  const int nx = P.nx, nt = P.nt, lane = pp.lane, nst = pp.nst;
+  double linf = 0.0, wd = 0.0;
+  double lo[Q];
+#pragma unroll
+  for (int j = 0; j < Q; ++j) lo[j] = 0.0;
+  const int npro = nst < nt ? nst : nt;
+  for (int t = 0; t < npro; ++t) {
+    const size_t o = (size_t)(nt - 1 - t) * nx;
+    pp.issue(t, lam + o, u + o, uh + o);
+  }
+  int s = 0;
+  for (int t = 0; t < nt; ++t) {
+    const int k = nt - 1 - t;
+    pp.wait(s);
+    pp.template ready<false>(nullptr);
+    const double* sy = pp.row(s, 0);
+    const double* su = pp.row(s, 1);
+    const double* sh = pp.row(s, 2);
+    double* lc = pp.out(t & 1);
+    double* uo = pp.out(3 + (t & 1));
+    double* lg = lam + (size_t)k * nx;
+    double* ug = unew + (size_t)k * nx;
+    double uk[Q], yv[Q], uhk[Q], rhs[Q], a[Q], b[Q], c[Q];
+#pragma unroll
+    for (int j = 0; j < Q; ++j) {
+      const int i = lane * Q + j;
+      if (i < nx) {
+        yv[j] = sy[i]; uk[j] = su[i]; uhk[j] = sh[i];
+        rhs[j] = yv[j] + lo[j];
+      } else {
+        yv[j] = 0.0; uk[j] = 0.0; uhk[j] = 0.0; rhs[j] = 0.0;
+      }
+    }
+    if (k > 0) {
+      fisher_matrix<Q>(P, uk, lane, a, b, c);
+      warp_tridiag<Q>(a, b, c, rhs, lane);
+    }
+#pragma unroll
+    for (int j = 0; j < Q; ++j) {
+      const int i = lane * Q + j;
+      if (i < nx) {
+        const double l = rhs[j];
+        const double step = uhk[j] - yv[j];
+        const double un = (mode == 0) ? step : uk[j];
+        if (TMA) { lc[i] = l; uo[i] = un; } else { lg[i] = l; ug[i] = un; }
+        wd = fma(uk[j] - uhk[j], step - uk[j], wd);
+        linf = fmax(linf, fabs(l));
+        lo[j] = l;
+      }
+    }
+    if (TMA) fence_proxy_async_smem();
+    __syncwarp();
+    pp.store_row(lg, lc);
+    pp.store_row(ug, uo);
+    pp.commit();
+    if (t + nst < nt) {
+      const size_t o = (size_t)(k - nst) * nx;
+      pp.issue(s, lam + o, u + o, uh + o);
+    }
+    if (++s == nst) s = 0;
+  }
+  pp.drain();
+  linf = warp_max(linf);
+  wd = warp_sum(wd);
   linf_out = finite_d(wd) ? linf : __longlong_as_double(0x7ff8000000000000LL);
   wd_out = wd;
 }
@@ -465,7 +555,7 @@ __device__ void bwd_sweep(const DevParams& P, Pipe& pp, const double* __restrict
 // recipe): with level sums sigma_j of the basic solution (mass multipliers 0) and c = nx dx^2,
 //   (D^T D + c I) t = -dx D^T sigma     [ <=> (I + c L1 L1^T) t = N lam_basic ; D = L1^{-1} first difference ]
 //   lam_mass[k] = -t_k ;  lam_loc[j][.] += dx sum_{k>=j} t_k .
-__device__ void min_norm_burgers_mass(const DevParams& P, int lane, double* __restrict__ lam, double* __restrict__ sig,
+static __device__ void min_norm_burgers_mass(const DevParams& P, int lane, double* __restrict__ lam, double* __restrict__ sig,
                                       double* __restrict__ tt) {
   const int nx = P.nx, nt = P.nt;
   const double c = (double)nx * P.dx * P.dx;
@@ -507,7 +597,7 @@ __device__ void min_norm_burgers_mass(const DevParams& P, int lane, double* __re
 // ------------------------------------------------------------------------------------------------
 // the persistent Gauss-Newton driver (a8, a9): one warp per sample
 // ------------------------------------------------------------------------------------------------
-template <int KIND, int Q>
+template <int KIND, int Q, bool FULL, bool TMA>
 __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ Proj1dArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const DevParams& P = A.P;
@@ -518,17 +608,19 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
   const size_t n = (size_t)P.n;
 
   unsigned char* base = smem_raw + (size_t)warp * A.warp_bytes;
-  Pipe pp;
+  Pipe<TMA> pp;
   pp.stage = reinterpret_cast<double*>(base);
-  pp.srow = pp.stage + (size_t)A.nst * 3 * A.nxp;
-  pp.bar0 = smem_u32(pp.srow + (size_t)5 * A.nxp);
+  pp.srow = pp.stage + (size_t)A.nst * 3 * A.rp;
+  pp.bar0 = smem_u32(pp.srow + (size_t)5 * A.rp);
   pp.phase = 0;
-  pp.nst = A.nst; pp.nxp = A.nxp; pp.nx = nx; pp.tma = A.tma; pp.lane = lane;
+  pp.nst = A.nst; pp.rp = A.rp; pp.nx = nx; pp.lane = lane;
   if (lane == 0) {
     for (int s = 0; s < A.nst; ++s) mbar_init(pp.bar0 + 8u * s, 1);
     mbar_fence_init();
     fence_proxy_async_smem();
   }
+  // zero the output/staging rows once: halo cells and q_{-1} must read as finite zeros
+  for (int i = lane; i < 5 * A.rp; i += 32) pp.srow[i] = 0.0;
   __syncwarp();
 
   const double* uh = A.u_hat + (size_t)b * n;
@@ -564,7 +656,8 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
 
   while (true) {
     const double* pt = have_trial ? trial : cur;
-    fwd_sweep<KIND, Q>(P, pp, pt, uh, u0, lam, M0, nrm);
+    if (KIND == KB) fwd_sweep_b<Q, FULL, TMA>(P, pp, pt, uh, u0, lam, M0, nrm);
+    else fwd_sweep_f<Q, TMA>(P, pp, pt, uh, u0, lam, nrm);
     if (have_trial) {
       if (!polishing) {
         const double phi_t = nrm.f + mu * nrm.h1;
@@ -601,11 +694,13 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
     }
     double linf, wd;
     if (final_solve) {
-      bwd_sweep<KIND, Q>(P, pp, cur, uh, lam, ustar, 1, want_sig ? sig : nullptr, linf, wd);
+      if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, ustar, 1, want_sig ? sig : nullptr, linf, wd);
+      else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, ustar, 1, linf, wd);
       if (!finite_d(linf)) status = SNAP_ST_NONFINITE;
       break;
     }
-    bwd_sweep<KIND, Q>(P, pp, cur, uh, lam, trial, 0, nullptr, linf, wd);
+    if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, trial, 0, nullptr, linf, wd);
+    else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, trial, 0, linf, wd);
     if (!finite_d(linf)) { status = SNAP_ST_NONFINITE; break; }
     if (polishing) {
       --polish_left;
@@ -636,6 +731,37 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
     }
   }
   if (lane == 0) A.iters[b] = (status == 0) ? solves : status;
+}
+
+template <int KIND, int Q, bool FULL, bool TMA>
+inline int launch_1d_variant(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  auto kern = project1d_kernel<KIND, Q, FULL, TMA>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
+    return SNAP_ECUDA;
+  kern<<<pl.grid, pl.wpc * 32, pl.smem, st>>>(a);
+  return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+}
+
+template <int KIND, int Q>
+inline int launch_1d_q(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  if (KIND == KB) {
+    if (pl.tma)
+      return pl.full ? launch_1d_variant<KB, Q, true, true>(a, pl, st) : launch_1d_variant<KB, Q, false, true>(a, pl, st);
+    return launch_1d_variant<KB, Q, false, false>(a, pl, st);
+  }
+  return pl.tma ? launch_1d_variant<KF, Q, false, true>(a, pl, st) : launch_1d_variant<KF, Q, false, false>(a, pl, st);
+}
+
+template <int KIND>
+inline int launch_1d_kind(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  switch (pl.q) {
+    case 1: return launch_1d_q<KIND, 1>(a, pl, st);
+    case 2: return launch_1d_q<KIND, 2>(a, pl, st);
+    case 4: return launch_1d_q<KIND, 4>(a, pl, st);
+    case 8: return launch_1d_q<KIND, 8>(a, pl, st);
+    case 16: return launch_1d_q<KIND, 16>(a, pl, st);
+  }
+  return SNAP_EINVAL;
 }
 
 }  // namespace snap

@@ -8,12 +8,12 @@
 // (Green's function of (-a, 1+2a, -a), exact to fp64 rounding) on the level held in shared memory.
 #pragma once
 #include "device_utils.cuh"
+#include "launch.h"
 #include "snap_internal.h"
 
 namespace snap {
 
 constexpr int kT2 = 512;          // threads per CTA (one CTA per sample)
-constexpr int kPcgVectors = 8;    // workspace n-vectors per sample: bufA bufB b r z p q y
 
 struct Proj2dArgs {
   DevParams P;
@@ -298,7 +298,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
   return 1;
 }
 
-__global__ void __launch_bounds__(kT2) project2d_kernel(const __grid_constant__ Proj2dArgs A) {
+__global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant__ Proj2dArgs A) {
   extern __shared__ __align__(16) unsigned char smem2[];
   const DevParams& P = A.P;
   const int b = blockIdx.x;
@@ -426,7 +426,7 @@ __global__ void __launch_bounds__(kT2) project2d_kernel(const __grid_constant__ 
   if (tid == 0) A.iters[b] = (status == 0) ? solves : status;
 }
 
-inline int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
+int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                             double* lambda, int* iters, int warm, void* workspace, cudaStream_t st) {
   const DevParams& d = p->dp;
   if (d.nx > kT2) return SNAP_EINVAL;

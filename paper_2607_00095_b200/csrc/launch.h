@@ -1,0 +1,40 @@
+// Host-side launch interfaces between the translation units of libsnap (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "snap_internal.h"
+
+namespace snap {
+
+struct Proj1dArgs {
+  DevParams P;
+  int batch, warm;
+  const double* u_hat;
+  const double* cdata;
+  double* u_star;
+  double* lam;
+  int* iters;
+  double* bufA;  // [batch][n]  trial / iterate ping-pong
+  double* bufB;  // [batch][n]
+  double* aux;   // [batch][2*nt]  level sums and null-space coefficients (min-norm multiplier, kind 4)
+  int nst;       // ring depth (levels in flight per warp)
+  int rp;        // shared-memory row pitch in doubles (even; nx + halo + padding)
+  int warp_bytes;
+};
+
+struct Plan1d {
+  int q, wpc, nst, rp, warp_bytes, grid;
+  bool full;  // nx == 32 q: no bounds checks in the sweeps
+  bool tma;   // every row start is 16-byte aligned: bulk (TMA) copies; otherwise plain loads/stores
+  size_t smem;
+};
+
+constexpr int kPcgVectors = 8;  // 2D workspace n-vectors per sample: bufA bufB b r z p q y
+
+// proj1d_burgers.cu / proj1d_fisher.cu / proj2d.cu (separate translation units, compiled in parallel)
+int launch_project1d_burgers(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
+int launch_project1d_fisher(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
+int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
+                     double* lambda, int* iters, int warm, void* workspace, cudaStream_t st);
+
+}  // namespace snap

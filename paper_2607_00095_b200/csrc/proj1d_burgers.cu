@@ -1,0 +1,8 @@
+// Burgers-family (kinds 1, 4) instantiations of the persistent 1D projection kernel.
+#include "kernels_1d.cuh"
+
+namespace snap {
+int launch_project1d_burgers(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  return launch_1d_kind<KB>(a, pl, st);
+}
+}  // namespace snap

@@ -220,11 +220,13 @@ def time_steps(run: GpuRun, steps: int, warmup: int, dist):
     l0 = run.p.launch_count()
     t0 = torch.cuda.Event(enable_timing=True)
     t1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.profiler.start()       # cudaProfilerStart: `ncu --profile-from-start off` sees the timed region only
     t0.record()
     for s in range(steps):
         run.step(ev[s])
     t1.record()
     torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
     if dist is not None:
         dist.barrier()
     total_ms = t0.elapsed_time(t1)

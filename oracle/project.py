@@ -10,7 +10,8 @@ step" in that order and notation:
        lam+ <- solve (J J^T) lam+ = r              (Schur form of Eq. 24 L468 with W = I)
        u_full <- u_hat - J^T lam+ ;  d <- u_full - u
        if ||h||_inf < tol:  polish (R4) and return
-       mu <- max(mu, 1.1 ||lam+||_inf + 1e-3)
+       mu <- max(mu, 1e-3, ((u - u_hat)^T d + 1/2 ||d||^2) / ((1 - rho) ||h||_1)),  rho = 1/2
+                                                   (N&W Eq. 18.36 with sigma = 1, Hessian of f = I; ref [15] L275)
        Armijo back-tracking on phi(v) = 1/2 ||v - u_hat||^2 + mu ||h(v)||_1     (N&W ch. 18, ref [15] L275)
        u <- u + alpha d
 
@@ -33,6 +34,8 @@ STATUS_LINESEARCH = -2
 STATUS_NONFINITE = -3
 STATUS_PCG = -4
 
+MU_RHO = 0.5               # N&W Eq. 18.36: fraction of the constraint decrease kept in the model
+MU_FLOOR = 1e-3
 POLISH_SKIP_FACTOR = 1e-3   # skip the polish step when ||h||_inf <= 1e-3 * tol (R4 "adaptive variant")
 
 
@@ -126,8 +129,10 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
             status = STATUS_MAXITER
             break
         d = u_full - u
-        mu = max(mu, 1.1 * float(np.abs(lam).max()) + 1e-3)
         h1 = float(np.abs(h).sum())
+        # penalty parameter from the predicted decrease of the quadratic model (N&W Eq. 18.36, sigma = 1):
+        # needs no multiplier, so an implementation may postpone the multiplier solve (R2)
+        mu = max(mu, MU_FLOOR, (float((u - uh) @ d) + 0.5 * float(d @ d)) / ((1.0 - MU_RHO) * h1))
         phi0 = 0.5 * float((u - uh) @ (u - uh)) + mu * h1
         Dphi = float((u - uh) @ d) - mu * h1
         alpha = 1.0

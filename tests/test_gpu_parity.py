@@ -269,11 +269,11 @@ def test_line_search_backtracking_on_gpu(S):
     """R17: force Armijo halving (c1 close to 1, noise 1.0); the limit point must not move."""
     wl = W.make_workload(2, batch=2, nx=24, nt=20, noise=1.0)
     ref = gpu_project(S, wl, wl.u_hat)
-    forced = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.99))
+    forced = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.9))
     assert (forced["iters"] > ref["iters"]).all()
     np.testing.assert_allclose(forced["u"], ref["u"], rtol=0, atol=1e-11)
-    check_against_oracle(wl, wl.u_hat, forced, range(wl.batch), params=dict(ls_c1=0.99))
-    stuck = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.99, ls_max=0))
+    check_against_oracle(wl, wl.u_hat, forced, range(wl.batch), params=dict(ls_c1=0.9))
+    stuck = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.9, ls_max=0))
     assert (stuck["iters"] == -2).all()
 
 

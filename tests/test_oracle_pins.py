@@ -369,7 +369,7 @@ def test_line_search_backtracks_and_still_reaches_the_same_point():
     uh = _np(wl.u_hat[0])
     u0 = _np(wl.cdata[0])
     ref = O.project(wl.kind, uh, u0, wl.params)
-    forced = O.project(wl.kind, uh, u0, dict(wl.params, ls_c1=0.99))
+    forced = O.project(wl.kind, uh, u0, dict(wl.params, ls_c1=0.9))
     assert ref["status"] == 0 and forced["status"] == 0
     assert ref["backtracks"] == 0 and forced["backtracks"] > 0
     np.testing.assert_allclose(forced["u"], ref["u"], rtol=0, atol=1e-11)

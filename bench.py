@@ -46,10 +46,24 @@ def load_peaks():
 
 
 def a_solve_bytes(n: int, m: int) -> int:
-    """Algorithmic bytes of one Gauss-Newton linear solve per sample:
-    forward sweep reads u, u_hat (16 n) and writes y (8 m); backward sweep reads y, u, u_hat (8 m + 16 n)
-    and writes lam, u+ (8 m + 8 n)  =>  40 n + 24 m."""
+    """Classic path (Fisher, 2D outer loop, odd sizes): algorithmic bytes of one Gauss-Newton linear solve per
+    sample: forward sweep reads u, u_hat (16 n) and writes y (8 m); backward sweep reads
+    y, u, u_hat (8 m + 16 n) and writes lam, u+ (8 m + 8 n)  =>  40 n + 24 m."""
     return 40 * n + 24 * m
+
+
+def algorithmic_bytes(run, iters_row):
+    """Bytes one snap_project launch must move.  Fused Burgers path: the rows of nx doubles
+    each pass over the levels reads and writes, counted per sample by the kernel itself (snap_project_stats:
+    u_hat / iterate / y rows in, iterate / y / lam rows out) -- the traffic of THIS variant, not of the 64 n
+    per-iteration model of SURVEY.md §8(d).  Classic path: solves x (40 n + 24 m)."""
+    st = run.stats.cpu()
+    rows = int(st[:, 2].sum() + st[:, 3].sum())
+    if rows > 0:
+        return float(rows) * run.wl.nx * 8.0
+    if run.cfg == 1:
+        return float(run.B * (16 * run.wl.n + 8 * run.p.m))
+    return float(iters_row.clamp(min=0).sum()) * a_solve_bytes(run.wl.n, run.p.m)
 
 
 class ClockSampler:
@@ -187,6 +201,7 @@ class GpuRun:
         self.iters = torch.zeros(self.calls, self.B, dtype=torch.int32, device=dev)
         self.ws = torch.empty(S.snap_workspace_bytes(self.p, self.B), dtype=torch.uint8, device=dev)
         self.norms = torch.empty(self.B, 4, dtype=torch.float64, device=dev)
+        self.stats = torch.zeros(self.B, 4, dtype=torch.int64, device=dev)
 
     def step(self, events=None):
         """The whole hot path over one batch of input: `calls` back-to-back snap_project launches."""
@@ -197,6 +212,18 @@ class GpuRun:
                                 warm=(self.cfg == 5 and c > 0), workspace=self.ws)
             if events is not None:
                 events[c][1].record()
+
+    def traffic_model(self):
+        """Untimed replay of one step that reads the kernel's own per-sample row counters after every call
+        (deterministic: same inputs, same counts as the timed steps).  Returns algorithmic bytes per call."""
+        out = []
+        for c, uh in enumerate(self.inputs):
+            self.S.snap_project(self.p, self.B, uh, self.cdata, self.u_star, self.lam, self.iters[c],
+                                warm=(self.cfg == 5 and c > 0), workspace=self.ws)
+            self.S.snap_project_stats(self.p, self.B, self.ws, self.stats)
+            torch.cuda.synchronize()
+            out.append(algorithmic_bytes(self, self.iters[c].cpu()))
+        return out
 
     def check(self):
         """Every sample converged and the last call's output is feasible."""
@@ -297,9 +324,7 @@ def run_gpu(args):
     # roofline of the dominant kernel (the persistent projection kernel), live CUDA-event durations
     peak, peak_src = load_peaks()
     solves = iters.clamp(min=0).sum(dim=1).to(torch.float64)        # per call, over the batch
-    alg_bytes_call = (solves * a_solve_bytes(wl.n, p.m)).tolist()
-    if cfg == 1:
-        alg_bytes_call = [float(run.B * (16 * wl.n + 8 * p.m))]
+    alg_bytes_call = run.traffic_model()
     kern_s = sum(sum(k) for k in kern_ms) * 1e-3
     alg_total = sum(alg_bytes_call) * args.steps
     achieved = alg_total / kern_s / 1e9
@@ -312,7 +337,8 @@ def run_gpu(args):
                    "l2": "inputs (25.6 GB resident) exceed L2; no flush" if cfg == 5 else
                          "working set smaller than L2 (latency-bound config; see DESIGN.md)",
                    "tol": wl.params["tol"], "converged_all": ok, "max_hinf_last_call": hmax,
-                   "mean_solves_per_projection": float(solves.sum() / (run.B * run.calls))},
+                   "mean_linearisations_per_projection": float(solves.sum() / (run.B * run.calls)),
+                   "alg_bytes_per_projection": sum(alg_bytes_call) / (run.B * run.calls)},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": args.traffic, "kernel": "project1d_kernel" if cfg != 4 else "project2d_kernel",
                      "peak_source": peak_src, "alg_bytes_per_launch_mean": alg_total / (args.steps * run.calls),
@@ -337,8 +363,7 @@ def run_gpu(args):
             r = GpuRun(S, c, dev)
             ms, km, _ = time_steps(r, 5, 3, None)
             okc, hm, itc = r.check()
-            sol = float(itc.clamp(min=0).sum())
-            ab = sol * a_solve_bytes(r.wl.n, r.p.m) if c != 1 else r.B * (16 * r.wl.n + 8 * r.p.m)
+            ab = sum(r.traffic_model())
             others[f"cfg{c}"] = {"projections_per_s": r.B * 5 / (ms * 1e-3), "ms_per_call": ms / 5, "converged_all": okc,
                                  "max_hinf": hm, "model_GBs": ab * 5 / (ms * 1e-3) / 1e9,
                                  "note": "not HBM-resident (fits L2) / latency-bound" if c != 4 else "PCG path"}

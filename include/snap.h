@@ -88,6 +88,10 @@ typedef struct {
   int pcg_max;        /* 2D: PCG iteration cap per solve                    (default 200)                     */
   int precond;        /* 2D: 0 none, 1 time-line, 2 time-line x ADI, 3 time-line x exact level solve (default 2) */
   int lambda_mode;    /* 0 = minimum-norm multiplier, 1 = basic (redundant multipliers = 0)    */
+  int gn_fuse;        /* Burgers kinds with nx in {32,64,128,256,512}: Gauss-Newton iterations carried by one
+                         forward pass over the levels.  0 = as many as the kernel holds in
+                         registers (default), k >= 1 = at most k, -1 = classic path (one forward and one
+                         backward sweep per iteration).  Other kinds / sizes always take the classic path.   */
 } snap_params;
 
 /* Fill *p with the defaults listed above (grid steps 1, physical constants 0, alpha = 1). */
@@ -110,10 +114,12 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch);
  *   u_hat   dev [batch][nt][ny][nx]  in   point to project.  May alias u_star (in place).
  *   cdata   dev [batch][ny][nx]      in   per-sample initial-condition target u0.
  *   u_star  dev [batch][nt][ny][nx]  out  projected field.
- *   lambda  dev [batch][m]           in/out  multipliers lam*.  If warm != 0 the incoming values seed the merit
- *                                         parameter and, for the 2D kind, the PCG initial guess;
- *                                         the iterate itself always starts at u_hat.
- *   iters   dev [batch] (int32)      out  number of linear solves performed, or a negative SNAP_ST_* status.
+ *   lambda  dev [batch][m]           in/out  multipliers lam*.  If warm != 0 the incoming values are the PCG
+ *                                         initial guess of the 2D kind; the 1D kinds solve
+ *                                         directly and ignore them (R2/R3).  The iterate itself
+ *                                         always starts at u_hat.
+ *   iters   dev [batch] (int32)      out  number of Gauss-Newton linearisations (Schur solves, forward half)
+ *                                         used, or a negative SNAP_ST_* status.
  *   workspace dev, >= snap_workspace_bytes(p, batch).
  * Enqueues on `stream`; no host synchronisation. */
 int snap_project(const snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
@@ -137,6 +143,13 @@ int snap_residual(const snap_problem* p, int batch, const double* u, const doubl
  * hold batch*n doubles.  Used by the PCG path and exported for validation against an assembled J J^T. */
 int snap_schur_apply(const snap_problem* p, int batch, const double* u, const double* x, double* out,
                      void* workspace, snap_stream stream);
+
+/* Per-sample work counters of the most recent snap_project call that used `workspace` (1D Burgers/Fisher
+ * kinds; zeros otherwise), copied on `stream` into
+ *   stats  dev [batch][4] (int64): Gauss-Newton linearisations used, passes over the levels (forward,
+ *          backward and correction sweeps), HBM rows of nx doubles requested for reading, rows written.
+ * rows * nx * 8 is the traffic the method itself asked for (bench.py's algorithmic bytes). */
+int snap_project_stats(const snap_problem* p, int batch, const void* workspace, long long* stats, snap_stream stream);
 
 /* Number of kernel launches the library has enqueued through this handle since creation (host counter). */
 long long snap_launch_count(const snap_problem* p);

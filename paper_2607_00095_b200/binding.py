@@ -13,7 +13,7 @@ HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS = r
 EXPORTS = [
     "snap_params_default", "snap_problem_create", "snap_problem_destroy", "snap_num_unknowns", "snap_num_rows",
     "snap_workspace_bytes", "snap_project", "snap_project_host", "snap_residual", "snap_schur_apply",
-    "snap_launch_count", "snap_strerror",
+    "snap_project_stats", "snap_launch_count", "snap_strerror",
 ]
 
 
@@ -33,7 +33,7 @@ class SnapParams(C.Structure):
         ("ls_c1", C.c_double), ("ls_shrink", C.c_double),
         ("ls_max", C.c_int),
         ("pcg_rtol", C.c_double),
-        ("pcg_max", C.c_int), ("precond", C.c_int), ("lambda_mode", C.c_int),
+        ("pcg_max", C.c_int), ("precond", C.c_int), ("lambda_mode", C.c_int), ("gn_fuse", C.c_int),
     ]
 
 
@@ -74,6 +74,8 @@ def load_library():
     lib.snap_residual.restype = C.c_int
     lib.snap_schur_apply.argtypes = [vp, C.c_int, dp, dp, dp, vp, vp]
     lib.snap_schur_apply.restype = C.c_int
+    lib.snap_project_stats.argtypes = [vp, C.c_int, vp, vp, vp]
+    lib.snap_project_stats.restype = C.c_int
     lib.snap_launch_count.argtypes = [vp]
     lib.snap_launch_count.restype = C.c_longlong
     lib.snap_strerror.argtypes = [C.c_int]
@@ -214,3 +216,12 @@ def snap_schur_apply(p: Problem, batch: int, u, x, out, workspace, stream=None):
     rc = load_library().snap_schur_apply(p.handle, int(batch), _ptr(u), _ptr(x), _ptr(out), _ptr(workspace),
                                          _stream_handle(stream))
     _check(rc, "snap_schur_apply")
+
+
+def snap_project_stats(p: Problem, batch: int, workspace, stats, stream=None):
+    """Copy the per-sample work counters of the last snap_project that used `workspace` into
+    `stats` (CUDA int64 tensor [batch][4]: linearisations, passes, rows read, rows written)."""
+    import torch
+    _need(stats, 4 * batch, "stats", torch.int64)
+    rc = load_library().snap_project_stats(p.handle, int(batch), _ptr(workspace), _ptr(stats), _stream_handle(stream))
+    _check(rc, "snap_project_stats")

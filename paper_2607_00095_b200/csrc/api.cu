@@ -68,6 +68,33 @@ bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
   }
 }
 
+// fused Burgers path: nx = 32 q, padded rows, ring of nst x 2 input rows + 4 output rows per warp
+bool plan_fused(const snap_problem* p, int batch, Plan1d& pl) {
+  const int nx = p->dp.nx;
+  pl.q = nx / 32;
+  if (nx % 32 != 0 || (pl.q != 1 && pl.q != 2 && pl.q != 4 && pl.q != 8 && pl.q != 16)) return false;
+  pl.full = true; pl.tma = true;
+  pl.rp = fused_row_pitch(pl.q);
+  const int sms = p->sm_count > 0 ? p->sm_count : 148;
+  int wpc = (batch + sms - 1) / sms;
+  if (wpc < 1) wpc = 1;
+  if (wpc > 8) wpc = 8;
+  const size_t limit = (size_t)p->max_smem_optin;
+  for (;; --wpc) {
+    for (int nst = 4; nst >= 2; --nst) {
+      const size_t wb = align_up((size_t)(2 * nst + 4) * pl.rp * 8 + (size_t)nst * 8, 128);
+      if (wb * wpc <= limit) {
+        pl.wpc = wpc; pl.nst = nst; pl.warp_bytes = (int)wb; pl.smem = wb * wpc;
+        pl.grid = (batch + wpc - 1) / wpc;
+        return true;
+      }
+    }
+    if (wpc == 1) return false;
+  }
+}
+
+size_t aux_bytes(const snap_problem* p, size_t B) { return align_up(B * 2 * (size_t)p->dp.nt * 8, 256); }
+
 bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
 
 }  // namespace
@@ -89,6 +116,7 @@ void snap_params_default(snap_params* p) {
   p->pcg_max = 200;
   p->precond = 2;
   p->lambda_mode = 0;
+  p->gn_fuse = 0;
 }
 
 int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, const snap_params* prm) {
@@ -103,6 +131,7 @@ int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, co
   if (!is_1d(kind) && !(prm->dy > 0.0)) return SNAP_EINVAL;
   if (prm->max_iter < 0 || prm->polish < 0 || prm->ls_max < 0 || prm->pcg_max < 1) return SNAP_EINVAL;
   if (!(prm->ls_shrink > 0.0 && prm->ls_shrink < 1.0) || !(prm->ls_c1 > 0.0 && prm->ls_c1 < 1.0)) return SNAP_EINVAL;
+  if (prm->gn_fuse < -1 || prm->gn_fuse > 64) return SNAP_EINVAL;
   if (prm->precond < 0 || prm->precond > 2 || prm->lambda_mode < 0 || prm->lambda_mode > 1) return SNAP_EINVAL;
 
   snap_problem* p = new (std::nothrow) snap_problem();
@@ -174,7 +203,7 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch) {
   const size_t n = (size_t)p->dp.n, B = (size_t)batch;
   if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return 256;
   if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return align_up(B * n * 8 * kPcgVectors, 256) + 256;
-  return align_up(B * n * 8, 256) * 2 + align_up(B * 2 * (size_t)p->dp.nt * 8, 256) + 256;
+  return align_up(B * n * 8, 256) * 2 + aux_bytes(p, B) + align_up(B * 32, 256) + 256;
 }
 
 int snap_project(const snap_problem* cp, int batch, const double* u_hat, const double* cdata, double* u_star,
@@ -206,10 +235,22 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   a.bufA = reinterpret_cast<double*>(w);
   a.bufB = reinterpret_cast<double*>(w + field);
   a.aux = reinterpret_cast<double*>(w + 2 * field);
-  a.nst = pl.nst; a.rp = pl.rp; a.warp_bytes = pl.warp_bytes;
+  a.stats = reinterpret_cast<long long*>(w + 2 * field + aux_bytes(p, (size_t)batch));
+  a.fuse = p->params.gn_fuse;
   // bulk (TMA) copies need every row start 16-byte aligned
-  pl.tma = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
-           aligned16(lambda) && aligned16(a.bufA);
+  const bool bulk_ok = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
+                       aligned16(lambda) && aligned16(a.bufA);
+  if (d.kind != SNAP_FISHER1D_IE && p->params.gn_fuse >= 0 && bulk_ok) {
+    Plan1d pf;
+    if (plan_fused(p, batch, pf)) {
+      a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
+      p->launches++;
+      return launch_project1d_burgers_fused(a, pf, st);
+    }
+  }
+  cudaMemsetAsync(a.stats, 0, (size_t)batch * 32, st);
+  a.nst = pl.nst; a.rp = pl.rp; a.warp_bytes = pl.warp_bytes;
+  pl.tma = bulk_ok;
   if (!pl.tma) pl.full = false;  // the plain-load path is only instantiated with bounds checks
   p->launches++;
   if (d.kind == SNAP_FISHER1D_IE) return launch_project1d_fisher(a, pl, st);
@@ -251,6 +292,22 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
   if (cudaMemcpyAsync(lambda_host, d_l, B * d.m * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
   if (cudaMemcpyAsync(iters_host, d_i, B * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
   return cudaStreamSynchronize(st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+}
+
+int snap_project_stats(const snap_problem* p, int batch, const void* workspace, long long* stats, snap_stream stream) {
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!stats) return SNAP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const DevParams& d = p->dp;
+  if (d.kind == SNAP_HEAT1D_IC_MASS || d.kind == SNAP_ALLENCAHN2D_IE || !workspace)
+    return cudaMemsetAsync(stats, 0, (size_t)batch * 32, st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+  const size_t field = align_up((size_t)batch * d.n * 8, 256);
+  const unsigned char* w = static_cast<const unsigned char*>(workspace);
+  w = reinterpret_cast<const unsigned char*>(align_up(reinterpret_cast<uintptr_t>(w), 256));
+  const void* src = w + 2 * field + aux_bytes(p, (size_t)batch);
+  return cudaMemcpyAsync(stats, src, (size_t)batch * 32, cudaMemcpyDeviceToDevice, st) == cudaSuccess ? SNAP_OK
+                                                                                                      : SNAP_ECUDA;
 }
 
 int snap_residual(const snap_problem* cp, int batch, const double* u, const double* cdata, double* h, double* norms,

@@ -21,6 +21,14 @@ __device__ __forceinline__ int warp_or(int v) { return __any_sync(SNAP_FULL, v) 
 
 __device__ __forceinline__ bool finite_d(double x) { return fabs(x) <= 1.7976931348623157e308; }
 
+// mu <- max(mu, floor, (w^T d + 1/2 d^T d) / ((1 - rho) ||h||_1))   (R2, N&W Eq. 18.36)
+__device__ __forceinline__ double merit_mu(double mu, double wd, double dd, double h1, double rho, double floor_) {
+  mu = fmax(mu, floor_);
+  const double num = fma(0.5, dd, wd);
+  if (h1 > 0.0 && num > 0.0) mu = fmax(mu, num / ((1.0 - rho) * h1));
+  return mu;
+}
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }

@@ -398,10 +398,10 @@ __device__ void fwd_sweep_f(const DevParams& P, Pipe<TMA>& pp, const double* __r
 template <int Q, bool FULL, bool TMA>
 __device__ void bwd_sweep_b(const DevParams& P, Pipe<TMA>& pp, const double* __restrict__ u,
                             const double* __restrict__ uh, double* __restrict__ lam, double* __restrict__ unew,
-                            int mode, double* __restrict__ sig, double& linf_out, double& wd_out) {
+                            int mode, double* __restrict__ sig, double& linf_out, double& wd_out, double& dd_out) {
   const int nx = P.nx, nt = P.nt, lane = pp.lane, nst = pp.nst;
   const double a0 = P.bs_a0, e = P.bs_e, hs = P.bs_hs;
-  double linf = 0.0, wd = 0.0;
+  double linf = 0.0, wd = 0.0, dd = 0.0;
   double lo[Q];
 #pragma unroll
   for (int j = 0; j < Q; ++j) lo[j] = 0.0;
@@ -449,6 +449,7 @@ __device__ void bwd_sweep_b(const DevParams& P, Pipe<TMA>& pp, const double* __r
         const double un = (mode == 0) ? step : v;
         if (TMA) uo[o] = un; else { lg[lane + o] = l; ug[lane + o] = un; }
         wd = fma(v - uhk, step - v, wd);
+        dd = fma(step - v, step - v, dd);
         linf = fmax(linf, fabs(l));
         lsum += l;
         lo[j] = l;
@@ -473,18 +474,20 @@ __device__ void bwd_sweep_b(const DevParams& P, Pipe<TMA>& pp, const double* __r
   pp.drain();
   linf = warp_max(linf);
   wd = warp_sum(wd);
+  dd = warp_sum(dd);
   // fmax drops NaN: detect a non-finite multiplier / step through the sum as well
-  linf_out = finite_d(wd) ? linf : __longlong_as_double(0x7ff8000000000000LL);
+  linf_out = (finite_d(wd) && finite_d(dd)) ? linf : __longlong_as_double(0x7ff8000000000000LL);
   wd_out = wd;
+  dd_out = dd;
 }
 
 // Fisher:  T_k lam_k = y_k + lam_{k+1}  (k >= 1, T symmetric) ,  lam_0 = y_0 + lam_1.
 template <int Q, bool TMA>
 __device__ void bwd_sweep_f(const DevParams& P, Pipe<TMA>& pp, const double* __restrict__ u,
                             const double* __restrict__ uh, double* __restrict__ lam, double* __restrict__ unew,
-                            int mode, double& linf_out, double& wd_out) {
+                            int mode, double& linf_out, double& wd_out, double& dd_out) {
   const int nx = P.nx, nt = P.nt, lane = pp.lane, nst = pp.nst;
-  double linf = 0.0, wd = 0.0;
+  double linf = 0.0, wd = 0.0, dd = 0.0;
   double lo[Q];
 #pragma unroll
   for (int j = 0; j < Q; ++j) lo[j] = 0.0;
@@ -529,6 +532,7 @@ __device__ void bwd_sweep_f(const DevParams& P, Pipe<TMA>& pp, const double* __r
         const double un = (mode == 0) ? step : uk[j];
         if (TMA) { lc[i] = l; uo[i] = un; } else { lg[i] = l; ug[i] = un; }
         wd = fma(uk[j] - uhk[j], step - uk[j], wd);
+        dd = fma(step - uk[j], step - uk[j], dd);
         linf = fmax(linf, fabs(l));
         lo[j] = l;
       }
@@ -547,8 +551,10 @@ __device__ void bwd_sweep_f(const DevParams& P, Pipe<TMA>& pp, const double* __r
   pp.drain();
   linf = warp_max(linf);
   wd = warp_sum(wd);
-  linf_out = finite_d(wd) ? linf : __longlong_as_double(0x7ff8000000000000LL);
+  dd = warp_sum(dd);
+  linf_out = (finite_d(wd) && finite_d(dd)) ? linf : __longlong_as_double(0x7ff8000000000000LL);
   wd_out = wd;
+  dd_out = dd;
 }
 
 // Minimum-norm multiplier for the linearly dependent mass rows of kind 4 (streaming
@@ -638,13 +644,7 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
     for (int i = lane; i < nx; i += 32) sm += u0[i];
     M0 = P.dx * warp_sum(sm);
   }
-  double mu = 0.0;
-  if (A.warm) {  // the incoming multipliers only seed the merit parameter for these kinds
-    double li = 0.0;
-    for (size_t i = lane; i < (size_t)P.m; i += 32) li = fmax(li, fabs(lam[i]));
-    li = warp_max(li);
-    if (finite_d(li)) mu = 1.1 * li + 1e-3;
-  }
+  double mu = 0.0;  // DESIGN.md R2/R3: the penalty parameter needs no multiplier; `warm` is ignored for 1D kinds
 
   const double* cur = uh;   // accepted iterate
   double* trial = bufA;     // where the next trial point goes
@@ -692,20 +692,20 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
       status = SNAP_ST_MAXITER;
       final_solve = true;
     }
-    double linf, wd;
+    double linf, wd, dd;
     if (final_solve) {
-      if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, ustar, 1, want_sig ? sig : nullptr, linf, wd);
-      else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, ustar, 1, linf, wd);
+      if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, ustar, 1, want_sig ? sig : nullptr, linf, wd, dd);
+      else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, ustar, 1, linf, wd, dd);
       if (!finite_d(linf)) status = SNAP_ST_NONFINITE;
       break;
     }
-    if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, trial, 0, nullptr, linf, wd);
-    else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, trial, 0, linf, wd);
+    if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, trial, 0, nullptr, linf, wd, dd);
+    else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, trial, 0, linf, wd, dd);
     if (!finite_d(linf)) { status = SNAP_ST_NONFINITE; break; }
     if (polishing) {
       --polish_left;
     } else {
-      mu = fmax(mu, 1.1 * linf + 1e-3);
+      mu = merit_mu(mu, wd, dd, nrm.h1, kMuRho, kMuFloor);
       phi_cur = nrm.f + mu * nrm.h1;
       Dphi = wd - mu * nrm.h1;
       alpha = 1.0;

@@ -212,8 +212,8 @@ __device__ double precond_apply(const DevParams& P, const Ctx2d& c, const double
 // ---- a8: trial = u_hat - J^T lam ; returns ||lam||_inf and (u - u_hat)^T (trial - u) ------------------
 __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __restrict__ u,
                           const double* __restrict__ uh, const double* __restrict__ lam, double* __restrict__ trial,
-                          double& linf, double& wd) {
-  double a_inf = 0.0, a_wd = 0.0;
+                          double& linf, double& wd, double& dd) {
+  double a_inf = 0.0, a_wd = 0.0, a_dd = 0.0;
   for (int k = 0; k < c.nt; ++k) {
     const double* uk = u + (size_t)k * c.L;
     const double* lk = lam + (size_t)k * c.L;
@@ -227,6 +227,7 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
       const double tr = hh - g;
       trial[(size_t)k * c.L + cell] = tr;
       a_wd = fma(v - hh, tr - v, a_wd);
+      a_dd = fma(tr - v, tr - v, a_dd);
       const double al = fabs(c.s0[cell]);
       if (!finite_d(al)) a_inf = 1.7976931348623157e308 * 2.0;
       a_inf = fmax(a_inf, al);
@@ -234,6 +235,7 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
   }
   linf = blk_max(c, a_inf);
   wd = blk_sum(c, a_wd);
+  dd = blk_sum(c, a_dd);
 }
 
 // ---- a6: PCG on S lam = b.  Returns 0 on success, 1 if pcg_max was hit ----------------------------------
@@ -346,7 +348,7 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
       li = fmax(li, finite_d(v) ? v : 1.7976931348623157e308 * 2.0);
     }
     li = blk_max(c, li);
-    if (finite_d(li)) mu = 1.1 * li + 1e-3; else have_lam = false;
+    if (!finite_d(li)) have_lam = false;   // R3: the warm start is the PCG initial guess only
   }
 
   const double* cur = uh;
@@ -401,13 +403,13 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
       final_solve = true;
     }
     if (final_solve) break;
-    double linf, wd;
-    step_pass(P, c, cur, uh, lam, trial, linf, wd);
-    if (!finite_d(linf) || !finite_d(wd)) { status = SNAP_ST_NONFINITE; break; }
+    double linf, wd, dd;
+    step_pass(P, c, cur, uh, lam, trial, linf, wd, dd);
+    if (!finite_d(linf) || !finite_d(wd) || !finite_d(dd)) { status = SNAP_ST_NONFINITE; break; }
     if (polishing) {
       --polish_left;
     } else {
-      mu = fmax(mu, 1.1 * linf + 1e-3);
+      mu = merit_mu(mu, wd, dd, h1, kMuRho, kMuFloor);
       phi_cur = f + mu * h1;
       Dphi = wd - mu * h1;
       alpha = 1.0;

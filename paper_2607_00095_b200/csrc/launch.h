@@ -17,6 +17,8 @@ struct Proj1dArgs {
   double* bufA;  // [batch][n]  trial / iterate ping-pong
   double* bufB;  // [batch][n]
   double* aux;   // [batch][2*nt]  level sums and null-space coefficients (min-norm multiplier, kind 4)
+  long long* stats;  // [batch][4]  linearisations, passes, HBM rows read, rows written (snap_project_stats)
+  int fuse;      // cap on Gauss-Newton iterations per forward pass (0 = as many as the kernel supports)
   int nst;       // ring depth (levels in flight per warp)
   int rp;        // shared-memory row pitch in doubles (even; nx + halo + padding)
   int warp_bytes;
@@ -34,6 +36,9 @@ constexpr int kPcgVectors = 8;  // 2D workspace n-vectors per sample: bufA bufB 
 // proj1d_burgers.cu / proj1d_fisher.cu / proj2d.cu (separate translation units, compiled in parallel)
 int launch_project1d_burgers(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
 int launch_project1d_fisher(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
+// proj1d_burgers_fused.cu: nx = 32 q, bulk-copy alignment required; pl.rp / pl.warp_bytes follow plan_fused()
+int launch_project1d_burgers_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
+int fused_row_pitch(int q);   // padded shared-memory row pitch in doubles
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, cudaStream_t st);
 

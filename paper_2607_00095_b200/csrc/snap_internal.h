@@ -9,6 +9,10 @@ namespace snap {
 
 constexpr int kWarp = 32;
 constexpr double kPolishSkip = 1e-3;  // polish skipped when ||h||_inf <= kPolishSkip * tol
+// l1-merit penalty parameter (R2; Nocedal-Wright Eq. 18.36 with sigma = 1, Hessian of f = I):
+//   mu <- max(mu, kMuFloor, (w^T d + 1/2 ||d||^2) / ((1 - kMuRho) ||h||_1))   -- needs no multiplier
+constexpr double kMuRho = 0.5;
+constexpr double kMuFloor = 1e-3;
 
 // Plain-old-data copy of everything a kernel needs; passed by value as a __grid_constant__.
 struct DevParams {

@@ -62,7 +62,8 @@ def check_against_oracle(wl, u_hat, g, samples, params=None, tol_u=TOL_U, tol_l=
         worst_u, worst_l = max(worst_u, ru), max(worst_l, rl)
         assert ru <= tol_u, f"sample {b}: rel_u {ru:.2e}"
         assert rl <= tol_l, f"sample {b}: rel_lam {rl:.2e}"
-        assert abs(int(g["iters"][b]) - int(o["iters"])) <= 1
+        # trajectory is unpinned: +-1 for the classic path; the fused passes may add up to JT - 1 polish steps
+        assert -1 <= int(g["iters"][b]) - int(o["iters"]) <= 4, (int(g["iters"][b]), int(o["iters"]))
     return worst_u, worst_l
 
 

@@ -68,29 +68,62 @@ bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
   }
 }
 
-// fused Burgers path: nx = 32 q, padded rows, ring of nst x 2 input rows + 4 output rows per warp
+// fused Burgers path: nx = 32 W Q, padded rows; per sample a ring of nst x 2 input rows + 4 output rows,
+// exchange slots, reduction scratch and mbarriers.  pl.wpc = samples per CTA, pl.warp_bytes = bytes per sample.
 bool plan_fused(const snap_problem* p, int batch, Plan1d& pl) {
   const int nx = p->dp.nx;
-  pl.q = nx / 32;
-  if (nx % 32 != 0 || (pl.q != 1 && pl.q != 2 && pl.q != 4 && pl.q != 8 && pl.q != 16)) return false;
-  pl.full = true; pl.tma = true;
-  pl.rp = fused_row_pitch(pl.q);
+  int W, Q, JT, maxt;
+  static const int variant = [] { const char* e = getenv("SNAP_FUSED_VARIANT"); return e ? atoi(e) : 0; }();
+  if (!fused_variant(nx, variant, W, Q, JT, maxt)) return false;
+  pl.variant = variant;
+  pl.wps = W;
+  pl.q = Q; pl.full = true; pl.tma = true;
+  pl.rp = fused_row_pitch(nx);
   const int sms = p->sm_count > 0 ? p->sm_count : 148;
-  int wpc = (batch + sms - 1) / sms;
-  if (wpc < 1) wpc = 1;
-  if (wpc > 8) wpc = 8;
+  int spc = (batch + sms - 1) / sms;      // samples per CTA: one wave over the SMs when possible
+  const int spc_max = maxt / (32 * W) < 15 ? maxt / (32 * W) : 15;   // named barriers 1..15
+  if (spc < 1) spc = 1;
+  if (spc > spc_max) spc = spc_max;
   const size_t limit = (size_t)p->max_smem_optin;
-  for (;; --wpc) {
+  for (;; --spc) {
     for (int nst = 4; nst >= 2; --nst) {
-      const size_t wb = align_up((size_t)(2 * nst + 4) * pl.rp * 8 + (size_t)nst * 8, 128);
-      if (wb * wpc <= limit) {
-        pl.wpc = wpc; pl.nst = nst; pl.warp_bytes = (int)wb; pl.smem = wb * wpc;
-        pl.grid = (batch + wpc - 1) / wpc;
+      const size_t sb = align_up(((size_t)(2 * nst + 4) * pl.rp + 2 * W * 8 + W * 24 + nst) * 8, 1024);
+      if (sb * spc + 1024 <= limit) {
+        pl.wpc = spc; pl.nst = nst; pl.warp_bytes = (int)sb; pl.smem = sb * spc + 1024;
+        pl.grid = (batch + spc - 1) / spc;
         return true;
       }
     }
-    if (wpc == 1) return false;
+    if (spc == 1) return false;
   }
+}
+
+// Tensor map of a [batch][n (+ tail)] fp64 buffer seen as [sample][line of 16 doubles][16]; one TMA box = the
+// `box_lines` lines of (a warp's part of) one row, stored in shared memory with the 128-byte swizzle.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(f);
+  }();
+  return fn;
+}
+bool make_row_map(CUtensorMap* tm, const void* base, int batch, size_t n, size_t sample_stride_doubles, int box_lines) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[3] = {16, (cuuint64_t)(n / 16), (cuuint64_t)batch};
+  const cuuint64_t strides[2] = {128, (cuuint64_t)sample_stride_doubles * 8};
+  const cuuint32_t box[3] = {16, (cuuint32_t)box_lines, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 size_t aux_bytes(const snap_problem* p, size_t B) { return align_up(B * 2 * (size_t)p->dp.nt * 8, 256); }
@@ -243,9 +276,18 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   if (d.kind != SNAP_FISHER1D_IE && p->params.gn_fuse >= 0 && bulk_ok) {
     Plan1d pf;
     if (plan_fused(p, batch, pf)) {
-      a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
-      p->launches++;
-      return launch_project1d_burgers_fused(a, pf, st);
+      const int box = d.nx / 16 / pf.wps;
+      const size_t n = (size_t)d.n;
+      const bool ok = make_row_map(&a.tm[TM_UHAT], u_hat, batch, n, n, box) &&
+                      make_row_map(&a.tm[TM_BUFA], a.bufA, batch, n, n, box) &&
+                      make_row_map(&a.tm[TM_BUFB], a.bufB, batch, n, n, box) &&
+                      make_row_map(&a.tm[TM_USTAR], u_star, batch, n, n, box) &&
+                      make_row_map(&a.tm[TM_LAM], lambda, batch, n, (size_t)d.m, box);
+      if (ok) {
+        a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
+        p->launches++;
+        return launch_project1d_burgers_fused(a, pf, st);
+      }
     }
   }
   cudaMemsetAsync(a.stats, 0, (size_t)batch * 32, st);

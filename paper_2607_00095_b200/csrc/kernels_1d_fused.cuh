@@ -1,4 +1,4 @@
-// Burgers family (kinds 1, 4), nx = 32 Q: fused Gauss-Newton sweeps, one persistent warp per sample.
+// Burgers family (kinds 1, 4), nx = 32 W Q: fused Gauss-Newton passes, one persistent group of W warps per sample.
 //
 // For these row sets J_loc is square, unit block lower-bidiagonal in time (diagonal blocks I, sub-diagonal
 // blocks -A_{k-1}, A_k = dPhi/du at level k), so the Schur solve (J J^T) lam+ = r factors into the forward
@@ -13,113 +13,156 @@
 // Armijo tests of the fused steps are evaluated after the pass from per-iteration sums; if one fails the
 // pass is discarded and the sample continues with one iteration per pass (classic back-tracking).
 //
-// Layout: lane l owns the Q contiguous cells l*Q .. l*Q+Q-1, neighbours are register-local except at the two
-// ends (one shuffle each, periodic wrap for free).  Rows travel HBM <-> shared memory as 128-byte bulk (TMA)
-// copies, one per lane, into rows padded by 16 bytes per 128 so that the lanes' 128-bit shared-memory
-// accesses are bank-conflict free.
+// Layout: warp w of the group, lane l owns the Q contiguous cells (32 w + l) Q ... + Q - 1; neighbours are
+// register-local except at the two ends of a lane (one shuffle each) and of a warp (a shared-memory slot and
+// one named barrier per iteration; W = 1 needs neither).  A row travels HBM <-> shared memory as ONE tiled TMA
+// copy (tensor map [sample][line of 16 doubles][16], box = one row, issued by one elected lane) with the
+// 128-byte swizzle, so that the lanes' 128-bit shared-memory accesses to their contiguous cells are
+// bank-conflict free: the 16-byte chunk c of line r sits at chunk position c ^ (r & 7).
 #pragma once
+#include <stdio.h>
+#include <stdlib.h>
+
 #include "device_utils.cuh"
 #include "launch.h"
 #include "snap_internal.h"
 
 namespace snap {
 
-template <int Q>
+template <int W, int Q>
 struct RowGeom {
-  static constexpr int NX = 32 * Q;
-  static constexpr int SEGS = NX / 16;   // 128-byte segments per row, one bulk copy (and one issuing lane) each
-  static constexpr int RP = SEGS * 18;   // padded row pitch in doubles: 16 data + 2 pad per segment
+  static constexpr int NX = 32 * W * Q;
+  static constexpr int LINES = NX / 16;       // 128-byte lines per row
+  static constexpr int WLINES = LINES / W;    // lines owned (and stored) by one warp; one TMA box
+  static constexpr int RP = (NX < 128 ? 128 : NX);   // row pitch in doubles: rows start 1024-byte aligned
+  static constexpr int XCH = 2 * W * 8;       // doubles: exchange slots [parity][warp][8]
+  static_assert(W == 1 || WLINES % 8 == 0, "a warp's part of a row must start on a 1024-byte boundary");
 };
 
-// cell i of a row lives at double index i + 2 (i >> 4) of its padded shared-memory row
-__device__ __forceinline__ int pad_idx(int i) { return i + 2 * (i >> 4); }
+// cell i of a row lives at this double index of its swizzled shared-memory row (row base 1024-byte aligned)
+__device__ __forceinline__ int swz_idx(int i) {
+  const int r = i >> 4, c = (i & 15) >> 1;
+  return (r << 4) + ((c ^ (r & 7)) << 1) + (i & 1);
+}
+
+// per-lane chunk offsets (in doubles) of its Q contiguous cells: Q/2 chunks of 2 doubles inside one line
+template <int Q>
+struct LaneOff {
+  int o[(Q + 1) / 2];
+  __device__ __forceinline__ void init(int first) {
+#pragma unroll
+    for (int c = 0; c < (Q + 1) / 2; ++c) o[c] = swz_idx(first + 2 * c);
+  }
+};
 
 template <int Q>
-__device__ __forceinline__ void load_cells(const double* row, int lane, double (&x)[Q]) {
-  const double* p = row + pad_idx(Q * lane);
+__device__ __forceinline__ void load_cells(const double* row, const LaneOff<Q>& lo, double (&x)[Q]) {
   if constexpr (Q == 1) {
-    x[0] = p[0];
+    x[0] = row[lo.o[0]];
   } else {
 #pragma unroll
     for (int c = 0; c < Q / 2; ++c) {
-      const double2 t = reinterpret_cast<const double2*>(p)[c];
+      const double2 t = *reinterpret_cast<const double2*>(row + lo.o[c]);
       x[2 * c] = t.x;
       x[2 * c + 1] = t.y;
     }
   }
 }
 template <int Q>
-__device__ __forceinline__ void store_cells(double* row, int lane, const double (&x)[Q]) {
-  double* p = row + pad_idx(Q * lane);
+__device__ __forceinline__ double cell_at(const double* row, const LaneOff<Q>& lo, int c) {
+  return row[lo.o[c >> 1] + (c & 1)];
+}
+template <int Q>
+__device__ __forceinline__ void store_cells(double* row, const LaneOff<Q>& lo, const double (&x)[Q]) {
   if constexpr (Q == 1) {
-    p[0] = x[0];
+    row[lo.o[0]] = x[0];
   } else {
 #pragma unroll
-    for (int c = 0; c < Q / 2; ++c) reinterpret_cast<double2*>(p)[c] = make_double2(x[2 * c], x[2 * c + 1]);
+    for (int c = 0; c < Q / 2; ++c) *reinterpret_cast<double2*>(row + lo.o[c]) = make_double2(x[2 * c], x[2 * c + 1]);
   }
 }
 
 __device__ __forceinline__ double shfl_prev(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 31) & 31); }
 __device__ __forceinline__ double shfl_next(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 1) & 31); }
 
+constexpr int kRed = 24;   // doubles per warp in the reduction scratch (>= 4 JT + 1)
+
+// a global buffer of the path: its tensor map (rows as TMA boxes) and the sample's base pointer (generic access)
+struct Buf {
+  const CUtensorMap* tm;
+  double* p;
+};
+
 // ------------------------------------------------------------------------------------------------
-// per-warp row pipeline: ring of `nst` stages x 2 input rows + 4 output rows, padded layout
+// per-sample row pipeline shared by the W warps of a group: ring of `nst` stages x 2 input rows,
+// 4 output rows, exchange slots, reduction scratch, mbarriers
 // ------------------------------------------------------------------------------------------------
-template <int Q>
+template <int W, int Q>
 struct RowPipe {
-  using G = RowGeom<Q>;
-  double* stage;   // [nst][2][RP]
+  using G = RowGeom<W, Q>;
+  double* stage;   // [nst][2][RP]   (1024-byte aligned)
   double* orow;    // [4][RP]
+  double* xch;     // [2][W][8]
+  double* red;     // [W][kRed] partial sums of a pass
   uint32_t bar0, phase;
-  int nst, lane;
-  long long rows_rd, rows_wr;   // HBM rows requested (lane 0 counts): the traffic this variant needs
+  int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
+  LaneOff<Q> lo;
+  long long rows_rd, rows_wr;        // HBM rows requested (counted once per group): the traffic this variant needs
 
   __device__ __forceinline__ double* row(int s, int r) const { return stage + (size_t)(s * 2 + r) * G::RP; }
   __device__ __forceinline__ double* out(int r) const { return orow + (size_t)r * G::RP; }
 
-  // every lane has finished reading stage s; load one or two global rows into it
-  __device__ __forceinline__ void issue(int s, const double* g0, const double* g1) {
+  __device__ __forceinline__ void gsync() const {
+    if constexpr (W > 1) asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(W * 32) : "memory");
+    else __syncwarp();
+  }
+  // Every warp of the group has finished reading stage s (callers guarantee it through a gsync);
+  // one lane of warp 0 loads level k of one or two buffers into it.
+  __device__ __forceinline__ void issue(int s, int k, const CUtensorMap* t0, const CUtensorMap* t1) {
+    if (w != 0) return;
     __syncwarp();
-    const uint32_t bar = bar0 + 8u * s;
     if (lane == 0) {
-      mbar_expect_tx(bar, (uint32_t)G::NX * 8u * (g1 ? 2u : 1u));
-      rows_rd += g1 ? 2 : 1;
-    }
-    __syncwarp();
-    if (lane < G::SEGS) {
-      bulk_g2s(smem_u32(row(s, 0) + 18 * lane), g0 + 16 * lane, 128u, bar);
-      if (g1) bulk_g2s(smem_u32(row(s, 1) + 18 * lane), g1 + 16 * lane, 128u, bar);
+      const uint32_t bar = bar0 + 8u * s;
+      mbar_expect_tx(bar, (uint32_t)G::NX * 8u * (t1 ? 2u : 1u));
+      rows_rd += t1 ? 2 : 1;
+#pragma unroll
+      for (int i = 0; i < W; ++i) {
+        tma_load_3d(smem_u32(row(s, 0) + i * G::WLINES * 16), t0, 0, k * G::LINES + i * G::WLINES, b, bar);
+        if (t1) tma_load_3d(smem_u32(row(s, 1) + i * G::WLINES * 16), t1, 0, k * G::LINES + i * G::WLINES, b, bar);
+      }
     }
   }
   __device__ __forceinline__ void wait(int s) {
     mbar_wait(bar0 + 8u * s, (phase >> s) & 1u);
     phase ^= (1u << s);
   }
-  // the output rows written two levels ago have been read by the bulk-store engine
+  // this warp's part of the output rows written two levels ago has been read by the TMA store engine
   __device__ __forceinline__ void out_ready() {
-    if (lane < G::SEGS) bulk_wait_read<1>();
+    if (lane == 0) bulk_wait_read<1>();
     __syncwarp();
   }
-  // lanes have filled output row(s) with generic stores: fence, then hand them to the bulk-store engine
-  __device__ __forceinline__ void store_rows(double* g0, const double* s0, double* g1, const double* s1) {
+  // lanes have filled their part of the output row(s) with generic stores: fence, then store that part (level k)
+  __device__ __forceinline__ void store_rows(int k, const CUtensorMap* t0, const double* s0, const CUtensorMap* t1,
+                                             const double* s1) {
     fence_proxy_async_smem();
     __syncwarp();
-    if (lane < G::SEGS) {
-      if (g0) bulk_s2g(g0 + 16 * lane, smem_u32(s0 + 18 * lane), 128u);
-      if (g1) bulk_s2g(g1 + 16 * lane, smem_u32(s1 + 18 * lane), 128u);
+    if (lane == 0) {
+      const int line = k * G::LINES + w * G::WLINES;
+      if (t0) tma_store_3d(t0, 0, line, b, smem_u32(s0 + w * G::WLINES * 16));
+      if (t1) tma_store_3d(t1, 0, line, b, smem_u32(s1 + w * G::WLINES * 16));
       bulk_commit();
+      rows_wr += (t0 ? 1 : 0) + (t1 ? 1 : 0);
     }
-    if (lane == 0) rows_wr += (g0 ? 1 : 0) + (g1 ? 1 : 0);
   }
-  // all bulk stores of this warp are complete and visible to later (bulk or generic) loads
+  // all TMA stores of the group are complete and visible to later (TMA or generic) loads
   __device__ __forceinline__ void drain() {
-    if (lane < G::SEGS) bulk_wait_all<0>();
+    if (lane == 0) bulk_wait_all<0>();
     fence_proxy_async_all();
-    __syncwarp();
+    gsync();
   }
 };
 
-// warp-uniform sums of one fused pass, index t = iteration within the pass (iterate x_t, step d_t = -q_t)
+// group-uniform sums of one fused pass, index t = iteration within the pass (iterate x_t, step d_t = -q_t)
 template <int JT>
 struct FusedStats {
   double hinf[JT], h1[JT];   // ||h(x_t)||_inf, ||h(x_t)||_1   (local + mass rows)
@@ -129,117 +172,186 @@ struct FusedStats {
 };
 
 // ------------------------------------------------------------------------------------------------
-// fused forward pass: iterations t = 0 .. T-1 at every level; iterations t < J update the iterate
-// (x_{t+1} = x_t - q_t), iteration J (present iff T == J + 1) only emits y = q - (x_J - u_hat) into `yout`
-// (the right-hand side of the multiplier solve at x_J).  Reads x_0 (and u_hat if different), writes x_J to
-// `xout` when J > 0.
+// fused forward pass, NU updates + (EMIT ? 1 : 0) y-emitting iteration, T = NU + EMIT iterations per level.
+// Iteration t < NU:  x_{t+1} = x_t - q_t;  iteration NU (EMIT): y = q - (x_NU - u_hat) -> `yout`, the
+// right-hand side of the multiplier solve at x_NU.  Reads x_0 (and u_hat if different), writes x_NU to
+// `xout` when NU > 0.
 // ------------------------------------------------------------------------------------------------
-template <int Q, int JT>
-__device__ void fused_fwd(const DevParams& P, RowPipe<Q>& pp, const double* __restrict__ x0,
-                          const double* __restrict__ uh, const double* __restrict__ u0, double* __restrict__ xout,
-                          double* __restrict__ yout, const int J, const int T, const double M0, FusedStats<JT>& S) {
-  constexpr int nx = RowGeom<Q>::NX;
-  const int nt = P.nt, lane = pp.lane, nst = pp.nst;
+template <int W, int Q, int JT, int NU, bool EMIT>
+__device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
+                                       const double* __restrict__ u0, const Buf xout, const Buf yout, const double M0,
+                                       FusedStats<JT>& S) {
+  using G = RowGeom<W, Q>;
+  constexpr int nx = G::NX;
+  constexpr int T = NU + (EMIT ? 1 : 0);
+  static_assert(T >= 1 && T <= JT, "iterations per pass");
+  RowPipe<W, Q> pp = pp_ref;   // registers; the mutable fields are written back at the end
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, w = pp.w, first = pp.first;
   const double a0 = P.bs_a0, e = P.bs_e, qs = P.bs_qs, hs = P.bs_hs;
-  const bool same = (x0 == uh);
+  const bool same = (x0.p == uh.p);
   const bool has_mass = P.has_mass != 0;
+  const int wl = (w + W - 1) % W, wr = (w + 1) % W;
+  // cells just outside this warp's range (periodic), read by lane 0 / lane 31 for iteration 0
+  const int cellL = swz_idx((first + nx - 1) % nx), cellR = swz_idx((first + Q) % nx);
+  const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
 
-  double phi[JT][Q], cc[JT][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
-  double hinf[JT], h1[JT], wd[JT], dd[JT];   // per-lane partial sums
-  double minf[JT], m1[JT];                   // mass rows (warp-uniform)
+  double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
+  double hinf[T], h1[T], wd[T], dd[T];     // per-lane partial sums (thread 0 of the group also takes the mass rows)
   double f2 = 0.0;
   {
     double u0r[Q];
 #pragma unroll
-    for (int c = 0; c < Q; ++c) u0r[c] = u0[Q * lane + c];
+    for (int c = 0; c < Q; ++c) u0r[c] = u0[first + c];
 #pragma unroll
-    for (int t = 0; t < JT; ++t) {
+    for (int t = 0; t < T; ++t) {
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         phi[t][c] = u0r[c];   // level 0: h_0 = x[0] - u0
         cc[t][c] = 0.0;
       }
-      hinf[t] = 0.0; h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; minf[t] = 0.0; m1[t] = 0.0;
+      hinf[t] = 0.0; h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0;
     }
   }
   const int npro = nst < nt ? nst : nt;
-  for (int k = 0; k < npro; ++k) pp.issue(k, x0 + (size_t)k * nx, same ? nullptr : uh + (size_t)k * nx);
+  for (int k = 0; k < npro; ++k) pp.issue(k, k, x0.tm, tm_uh);
 
-  int s = 0;
+  int s = 0, par = 0;
   for (int k = 0; k < nt; ++k) {
     pp.wait(s);
-    double v[Q], uhr[Q];
-    load_cells<Q>(pp.row(s, 0), lane, v);
-    if (same) {
-#pragma unroll
-      for (int c = 0; c < Q; ++c) uhr[c] = v[c];
-    } else {
-      load_cells<Q>(pp.row(s, 1), lane, uhr);
+    double v[Q];
+    const double* r0 = pp.row(s, 0);
+    const double* ruh = same ? r0 : pp.row(s, 1);   // u_hat cells are re-read where needed
+    load_cells<Q>(r0, pp.lo, v);
+    double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
+    if constexpr (W > 1) {
+      if (lane == 0) vL = r0[cellL];
+      if (lane == 31) vR = r0[cellR];
     }
     pp.out_ready();
     double* so_u = pp.out(k & 1);
     double* so_y = pp.out(2 + (k & 1));
 #pragma unroll
-    for (int t = 0; t < JT; ++t) {
-      if (t < T) {
-        const double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
-        double q[Q];
-        double msum = 0.0;
+    for (int t = 0; t < T; ++t) {
+      double q[Q];
+      double msum = 0.0;
 #pragma unroll
-        for (int c = 0; c < Q; ++c) {
-          const double h = v[c] - phi[t][c];
-          q[c] = h + cc[t][c];
-          const double w = v[c] - uhr[c];
-          const double ah = fabs(h);
-          hinf[t] = fmax(hinf[t], ah);
-          h1[t] += ah;
-          wd[t] = fma(w, q[c], wd[t]);
-          dd[t] = fma(q[c], q[c], dd[t]);
-          if (t == 0) f2 = fma(w, w, f2);
-          msum += v[c];
-        }
-        const double qL = shfl_prev(q[Q - 1], lane), qR = shfl_next(q[0], lane);
-#pragma unroll
-        for (int c = 0; c < Q; ++c) {
-          const double up = (c < Q - 1) ? v[c + 1] : vR, um = (c > 0) ? v[c - 1] : vL;
-          const double qr = (c < Q - 1) ? q[c + 1] : qR, ql = (c > 0) ? q[c - 1] : qL;
-          phi[t][c] = fma(a0, v[c], (up + um) * fma(-qs, up - um, e));
-          cc[t][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * q[c]));
-        }
-        if (has_mass) {
-          const double hm = fabs(fma(P.dx, warp_sum(msum), -M0));
-          minf[t] = fmax(minf[t], hm);
-          m1[t] += hm;
-        }
-        if (t < J) {
-#pragma unroll
-          for (int c = 0; c < Q; ++c) v[c] -= q[c];
-        } else {
-          double yv[Q];
-#pragma unroll
-          for (int c = 0; c < Q; ++c) yv[c] = q[c] - (v[c] - uhr[c]);
-          store_cells<Q>(so_y, lane, yv);
-        }
+      for (int c = 0; c < Q; ++c) {
+        const double h = v[c] - phi[t][c];
+        q[c] = h + cc[t][c];
+        const double wv = v[c] - cell_at<Q>(ruh, pp.lo, c);
+        const double ah = fabs(h);
+        hinf[t] = fmax(hinf[t], ah);
+        h1[t] += ah;
+        wd[t] = fma(wv, q[c], wd[t]);
+        dd[t] = fma(q[c], q[c], dd[t]);
+        if (t == 0) f2 = fma(wv, wv, f2);
+        msum += v[c];
       }
+      // end values of the next iterate (only the two ends are exchanged; the rest is updated in place below)
+      const double vn0 = (t < NU) ? v[0] - q[0] : v[0], vnE = (t < NU) ? v[Q - 1] - q[Q - 1] : v[Q - 1];
+      double qL = shfl_prev(q[Q - 1], lane), qR = shfl_next(q[0], lane);
+      double vnL = 0.0, vnR = 0.0;
+      if (t + 1 < T) { vnL = shfl_prev(vnE, lane); vnR = shfl_next(vn0, lane); }
+      double mtot = 0.0;
+      if constexpr (W > 1) {
+        const double ps = has_mass ? warp_sum(msum) : 0.0;
+        double* xs = pp.xch + (size_t)par * (W * 8);
+        if (lane == 0) { xs[w * 8 + 0] = q[0]; xs[w * 8 + 2] = vn0; xs[w * 8 + 4] = ps; }
+        if (lane == 31) { xs[w * 8 + 1] = q[Q - 1]; xs[w * 8 + 3] = vnE; }
+        pp.gsync();
+        if (lane == 0) { qL = xs[wl * 8 + 1]; vnL = xs[wl * 8 + 3]; }
+        if (lane == 31) { qR = xs[wr * 8 + 0]; vnR = xs[wr * 8 + 2]; }
+        if (has_mass) {
+#pragma unroll
+          for (int i = 0; i < W; ++i) mtot += xs[i * 8 + 4];
+        }
+        par ^= 1;
+      } else {
+        if (has_mass) mtot = warp_sum(msum);
+      }
+      if (has_mass && w == 0 && lane == 0) {
+        const double hm = fabs(fma(P.dx, mtot, -M0));
+        hinf[t] = fmax(hinf[t], hm);
+        h1[t] += hm;
+      }
+      // state for the next level (needs the old v and q with neighbours), then the update in place
+      double um = vL, ql = qL;
+#pragma unroll
+      for (int c = 0; c < Q; ++c) {
+        const double up = (c < Q - 1) ? v[c + 1] : vR;
+        const double qr = (c < Q - 1) ? q[c + 1] : qR;
+        const double vc = v[c], qc = q[c];
+        phi[t][c] = fma(a0, vc, (up + um) * fma(-qs, up - um, e));
+        cc[t][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
+        um = vc; ql = qc;
+        if (t < NU) v[c] = vc - qc;
+        else if (EMIT) q[c] = qc - (vc - cell_at<Q>(ruh, pp.lo, c));   // y
+      }
+      if (t < NU) { vL = vnL; vR = vnR; }
+      else store_cells<Q>(so_y, pp.lo, q);
     }
-    if (J > 0) store_cells<Q>(so_u, lane, v);
-    pp.store_rows(J > 0 ? xout + (size_t)k * nx : nullptr, so_u, T > J ? yout + (size_t)k * nx : nullptr, so_y);
-    if (k + nst < nt) pp.issue(s, x0 + (size_t)(k + nst) * nx, same ? nullptr : uh + (size_t)(k + nst) * nx);
+    if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
+    pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
+    // stage s is free: every warp loaded its cells before the first exchange barrier of this level
+    if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
     if (++s == nst) s = 0;
   }
   pp.drain();
-  f2 = warp_sum(f2);
-  S.f0 = 0.5 * f2;
+  // ---- reduce: lanes -> warp -> group (fixed order: identical in every warp, run-to-run deterministic) ----
+  double part[4 * T + 1];
 #pragma unroll
-  for (int t = 0; t < JT; ++t) {
-    if (t < T) {
-      double a = warp_max(hinf[t]), b = warp_sum(h1[t]);
-      const double c1 = -warp_sum(wd[t]), c2 = warp_sum(dd[t]);
-      if (has_mass) { a = fmax(a, minf[t]); b += m1[t]; }
-      S.hinf[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
-      // fmax drops NaN, the sums do not: a non-finite residual or direction shows up in h1 / dd
-      S.bad[t] = !(finite_d(a) && finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(f2));
+  for (int t = 0; t < T; ++t) {
+    part[4 * t + 0] = warp_max(hinf[t]);
+    part[4 * t + 1] = warp_sum(h1[t]);
+    part[4 * t + 2] = warp_sum(wd[t]);
+    part[4 * t + 3] = warp_sum(dd[t]);
+  }
+  part[4 * T] = warp_sum(f2);
+  if constexpr (W > 1) {
+    if (lane == 0) {
+#pragma unroll
+      for (int i = 0; i < 4 * T + 1; ++i) pp.red[w * kRed + i] = part[i];
     }
+    pp.gsync();
+#pragma unroll
+    for (int i = 0; i < 4 * T + 1; ++i) {
+      double acc = pp.red[i];
+#pragma unroll
+      for (int ww = 1; ww < W; ++ww) {
+        const double o = pp.red[ww * kRed + i];
+        acc = ((i & 3) == 0 && i < 4 * T) ? fmax(acc, o) : acc + o;
+      }
+      part[i] = acc;
+    }
+    pp.gsync();
+  }
+  S.f0 = 0.5 * part[4 * T];
+#pragma unroll
+  for (int t = 0; t < T; ++t) {
+    const double a = part[4 * t + 0], b = part[4 * t + 1];
+    const double c1 = -part[4 * t + 2], c2 = part[4 * t + 3];
+    S.hinf[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
+    // fmax drops NaN, the sums do not: a non-finite residual or direction shows up in h1 / dd
+    S.bad[t] = !(finite_d(a) && finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(part[4 * T]));
+  }
+  pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
+}
+
+// runtime (J, T) -> static instantiation
+template <int W, int Q, int JT>
+__device__ __forceinline__ void fused_fwd_dispatch(const DevParams& P, RowPipe<W, Q>& pp, const Buf x0, const Buf uh,
+                                                   const double* u0, const Buf xout, const Buf yout, int J, int T,
+                                                   double M0, FusedStats<JT>& S) {
+  if (T == J) {   // only the first pass: JT updates, no y
+    fused_fwd<W, Q, JT, JT, false>(P, pp, x0, uh, u0, xout, yout, M0, S);
+    return;
+  }
+  if (J == 0) fused_fwd<W, Q, JT, 0, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+  else if (J == 1) fused_fwd<W, Q, JT, 1, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+  else if (J == 2) {
+    if constexpr (JT >= 3) fused_fwd<W, Q, JT, 2, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+  } else if (J == 3) {
+    if constexpr (JT >= 4) fused_fwd<W, Q, JT, 3, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
   }
 }
 
@@ -249,30 +361,29 @@ __device__ void fused_fwd(const DevParams& P, RowPipe<Q>& pp, const double* __re
 // y is read from `lam`, which is overwritten in place; x is copied to `ucopy` when that is not null.
 // sig != nullptr: level sums of lam (input of the min-norm correction).  Returns sum(lam) (finite check).
 // ------------------------------------------------------------------------------------------------
-template <int Q>
-__device__ double fused_bwd(const DevParams& P, RowPipe<Q>& pp, const double* __restrict__ x, double* __restrict__ lam,
-                            double* __restrict__ ucopy, double* __restrict__ sig) {
-  constexpr int nx = RowGeom<Q>::NX;
-  const int nt = P.nt, lane = pp.lane, nst = pp.nst;
+template <int W, int Q>
+__device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x, const Buf lam,
+                                         const CUtensorMap* ucopy, double* __restrict__ sig) {
+  using G = RowGeom<W, Q>;
+  RowPipe<W, Q> pp = pp_ref;
+
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, w = pp.w, first = pp.first;
   const double a0 = P.bs_a0, e = P.bs_e, hs = P.bs_hs;
+  const int wl = (w + W - 1) % W, wr = (w + 1) % W;
   double lo[Q];
 #pragma unroll
   for (int c = 0; c < Q; ++c) lo[c] = 0.0;
-  double chk = 0.0;
+  double lL = 0.0, lR = 0.0, chk = 0.0;
   const int npro = nst < nt ? nst : nt;
-  for (int t = 0; t < npro; ++t) {
-    const size_t o = (size_t)(nt - 1 - t) * nx;
-    pp.issue(t, lam + o, x + o);
-  }
-  int s = 0;
+  for (int t = 0; t < npro; ++t) pp.issue(t, nt - 1 - t, lam.tm, x.tm);
+  int s = 0, par = 0;
   for (int t = 0; t < nt; ++t) {
     const int k = nt - 1 - t;
     pp.wait(s);
     double yv[Q], v[Q], l[Q];
-    load_cells<Q>(pp.row(s, 0), lane, yv);
-    load_cells<Q>(pp.row(s, 1), lane, v);
+    load_cells<Q>(pp.row(s, 0), pp.lo, yv);
+    load_cells<Q>(pp.row(s, 1), pp.lo, v);
     pp.out_ready();
-    const double lL = shfl_prev(lo[Q - 1], lane), lR = shfl_next(lo[0], lane);
     double lsum = 0.0;
 #pragma unroll
     for (int c = 0; c < Q; ++c) {
@@ -282,38 +393,53 @@ __device__ double fused_bwd(const DevParams& P, RowPipe<Q>& pp, const double* __
     }
 #pragma unroll
     for (int c = 0; c < Q; ++c) lo[c] = l[c];
-    chk += lsum;
-    if (sig) {
-      const double sk = warp_sum(lsum);
-      if (lane == 0) sig[k] = sk;
+    lL = shfl_prev(l[Q - 1], lane);
+    lR = shfl_next(l[0], lane);
+    double stot = (sig || W > 1) ? warp_sum(lsum) : 0.0;
+    if constexpr (W > 1) {
+      double* xs = pp.xch + (size_t)par * (W * 8);
+      if (lane == 0) { xs[w * 8 + 0] = l[0]; xs[w * 8 + 4] = stot; }
+      if (lane == 31) xs[w * 8 + 1] = l[Q - 1];
+      pp.gsync();
+      if (lane == 0) lL = xs[wl * 8 + 1];
+      if (lane == 31) lR = xs[wr * 8 + 0];
+      stot = 0.0;
+#pragma unroll
+      for (int i = 0; i < W; ++i) stot += xs[i * 8 + 4];
+      par ^= 1;
+      chk += stot;
+    } else {
+      chk += lsum;
     }
+    if (sig && w == 0 && lane == 0) sig[k] = stot;
     double* so_l = pp.out(t & 1);
     double* so_u = pp.out(2 + (t & 1));
-    store_cells<Q>(so_l, lane, l);
-    if (ucopy) store_cells<Q>(so_u, lane, v);
-    pp.store_rows(lam + (size_t)k * nx, so_l, ucopy ? ucopy + (size_t)k * nx : nullptr, so_u);
-    if (t + nst < nt) {
-      const size_t o = (size_t)(k - nst) * nx;
-      pp.issue(s, lam + o, x + o);
-    }
+    store_cells<Q>(so_l, pp.lo, l);
+    if (ucopy) store_cells<Q>(so_u, pp.lo, v);
+    pp.store_rows(k, lam.tm, so_l, ucopy, so_u);
+    if (t + nst < nt) pp.issue(s, k - nst, lam.tm, x.tm);
     if (++s == nst) s = 0;
   }
   pp.drain();
-  return warp_sum(chk);
+  pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
+  return (W > 1) ? chk : warp_sum(chk);
 }
 
 // Minimum-norm multiplier for the linearly dependent mass rows of kind 4 (streaming
 // recipe): with level sums sigma_j of the basic solution (mass multipliers 0) and c = nx dx^2,
 //   (D^T D + c I) t = -dx D^T sigma ,  lam_mass[k] = -t_k ,  lam_loc[j][.] += dx sum_{k>=j} t_k
 // (D = first difference).  The rank-nt update of lam is one more streaming pass through the row pipe.
-template <int Q>
-__device__ void fused_min_norm(const DevParams& P, RowPipe<Q>& pp, double* __restrict__ lam, double* __restrict__ sig,
-                               double* __restrict__ tt) {
-  constexpr int nx = RowGeom<Q>::NX;
-  const int nt = P.nt, lane = pp.lane, nst = pp.nst;
+template <int W, int Q>
+__device__ __noinline__ void fused_min_norm(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf lamb,
+                                            double* __restrict__ sig, double* __restrict__ tt) {
+  using G = RowGeom<W, Q>;
+  RowPipe<W, Q> pp = pp_ref;
+  constexpr int nx = G::NX;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
   const double c = (double)nx * P.dx * P.dx;
-  __syncwarp();
-  if (lane == 0) {
+  __threadfence_block();
+  pp.gsync();
+  if (pp.w == 0 && lane == 0) {
     // Thomas on the SPD tridiagonal diag (2+c, ..., 2+c, 1+c), off-diagonals -1
     double cp = 0.0, dp = 0.0;
     for (int k = 0; k < nt; ++k) {
@@ -333,59 +459,71 @@ __device__ void fused_min_norm(const DevParams& P, RowPipe<Q>& pp, double* __res
       suf += x;
       sig[k] = suf;
     }
+    __threadfence_block();
   }
-  __syncwarp();
-  double* lmass = lam + (size_t)nt * nx;
-  for (int k = lane; k < nt; k += 32) lmass[k] = -tt[k];
+  pp.gsync();
+  double* lmass = lamb.p + (size_t)nt * nx;
+  for (int k = pp.w * 32 + lane; k < nt; k += W * 32) lmass[k] = -tt[k];
   const int npro = nst < nt ? nst : nt;
-  for (int k = 0; k < npro; ++k) pp.issue(k, lam + (size_t)k * nx, nullptr);
+  for (int k = 0; k < npro; ++k) pp.issue(k, k, lamb.tm, nullptr);
   int s = 0;
   for (int k = 0; k < nt; ++k) {
     pp.wait(s);
     double l[Q];
-    load_cells<Q>(pp.row(s, 0), lane, l);
+    load_cells<Q>(pp.row(s, 0), pp.lo, l);
     pp.out_ready();
     const double add = P.dx * sig[k];
 #pragma unroll
     for (int cidx = 0; cidx < Q; ++cidx) l[cidx] += add;
     double* so = pp.out(k & 1);
-    store_cells<Q>(so, lane, l);
-    pp.store_rows(lam + (size_t)k * nx, so, nullptr, nullptr);
-    if (k + nst < nt) pp.issue(s, lam + (size_t)(k + nst) * nx, nullptr);
+    store_cells<Q>(so, pp.lo, l);
+    pp.store_rows(k, lamb.tm, so, nullptr, nullptr);
+    if constexpr (W > 1) pp.gsync();   // every warp has read stage s
+    if (k + nst < nt) pp.issue(s, k + nst, lamb.tm, nullptr);
     if (++s == nst) s = 0;
   }
   pp.drain();
+  pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
 }
 
 // ------------------------------------------------------------------------------------------------
-// the persistent Gauss-Newton driver (a8, a9)
+// the persistent Gauss-Newton driver (a8, a9); every warp of a group runs it with identical values
 // ------------------------------------------------------------------------------------------------
-template <int Q, int JT>
-__global__ void __launch_bounds__(256) project1d_fused_kernel(const __grid_constant__ Proj1dArgs A) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  using G = RowGeom<Q>;
+template <int W, int Q, int JT, int MAXT>
+__global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_constant__ Proj1dArgs A) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  using G = RowGeom<W, Q>;
   const DevParams& P = A.P;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int b = blockIdx.x * (blockDim.x >> 5) + warp;
-  if (b >= A.batch) return;
+  const int gwarp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int slot = gwarp / W, w = gwarp % W;
+  const int b = blockIdx.x * (blockDim.x / (32 * W)) + slot;
+  if (b >= A.batch) return;   // whole groups leave together: the named barriers of the others are unaffected
   constexpr int nx = G::NX;
   const int nt = P.nt;
   const size_t n = (size_t)P.n;
+  const int gtid = w * 32 + lane;
+  constexpr int GT = W * 32;
 
-  unsigned char* base = smem_raw + (size_t)warp * A.warp_bytes;
-  RowPipe<Q> pp;
+  // swizzled rows need 1024-byte aligned bases: align the CTA's window, per-sample strides are multiples of 1024
+  unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) + (size_t)slot * A.warp_bytes;
+  RowPipe<W, Q> pp;
   pp.stage = reinterpret_cast<double*>(base);
   pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;
-  pp.bar0 = smem_u32(pp.orow + (size_t)4 * G::RP);
+  pp.xch = pp.orow + (size_t)4 * G::RP;
+  pp.red = pp.xch + G::XCH;
+  pp.bar0 = smem_u32(pp.red + W * kRed);
   pp.phase = 0;
-  pp.nst = A.nst; pp.lane = lane;
+  pp.nst = A.nst; pp.lane = lane; pp.w = w; pp.bar_id = 1 + slot;
+  pp.first = (w * 32 + lane) * Q;
+  pp.b = b;
+  pp.lo.init(pp.first);
   pp.rows_rd = 0; pp.rows_wr = 0;
-  if (lane == 0) {
+  if (gtid == 0) {
     for (int s = 0; s < A.nst; ++s) mbar_init(pp.bar0 + 8u * s, 1);
     mbar_fence_init();
     fence_proxy_async_smem();
   }
-  __syncwarp();
+  pp.gsync();
 
   const double* uh = A.u_hat + (size_t)b * n;
   const double* u0 = A.cdata + (size_t)b * nx;
@@ -395,12 +533,21 @@ __global__ void __launch_bounds__(256) project1d_fused_kernel(const __grid_const
   double* bufB = A.bufB + (size_t)b * n;
   double* sig = A.aux + (size_t)b * 2 * nt;
   double* tt = sig + nt;
+  // sample base pointer -> (tensor map, pointer); u_star may alias u_hat (same map contents)
+  auto mk = [&](const double* q) -> Buf {
+    const CUtensorMap* t = nullptr;
+    if (q == uh) t = &A.tm[TM_UHAT];
+    else if (q == bufA) t = &A.tm[TM_BUFA];
+    else if (q == bufB) t = &A.tm[TM_BUFB];
+    else if (q == ustar) t = &A.tm[TM_USTAR];
+    else if (q == lam) t = &A.tm[TM_LAM];
+    return Buf{t, const_cast<double*>(q)};
+  };
 
   double M0 = 0.0;
-  if (P.has_mass) {
+  if (P.has_mass) {   // every warp sums the whole u0 row in the same order: identical M0 in the group
     double sm = 0.0;
-#pragma unroll
-    for (int c = 0; c < Q; ++c) sm += u0[Q * lane + c];
+    for (int i = lane; i < nx; i += 32) sm += u0[i];
     M0 = P.dx * warp_sum(sm);
   }
   // iterates ping-pong between two buffers; u_star itself serves as one of them unless it aliases u_hat
@@ -433,14 +580,13 @@ __global__ void __launch_bounds__(256) project1d_fused_kernel(const __grid_const
       J = 0;                                  // classic trial evaluation: `cur` lives in the other work buffer
     } else {
       J = jcap;
-      if (sweeps > 0 && J > JT - 1) J = JT - 1;
       const int budget = P.max_iter - steps - (pend ? 1 : 0);
       if (J > budget) J = budget;
     }
-    if (J > JT - 1 && (sweeps > 0 || conv)) J = JT - 1;
+    if (J > JT - 1 && (sweeps > 0 || conv || jcap < JT)) J = JT - 1;
     if (J < 0) J = 0;
     const int T = (J < JT) ? J + 1 : J;
-    fused_fwd<Q, JT>(P, pp, x0, uh, u0, xo, lam, J, T, M0, S);
+    fused_fwd_dispatch<W, Q, JT>(P, pp, mk(x0), mk(uh), u0, mk(xo), mk(lam), J, T, M0, S);
     ++sweeps;
 
     // ---- a pending step is judged by iteration 0 of this pass ---------------------------------------------
@@ -454,10 +600,10 @@ __global__ void __launch_bounds__(256) project1d_fused_kernel(const __grid_const
           continue;
         }
         if (++tries > P.ls_max) { status = SNAP_ST_LINESEARCH; break; }
-        for (size_t i = lane; i < n; i += 32) trial[i] = fma(P.ls_shrink, trial[i] - cur[i], cur[i]);
+        for (size_t i = gtid; i < n; i += GT) trial[i] = fma(P.ls_shrink, trial[i] - cur[i], cur[i]);
         __threadfence();
         fence_proxy_async_all();
-        __syncwarp();
+        pp.gsync();
         alpha *= P.ls_shrink;
         jcap = 1;
         continue;
@@ -527,10 +673,10 @@ __global__ void __launch_bounds__(256) project1d_fused_kernel(const __grid_const
     if (backtrack) {      // first reduction of the step x_0 -> x_1 (mu, phi_cur, Dphi are those of this step)
       trial = xo;
       if (++tries > P.ls_max) { status = SNAP_ST_LINESEARCH; break; }
-      for (size_t i = lane; i < n; i += 32) trial[i] = fma(P.ls_shrink, trial[i] - cur[i], cur[i]);
+      for (size_t i = gtid; i < n; i += GT) trial[i] = fma(P.ls_shrink, trial[i] - cur[i], cur[i]);
       __threadfence();
       fence_proxy_async_all();
-      __syncwarp();
+      pp.gsync();
       alpha = P.ls_shrink;
       pend = true; pend_J = 1; jcap = 1;
       continue;
@@ -554,40 +700,54 @@ __global__ void __launch_bounds__(256) project1d_fused_kernel(const __grid_const
   long long* stat = A.stats ? A.stats + (size_t)b * 4 : nullptr;
   if (status == SNAP_ST_NONFINITE) {  // R16: u* = u_hat, lam = 0
     if (ustar != uh)
-      for (size_t i = lane; i < n; i += 32) ustar[i] = uh[i];
-    for (size_t i = lane; i < (size_t)P.m; i += 32) lam[i] = 0.0;
+      for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
+    for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
   } else {
     if (status == SNAP_ST_LINESEARCH) {   // multiplier at the last accepted iterate (as the oracle returns it)
-      fused_fwd<Q, JT>(P, pp, cur, uh, u0, nullptr, lam, 0, 1, M0, S);
+      fused_fwd_dispatch<W, Q, JT>(P, pp, mk(cur), mk(uh), u0, Buf{nullptr, nullptr}, mk(lam), 0, 1, M0, S);
       ++sweeps;
       xfin = cur;
     }
     const bool want_sig = (P.kind == SNAP_BURGERS1D_LF_MASS) && (P.lambda_mode == 0);
-    const double chk = fused_bwd<Q>(P, pp, xfin, lam, (xfin != ustar) ? ustar : nullptr, want_sig ? sig : nullptr);
+    const double chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), (xfin != ustar) ? &A.tm[TM_USTAR] : nullptr,
+                                       want_sig ? sig : nullptr);
+    ++sweeps;
     if (!finite_d(chk)) {
       status = SNAP_ST_NONFINITE;
-      __syncwarp();
-      for (size_t i = lane; i < n; i += 32) ustar[i] = uh[i];
-      for (size_t i = lane; i < (size_t)P.m; i += 32) lam[i] = 0.0;
+      pp.gsync();
+      for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
+      for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
     } else if (P.has_mass) {
-      if (want_sig) fused_min_norm<Q>(P, pp, lam, sig, tt);
-      else
-        for (int k = lane; k < nt; k += 32) lam[n + k] = 0.0;
+      if (want_sig) {
+        fused_min_norm<W, Q>(P, pp, mk(lam), sig, tt);
+        ++sweeps;
+      } else {
+        for (int k = gtid; k < nt; k += GT) lam[n + k] = 0.0;
+      }
     }
   }
-  if (lane == 0) {
+  if (gtid == 0) {
     A.iters[b] = (status == 0) ? solves : status;
     if (stat) { stat[0] = solves; stat[1] = sweeps; stat[2] = pp.rows_rd; stat[3] = pp.rows_wr; }
   }
 }
 
-template <int Q, int JT>
+template <int W, int Q, int JT, int MAXT>
 inline int launch_fused_variant(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
-  auto kern = project1d_fused_kernel<Q, JT>;
+  auto kern = project1d_fused_kernel<W, Q, JT, MAXT>;
+  if (pl.wpc * W * 32 > MAXT) return SNAP_EINVAL;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
     return SNAP_ECUDA;
-  kern<<<pl.grid, pl.wpc * 32, pl.smem, st>>>(a);
-  return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+  kern<<<pl.grid, pl.wpc * W * 32, pl.smem, st>>>(a);
+  const cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess && getenv("SNAP_DEBUG")) {
+    cudaFuncAttributes fa;
+    cudaFuncGetAttributes(&fa, kern);
+    fprintf(stderr, "snap: fused<%d,%d,%d,%d> launch failed: %s; grid %d block %d smem %zu; regs %d maxThreads %d local %zu\n",
+            W, Q, JT, MAXT, cudaGetErrorString(err), pl.grid, pl.wpc * W * 32, pl.smem, fa.numRegs, fa.maxThreadsPerBlock,
+            fa.localSizeBytes);
+  }
+  return err == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
 }
 
 }  // namespace snap

@@ -1,12 +1,17 @@
 // Host-side launch interfaces between the translation units of libsnap (not part of the C ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "snap_internal.h"
 
 namespace snap {
 
+// buffers of the fused path addressed through tensor maps (one row = one box)
+enum { TM_UHAT = 0, TM_BUFA = 1, TM_BUFB = 2, TM_USTAR = 3, TM_LAM = 4, TM_COUNT = 5 };
+
 struct Proj1dArgs {
+  alignas(64) CUtensorMap tm[TM_COUNT];   // fused path only: [sample][line of 16 doubles][16], 128-byte swizzle
   DevParams P;
   int batch, warm;
   const double* u_hat;
@@ -26,6 +31,8 @@ struct Proj1dArgs {
 
 struct Plan1d {
   int q, wpc, nst, rp, warp_bytes, grid;
+  int wps;       // fused path: warps per sample
+  int variant;   // fused path: tuning variant of the nx = 256 instantiation (0 = default)
   bool full;  // nx == 32 q: no bounds checks in the sweeps
   bool tma;   // every row start is 16-byte aligned: bulk (TMA) copies; otherwise plain loads/stores
   size_t smem;
@@ -38,7 +45,9 @@ int launch_project1d_burgers(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t
 int launch_project1d_fisher(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
 // proj1d_burgers_fused.cu: nx = 32 q, bulk-copy alignment required; pl.rp / pl.warp_bytes follow plan_fused()
 int launch_project1d_burgers_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
-int fused_row_pitch(int q);   // padded shared-memory row pitch in doubles
+int fused_row_pitch(int nx);   // padded shared-memory row pitch in doubles
+// (warps per sample, cells per lane, iterations per pass, max threads per CTA) of the instantiation for nx
+bool fused_variant(int nx, int variant, int& W, int& Q, int& JT, int& maxt);
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, cudaStream_t st);
 

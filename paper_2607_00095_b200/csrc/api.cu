@@ -223,6 +223,12 @@ int snap_problem_destroy(snap_problem* p) {
   if (!p) return SNAP_EINVAL;
   if (p->d_green) cudaFree(p->d_green);
   if (p->stage) cudaFree(p->stage);
+  if (p->s_in) {
+    cudaStreamDestroy(p->s_in);
+    cudaStreamDestroy(p->s_out);
+    for (int i = 0; i < kHostChunksMax; ++i) { cudaEventDestroy(p->ev_in[i]); cudaEventDestroy(p->ev_k[i]); }
+    cudaEventDestroy(p->ev_done);
+  }
   delete p;
   return SNAP_OK;
 }
@@ -306,10 +312,17 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
   if (!u_hat_host || !cdata_host || !u_star_host || !lambda_host || !iters_host) return SNAP_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const DevParams& d = p->dp;
-  const size_t B = (size_t)batch;
-  const size_t b_u = align_up(B * d.n * 8, 256), b_c = align_up(B * d.lvl * 8, 256), b_l = align_up(B * d.m * 8, 256),
-               b_i = align_up(B * 4, 256), b_w = align_up(snap_workspace_bytes(p, batch), 256);
-  const size_t total = 2 * b_u + b_c + b_l + b_i + b_w;
+  // The batch is cut into chunks of samples (independent blocks) that flow through three
+  // streams: host->device copy of chunk c+1, projection of chunk c and device->host copy of chunk c-1 overlap,
+  // so that both directions of the host link are busy at once.
+  int nchunk = batch >= 512 ? 4 : (batch >= 128 ? 2 : 1);
+  const int cb = (batch + nchunk - 1) / nchunk;            // samples per chunk
+  nchunk = (batch + cb - 1) / cb;
+  const size_t C = (size_t)cb;
+  const size_t b_u = align_up(C * d.n * 8, 256), b_c = align_up(C * d.lvl * 8, 256), b_l = align_up(C * d.m * 8, 256),
+               b_i = align_up(C * 4, 256), b_w = align_up(snap_workspace_bytes(p, cb), 256);
+  const size_t per_chunk = 2 * b_u + b_c + b_l + b_i + b_w;
+  const size_t total = per_chunk * nchunk;
   if (p->stage_bytes < total) {
     if (p->stage) cudaFree(p->stage);
     p->stage = nullptr;
@@ -317,22 +330,45 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
     if (cudaMalloc(&p->stage, total) != cudaSuccess) return SNAP_ENOMEM;
     p->stage_bytes = total;
   }
-  unsigned char* s = static_cast<unsigned char*>(p->stage);
-  double* d_uh = reinterpret_cast<double*>(s);
-  double* d_us = reinterpret_cast<double*>(s + b_u);
-  double* d_c = reinterpret_cast<double*>(s + 2 * b_u);
-  double* d_l = reinterpret_cast<double*>(s + 2 * b_u + b_c);
-  int* d_i = reinterpret_cast<int*>(s + 2 * b_u + b_c + b_l);
-  void* d_w = s + 2 * b_u + b_c + b_l + b_i;
-  if (cudaMemcpyAsync(d_uh, u_hat_host, B * d.n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return SNAP_ECUDA;
-  if (cudaMemcpyAsync(d_c, cdata_host, B * d.lvl * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return SNAP_ECUDA;
-  if (warm && cudaMemcpyAsync(d_l, lambda_host, B * d.m * 8, cudaMemcpyHostToDevice, st) != cudaSuccess)
+  if (!p->s_in) {
+    if (cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) != cudaSuccess)
+      return SNAP_ECUDA;
+    for (int i = 0; i < kHostChunksMax; ++i)
+      if (cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&p->ev_k[i], cudaEventDisableTiming) != cudaSuccess)
+        return SNAP_ECUDA;
+    if (cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) != cudaSuccess) return SNAP_ECUDA;
+  }
+  // order the copy streams after whatever the caller has already enqueued on `stream`
+  if (cudaEventRecord(p->ev_done, st) != cudaSuccess || cudaStreamWaitEvent(p->s_in, p->ev_done, 0) != cudaSuccess)
     return SNAP_ECUDA;
-  const int rc = snap_project(p, batch, d_uh, d_c, d_us, d_l, d_i, warm, d_w, stream);
-  if (rc != SNAP_OK) return rc;
-  if (cudaMemcpyAsync(u_star_host, d_us, B * d.n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
-  if (cudaMemcpyAsync(lambda_host, d_l, B * d.m * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
-  if (cudaMemcpyAsync(iters_host, d_i, B * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return SNAP_ECUDA;
+  for (int c = 0; c < nchunk; ++c) {
+    const int b0 = c * cb, nb = (batch - b0 < cb) ? batch - b0 : cb;
+    const size_t B = (size_t)nb;
+    unsigned char* s = static_cast<unsigned char*>(p->stage) + (size_t)c * per_chunk;
+    double* d_uh = reinterpret_cast<double*>(s);
+    double* d_us = reinterpret_cast<double*>(s + b_u);
+    double* d_c = reinterpret_cast<double*>(s + 2 * b_u);
+    double* d_l = reinterpret_cast<double*>(s + 2 * b_u + b_c);
+    int* d_i = reinterpret_cast<int*>(s + 2 * b_u + b_c + b_l);
+    void* d_w = s + 2 * b_u + b_c + b_l + b_i;
+    bool ok = cudaMemcpyAsync(d_uh, u_hat_host + (size_t)b0 * d.n, B * d.n * 8, cudaMemcpyHostToDevice, p->s_in) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(d_c, cdata_host + (size_t)b0 * d.lvl, B * d.lvl * 8, cudaMemcpyHostToDevice, p->s_in) == cudaSuccess;
+    if (warm)
+      ok = ok && cudaMemcpyAsync(d_l, lambda_host + (size_t)b0 * d.m, B * d.m * 8, cudaMemcpyHostToDevice, p->s_in) == cudaSuccess;
+    ok = ok && cudaEventRecord(p->ev_in[c], p->s_in) == cudaSuccess && cudaStreamWaitEvent(st, p->ev_in[c], 0) == cudaSuccess;
+    if (!ok) return SNAP_ECUDA;
+    const int rc = snap_project(p, nb, d_uh, d_c, d_us, d_l, d_i, warm, d_w, stream);
+    if (rc != SNAP_OK) return rc;
+    ok = cudaEventRecord(p->ev_k[c], st) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_k[c], 0) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(u_star_host + (size_t)b0 * d.n, d_us, B * d.n * 8, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(lambda_host + (size_t)b0 * d.m, d_l, B * d.m * 8, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(iters_host + b0, d_i, B * 4, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
+    if (!ok) return SNAP_ECUDA;
+  }
+  if (cudaEventRecord(p->ev_done, p->s_out) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_done, 0) != cudaSuccess)
+    return SNAP_ECUDA;
   return cudaStreamSynchronize(st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
 }
 

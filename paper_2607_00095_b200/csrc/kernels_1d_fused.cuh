@@ -232,13 +232,14 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
     double* so_y = pp.out(2 + (k & 1));
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-      double q[Q];
+      double q[Q], uhr[Q];
       double msum = 0.0;
+      load_cells<Q>(ruh, pp.lo, uhr);   // 128-bit conflict-free reads; not kept across iterations (registers)
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         const double h = v[c] - phi[t][c];
         q[c] = h + cc[t][c];
-        const double wv = v[c] - cell_at<Q>(ruh, pp.lo, c);
+        const double wv = v[c] - uhr[c];
         const double ah = fabs(h);
         hinf[t] = fmax(hinf[t], ah);
         h1[t] += ah;
@@ -285,7 +286,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         cc[t][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
         um = vc; ql = qc;
         if (t < NU) v[c] = vc - qc;
-        else if (EMIT) q[c] = qc - (vc - cell_at<Q>(ruh, pp.lo, c));   // y
+        else if (EMIT) q[c] = qc - (vc - uhr[c]);   // y
       }
       if (t < NU) { vL = vnL; vR = vnR; }
       else store_cells<Q>(so_y, pp.lo, q);

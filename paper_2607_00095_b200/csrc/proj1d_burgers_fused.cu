@@ -11,11 +11,8 @@ bool fused_variant(int nx, int variant, int& W, int& Q, int& JT, int& maxt) {
     case 64: W = 1; Q = 2; JT = 4; maxt = 256; return true;
     case 128: W = 1; Q = 4; JT = 4; maxt = 256; return true;
     case 256:
-      switch (variant) {
-        case 1: W = 2; Q = 4; JT = 3; maxt = 448; return true;
-        case 2: W = 2; Q = 4; JT = 4; maxt = 448; return true;
-        default: W = 1; Q = 8; JT = 3; maxt = 256; return true;
-      }
+      (void)variant;
+      W = 1; Q = 8; JT = 3; maxt = 256; return true;
     case 512: W = 2; Q = 8; JT = 3; maxt = 256; return true;
   }
   return false;
@@ -29,11 +26,7 @@ int launch_project1d_burgers_fused(const Proj1dArgs& a, const Plan1d& pl, cudaSt
     case 64: return launch_fused_variant<1, 2, 4, 256>(a, pl, st);
     case 128: return launch_fused_variant<1, 4, 4, 256>(a, pl, st);
     case 256:
-      switch (pl.variant) {
-        case 1: return launch_fused_variant<2, 4, 3, 448>(a, pl, st);
-        case 2: return launch_fused_variant<2, 4, 4, 448>(a, pl, st);
-        default: return launch_fused_variant<1, 8, 3, 256>(a, pl, st);
-      }
+      return launch_fused_variant<1, 8, 3, 256>(a, pl, st);
     case 512: return launch_fused_variant<2, 8, 3, 256>(a, pl, st);
   }
   return SNAP_EINVAL;

@@ -303,3 +303,77 @@ def test_host_buffer_entry_point(S):
     np.testing.assert_array_equal(lam.numpy(), ref["lam"])
     np.testing.assert_array_equal(it.numpy(), ref["iters"])
     p.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# fused Gauss-Newton passes (Burgers kinds, nx = 32 * 2^j): every mode must reach the oracle's point
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", [2, 5])
+@pytest.mark.parametrize("gn_fuse", [-1, 1, 2, 0])
+def test_fused_pass_modes_agree_with_oracle(S, cfg, gn_fuse):
+    """gn_fuse = -1 classic sweeps, 1 / 2 / 0 (= max) iterations per forward pass: same limit point."""
+    for kw in (dict(batch=3, nx=32, nt=33), dict(batch=2, nx=64, nt=40), dict(batch=2, nx=128, nt=24)):
+        wl = W.make_workload(cfg, **kw)
+        g = gpu_project(S, wl, wl.u_hat, params=dict(gn_fuse=gn_fuse))
+        assert g["norms"][:, 0].max() < 1e-10
+        check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
+
+
+def test_fused_path_wide_rows_two_warps_per_sample(S):
+    """nx = 512 runs the fused kernel with two warps per sample (end cells exchanged through shared memory)."""
+    for cfg in (2, 5):
+        wl = W.make_workload(cfg, batch=2, nx=512, nt=12)
+        g = gpu_project(S, wl, wl.u_hat)
+        assert g["norms"][:, 0].max() < 1e-10
+        check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
+
+
+def test_fused_path_line_search_and_status_codes(S):
+    """R17 on a fused size: forced Armijo halving falls back to one iteration per pass and reaches the same
+    point; exhausted back-tracking, max_iter and non-finite inputs report their status."""
+    wl = W.make_workload(2, batch=2, nx=32, nt=20, noise=1.0)
+    ref = gpu_project(S, wl, wl.u_hat)
+    forced = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.9))
+    assert (forced["iters"] > ref["iters"]).all()
+    np.testing.assert_allclose(forced["u"], ref["u"], rtol=0, atol=1e-11)
+    check_against_oracle(wl, wl.u_hat, forced, range(wl.batch), params=dict(ls_c1=0.9))
+    stuck = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.9, ls_max=0))
+    assert (stuck["iters"] == -2).all()
+    o = O.project(wl.kind, wl.u_hat[0].numpy(), wl.cdata[0].numpy(), dict(wl.params, ls_c1=0.9, ls_max=0))
+    assert o["status"] == -2
+    np.testing.assert_allclose(stuck["u"][0], o["u"], rtol=0, atol=1e-12)
+    capped = gpu_project(S, wl, wl.u_hat, params=dict(max_iter=1))
+    assert (capped["iters"] == -1).all()
+    o = O.project(wl.kind, wl.u_hat[0].numpy(), wl.cdata[0].numpy(), dict(wl.params, max_iter=1))
+    np.testing.assert_allclose(capped["u"][0], o["u"], rtol=0, atol=1e-12)
+    np.testing.assert_allclose(capped["lam"][0], o["lam"], rtol=0, atol=1e-9 * np.abs(o["lam"]).max())
+    wl = W.make_workload(2, batch=2, nx=32, nt=200)
+    big = wl.u_hat * 1e155
+    g = gpu_project(S, wl, big)
+    assert (g["iters"] == -3).all()
+    np.testing.assert_array_equal(g["u"], big.numpy())
+    assert np.all(g["lam"] == 0)
+
+
+def test_project_stats_counts_the_rows_moved(S):
+    """snap_project_stats: rows read / written by the fused passes are consistent with the pass structure."""
+    dev = torch.device("cuda:0")
+    wl = W.make_workload(5, batch=3, nx=64, nt=40)
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    B = wl.batch
+    uh = wl.u_hat.to(dev)
+    us = torch.empty_like(uh)
+    lam = torch.zeros(B, p.m, dtype=torch.float64, device=dev)
+    it = torch.zeros(B, dtype=torch.int32, device=dev)
+    ws = S.snap_project(p, B, uh, wl.cdata.to(dev), us, lam, it)
+    st = torch.zeros(B, 4, dtype=torch.int64, device=dev)
+    S.snap_project_stats(p, B, ws, st)
+    torch.cuda.synchronize()
+    st = st.cpu().numpy()
+    assert (st[:, 0] == it.cpu().numpy()).all()
+    nt = wl.nt
+    assert (st[:, 2] % nt == 0).all() and (st[:, 3] % nt == 0).all()
+    # at least: one forward pass (u_hat in, iterate out), y emission, multiplier sweep (y, u in; lam out), correction
+    assert (st[:, 2] >= 5 * nt).all() and (st[:, 3] >= 4 * nt).all()
+    assert (st[:, 1] >= 4).all()
+    p.destroy()

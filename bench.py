@@ -33,6 +33,7 @@ import workloads as W  # noqa: E402
 METRIC = "projected samples/sec to ||h||inf<1e-10 (fp64, 1 B200); % of HBM roofline"
 UNIT = "projections/s"
 N_TAU = 50
+PROFILED_TRAFFIC_CFG5 = 5.831e9   # bytes, see profiles/r01c_project1d_fused.md
 
 
 def load_peaks():
@@ -325,6 +326,12 @@ def run_gpu(args):
     peak, peak_src = load_peaks()
     solves = iters.clamp(min=0).sum(dim=1).to(torch.float64)        # per call, over the batch
     alg_bytes_call = run.traffic_model()
+    traffic, traffic_note = args.traffic, None
+    if traffic is None and cfg == 5:
+        # ncu --set full capture of the first two launches of the timed step (tau = 1/50, 2/50), profiles/r01c_*.md
+        traffic = PROFILED_TRAFFIC_CFG5
+        traffic_note = ("dram__bytes_read.sum + dram__bytes_write.sum of launch 0 (tau=1/50), profiles/r01c_project1d_fused.md; "
+                        f"algorithmic bytes of that launch: {alg_bytes_call[0]:.4g}")
     kern_s = sum(sum(k) for k in kern_ms) * 1e-3
     alg_total = sum(alg_bytes_call) * args.steps
     achieved = alg_total / kern_s / 1e9
@@ -340,7 +347,10 @@ def run_gpu(args):
                    "mean_linearisations_per_projection": float(solves.sum() / (run.B * run.calls)),
                    "alg_bytes_per_projection": sum(alg_bytes_call) / (run.B * run.calls)},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": args.traffic, "kernel": "project1d_kernel" if cfg != 4 else "project2d_kernel",
+                     "traffic": traffic, "traffic_note": traffic_note,
+                     "kernel": {5: "project1d_fused_kernel<1,8,3,256>", 2: "project1d_fused_kernel<1,4,4,256>",
+                                3: "project1d_kernel<2,4,0,1> (Fisher, classic sweeps)", 4: "project2d_kernel",
+                                1: "heat_project_kernel"}[cfg],
                      "peak_source": peak_src, "alg_bytes_per_launch_mean": alg_total / (args.steps * run.calls),
                      "launch_ms_mean": 1e3 * kern_s / (args.steps * run.calls),
                      "frac_of_8TBs_spec": achieved / 8000.0},

@@ -85,6 +85,51 @@ __device__ __forceinline__ void store_cells(double* row, const LaneOff<Q>& lo, c
 __device__ __forceinline__ double shfl_prev(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 31) & 31); }
 __device__ __forceinline__ double shfl_next(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 1) & 31); }
 
+#ifndef SNAP_CC_SMEM
+#define SNAP_CC_SMEM 0
+#endif
+constexpr bool kCcSmem = SNAP_CC_SMEM != 0;   // keep (A_{k-1} q_{k-1}) of every iteration in shared memory, not registers
+
+// per-lane private vectors of Q doubles in shared memory, slot-major so that a warp's 128-bit accesses are conflict free
+template <int Q>
+__device__ __forceinline__ void ld_priv(const double* base, int slot, int lane, double (&x)[Q]) {
+  if constexpr (Q == 1) {
+    x[0] = base[slot * 32 + lane];
+  } else {
+#pragma unroll
+    for (int c = 0; c < Q / 2; ++c) {
+      const double2 t = reinterpret_cast<const double2*>(base)[(slot * (Q / 2) + c) * 32 + lane];
+      x[2 * c] = t.x;
+      x[2 * c + 1] = t.y;
+    }
+  }
+}
+template <int Q>
+__device__ __forceinline__ void st_priv(double* base, int slot, int lane, const double (&x)[Q]) {
+  if constexpr (Q == 1) {
+    base[slot * 32 + lane] = x[0];
+  } else {
+#pragma unroll
+    for (int c = 0; c < Q / 2; ++c)
+      reinterpret_cast<double2*>(base)[(slot * (Q / 2) + c) * 32 + lane] = make_double2(x[2 * c], x[2 * c + 1]);
+  }
+}
+
+// balanced sum of a lane's Q values (dependency depth log2 Q instead of Q)
+template <int Q>
+__device__ __forceinline__ double tree_sum(const double (&x)[Q]) {
+  if constexpr (Q == 1) return x[0];
+  else if constexpr (Q == 2) return x[0] + x[1];
+  else if constexpr (Q == 4) return (x[0] + x[1]) + (x[2] + x[3]);
+  else if constexpr (Q == 8) return ((x[0] + x[1]) + (x[2] + x[3])) + ((x[4] + x[5]) + (x[6] + x[7]));
+  else {
+    double a = 0.0, b = 0.0, c = 0.0, d = 0.0;
+#pragma unroll
+    for (int i = 0; i < Q; i += 4) { a += x[i]; b += x[i + 1]; c += x[i + 2]; d += x[i + 3]; }
+    return (a + b) + (c + d);
+  }
+}
+
 constexpr int kRed = 24;   // doubles per warp in the reduction scratch (>= 4 JT + 1)
 
 // a global buffer of the path: its tensor map (rows as TMA boxes) and the sample's base pointer (generic access)
@@ -104,6 +149,7 @@ struct RowPipe {
   double* orow;    // [4][RP]
   double* xch;     // [2][W][8]
   double* red;     // [W][kRed] partial sums of a pass
+  double* wst;     // this warp's private state rows [JT][Q/2][32] double2 (A q of the iterations in flight)
   uint32_t bar0, phase;
   int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
   LaneOff<Q> lo;
@@ -165,7 +211,8 @@ struct RowPipe {
 // group-uniform sums of one fused pass, index t = iteration within the pass (iterate x_t, step d_t = -q_t)
 template <int JT>
 struct FusedStats {
-  double hinf[JT], h1[JT];   // ||h(x_t)||_inf, ||h(x_t)||_1   (local + mass rows)
+  double hlev[JT];           // ||h(x_t)||_inf against the two thresholds: 0: <= kPolishSkip tol, 1: < tol, 2: >= tol
+  double h1[JT];             // ||h(x_t)||_1   (local + mass rows)
   double wd[JT], dd[JT];     // (x_t - u_hat)^T d_t ,  ||d_t||^2
   double f0;                 // 1/2 ||x_0 - u_hat||^2
   bool bad[JT];              // something non-finite in iteration t
@@ -195,8 +242,12 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   const int cellL = swz_idx((first + nx - 1) % nx), cellR = swz_idx((first + Q) % nx);
   const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
 
-  double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
-  double hinf[T], h1[T], wd[T], dd[T];     // per-lane partial sums (thread 0 of the group also takes the mass rows)
+  double phi[T][Q];                        // Phi(x_t[k-1]) of iteration t, own cells
+  double cc[kCcSmem ? 1 : T][Q];           // (A_{k-1} q_{k-1}) of iteration t: registers, or pp.wst (shared memory)
+  double h1[T], wd[T], dd[T];              // per-lane partial sums (thread 0 of the group also takes the mass rows)
+  bool ge_tol[T], gt_skip[T];              // some |h| >= tol / > kPolishSkip tol seen (all ||h||_inf is needed for)
+  double ms[T];                            // per-lane sum of the iterate's cells (mass rows)
+  const double tol = P.tol, skip = kPolishSkip * P.tol;
   double f2 = 0.0;
   {
     double u0r[Q];
@@ -207,9 +258,14 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         phi[t][c] = u0r[c];   // level 0: h_0 = x[0] - u0
-        cc[t][c] = 0.0;
+        if (!kCcSmem) cc[t][c] = 0.0;
       }
-      hinf[t] = 0.0; h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0;
+      if (kCcSmem) {
+#pragma unroll
+        for (int c = 0; c < Q; ++c) cc[0][c] = 0.0;
+        st_priv<Q>(pp.wst, t, lane, cc[0]);
+      }
+      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false; ms[t] = 0.0;
     }
   }
   const int npro = nst < nt ? nst : nt;
@@ -233,20 +289,22 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
 #pragma unroll
     for (int t = 0; t < T; ++t) {
       double q[Q], uhr[Q];
-      double msum = 0.0;
+      const double msum = tree_sum<Q>(v);
       load_cells<Q>(ruh, pp.lo, uhr);   // 128-bit conflict-free reads; not kept across iterations (registers)
+      const int ti = kCcSmem ? 0 : t;
+      if (kCcSmem) ld_priv<Q>(pp.wst, t, lane, cc[0]);
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         const double h = v[c] - phi[t][c];
-        q[c] = h + cc[t][c];
+        q[c] = h + cc[ti][c];
         const double wv = v[c] - uhr[c];
         const double ah = fabs(h);
-        hinf[t] = fmax(hinf[t], ah);
+        ge_tol[t] |= (ah >= tol);
+        gt_skip[t] |= (ah > skip);
         h1[t] += ah;
         wd[t] = fma(wv, q[c], wd[t]);
         dd[t] = fma(q[c], q[c], dd[t]);
         if (t == 0) f2 = fma(wv, wv, f2);
-        msum += v[c];
       }
       // end values of the next iterate (only the two ends are exchanged; the rest is updated in place below)
       const double vn0 = (t < NU) ? v[0] - q[0] : v[0], vnE = (t < NU) ? v[Q - 1] - q[Q - 1] : v[Q - 1];
@@ -267,13 +325,14 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
           for (int i = 0; i < W; ++i) mtot += xs[i * 8 + 4];
         }
         par ^= 1;
+        if (has_mass && w == 0 && lane == 0) {
+          const double hm = fabs(fma(P.dx, mtot, -M0));
+          ge_tol[t] |= (hm >= tol);
+          gt_skip[t] |= (hm > skip);
+          h1[t] += hm;
+        }
       } else {
-        if (has_mass) mtot = warp_sum(msum);
-      }
-      if (has_mass && w == 0 && lane == 0) {
-        const double hm = fabs(fma(P.dx, mtot, -M0));
-        hinf[t] = fmax(hinf[t], hm);
-        h1[t] += hm;
+        ms[t] = msum;   // reduced after the iterations of this level, all T butterflies interleaved
       }
       // state for the next level (needs the old v and q with neighbours), then the update in place
       double um = vL, ql = qL;
@@ -283,13 +342,32 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         const double qr = (c < Q - 1) ? q[c + 1] : qR;
         const double vc = v[c], qc = q[c];
         phi[t][c] = fma(a0, vc, (up + um) * fma(-qs, up - um, e));
-        cc[t][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
+        cc[ti][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
         um = vc; ql = qc;
         if (t < NU) v[c] = vc - qc;
         else if (EMIT) q[c] = qc - (vc - uhr[c]);   // y
       }
+      if (kCcSmem) st_priv<Q>(pp.wst, t, lane, cc[0]);
       if (t < NU) { vL = vnL; vR = vnR; }
       else store_cells<Q>(so_y, pp.lo, q);
+    }
+    if constexpr (W == 1) {
+      if (has_mass) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+          for (int t = 0; t < T; ++t) ms[t] += __shfl_xor_sync(SNAP_FULL, ms[t], o);
+        }
+        if (lane == 0) {
+#pragma unroll
+          for (int t = 0; t < T; ++t) {
+            const double hm = fabs(fma(P.dx, ms[t], -M0));
+            ge_tol[t] |= (hm >= tol);
+            gt_skip[t] |= (hm > skip);
+            h1[t] += hm;
+          }
+        }
+      }
     }
     if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
     pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
@@ -302,7 +380,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   double part[4 * T + 1];
 #pragma unroll
   for (int t = 0; t < T; ++t) {
-    part[4 * t + 0] = warp_max(hinf[t]);
+    part[4 * t + 0] = __any_sync(SNAP_FULL, ge_tol[t]) ? 2.0 : (__any_sync(SNAP_FULL, gt_skip[t]) ? 1.0 : 0.0);
     part[4 * t + 1] = warp_sum(h1[t]);
     part[4 * t + 2] = warp_sum(wd[t]);
     part[4 * t + 3] = warp_sum(dd[t]);
@@ -331,7 +409,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   for (int t = 0; t < T; ++t) {
     const double a = part[4 * t + 0], b = part[4 * t + 1];
     const double c1 = -part[4 * t + 2], c2 = part[4 * t + 3];
-    S.hinf[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
+    S.hlev[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
     // fmax drops NaN, the sums do not: a non-finite residual or direction shows up in h1 / dd
     S.bad[t] = !(finite_d(a) && finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(part[4 * T]));
   }
@@ -512,7 +590,8 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;
   pp.xch = pp.orow + (size_t)4 * G::RP;
   pp.red = pp.xch + G::XCH;
-  pp.bar0 = smem_u32(pp.red + W * kRed);
+  pp.wst = pp.red + W * kRed + (size_t)w * (JT * Q * 32);
+  pp.bar0 = smem_u32(pp.red + W * kRed + (size_t)W * (JT * Q * 32));
   pp.phase = 0;
   pp.nst = A.nst; pp.lane = lane; pp.w = w; pp.bar_id = 1 + slot;
   pp.first = (w * 32 + lane) * Q;
@@ -623,9 +702,9 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     double f_t = S.f0;
     for (int t = 0; t < T; ++t) {
       if (!conv) {
-        if (S.hinf[t] < P.tol) {
+        if (S.hlev[t] < 2.0) {              // ||h(x_t)||_inf < tol
           conv = true;
-          polish_left = (S.hinf[t] > kPolishSkip * P.tol) ? P.polish : 0;
+          polish_left = (S.hlev[t] > 0.0) ? P.polish : 0;   // polish unless already <= kPolishSkip tol
         } else if (steps >= P.max_iter) {
           status = SNAP_ST_MAXITER;
           conv = true;

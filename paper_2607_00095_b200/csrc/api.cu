@@ -73,9 +73,7 @@ bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
 bool plan_fused(const snap_problem* p, int batch, Plan1d& pl) {
   const int nx = p->dp.nx;
   int W, Q, JT, maxt;
-  static const int variant = [] { const char* e = getenv("SNAP_FUSED_VARIANT"); return e ? atoi(e) : 0; }();
-  if (!fused_variant(nx, variant, W, Q, JT, maxt)) return false;
-  pl.variant = variant;
+  if (!fused_variant(nx, W, Q, JT, maxt)) return false;
   pl.wps = W;
   pl.q = Q; pl.full = true; pl.tma = true;
   pl.rp = fused_row_pitch(nx);
@@ -87,7 +85,7 @@ bool plan_fused(const snap_problem* p, int batch, Plan1d& pl) {
   const size_t limit = (size_t)p->max_smem_optin;
   for (;; --spc) {
     for (int nst = 4; nst >= 2; --nst) {
-      const size_t sb = align_up(((size_t)(2 * nst + 4) * pl.rp + 2 * W * 8 + W * 24 + (size_t)JT * nx + nst) * 8, 1024);
+      const size_t sb = align_up(((size_t)(2 * nst + 4) * pl.rp + 2 * W * 8 + W * 24 + nst) * 8, 1024);
       if (sb * spc + 1024 <= limit) {
         pl.wpc = spc; pl.nst = nst; pl.warp_bytes = (int)sb; pl.smem = sb * spc + 1024;
         pl.grid = (batch + spc - 1) / spc;

@@ -85,36 +85,6 @@ __device__ __forceinline__ void store_cells(double* row, const LaneOff<Q>& lo, c
 __device__ __forceinline__ double shfl_prev(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 31) & 31); }
 __device__ __forceinline__ double shfl_next(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 1) & 31); }
 
-#ifndef SNAP_CC_SMEM
-#define SNAP_CC_SMEM 0
-#endif
-constexpr bool kCcSmem = SNAP_CC_SMEM != 0;   // keep (A_{k-1} q_{k-1}) of every iteration in shared memory, not registers
-
-// per-lane private vectors of Q doubles in shared memory, slot-major so that a warp's 128-bit accesses are conflict free
-template <int Q>
-__device__ __forceinline__ void ld_priv(const double* base, int slot, int lane, double (&x)[Q]) {
-  if constexpr (Q == 1) {
-    x[0] = base[slot * 32 + lane];
-  } else {
-#pragma unroll
-    for (int c = 0; c < Q / 2; ++c) {
-      const double2 t = reinterpret_cast<const double2*>(base)[(slot * (Q / 2) + c) * 32 + lane];
-      x[2 * c] = t.x;
-      x[2 * c + 1] = t.y;
-    }
-  }
-}
-template <int Q>
-__device__ __forceinline__ void st_priv(double* base, int slot, int lane, const double (&x)[Q]) {
-  if constexpr (Q == 1) {
-    base[slot * 32 + lane] = x[0];
-  } else {
-#pragma unroll
-    for (int c = 0; c < Q / 2; ++c)
-      reinterpret_cast<double2*>(base)[(slot * (Q / 2) + c) * 32 + lane] = make_double2(x[2 * c], x[2 * c + 1]);
-  }
-}
-
 // balanced sum of a lane's Q values (dependency depth log2 Q instead of Q)
 template <int Q>
 __device__ __forceinline__ double tree_sum(const double (&x)[Q]) {
@@ -149,7 +119,6 @@ struct RowPipe {
   double* orow;    // [4][RP]
   double* xch;     // [2][W][8]
   double* red;     // [W][kRed] partial sums of a pass
-  double* wst;     // this warp's private state rows [JT][Q/2][32] double2 (A q of the iterations in flight)
   uint32_t bar0, phase;
   int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
   LaneOff<Q> lo;
@@ -242,8 +211,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   const int cellL = swz_idx((first + nx - 1) % nx), cellR = swz_idx((first + Q) % nx);
   const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
 
-  double phi[T][Q];                        // Phi(x_t[k-1]) of iteration t, own cells
-  double cc[kCcSmem ? 1 : T][Q];           // (A_{k-1} q_{k-1}) of iteration t: registers, or pp.wst (shared memory)
+  double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
   double h1[T], wd[T], dd[T];              // per-lane partial sums (thread 0 of the group also takes the mass rows)
   bool ge_tol[T], gt_skip[T];              // some |h| >= tol / > kPolishSkip tol seen (all ||h||_inf is needed for)
   double ms[T];                            // per-lane sum of the iterate's cells (mass rows)
@@ -258,12 +226,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         phi[t][c] = u0r[c];   // level 0: h_0 = x[0] - u0
-        if (!kCcSmem) cc[t][c] = 0.0;
-      }
-      if (kCcSmem) {
-#pragma unroll
-        for (int c = 0; c < Q; ++c) cc[0][c] = 0.0;
-        st_priv<Q>(pp.wst, t, lane, cc[0]);
+        cc[t][c] = 0.0;
       }
       h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false; ms[t] = 0.0;
     }
@@ -291,12 +254,10 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
       double q[Q], uhr[Q];
       const double msum = tree_sum<Q>(v);
       load_cells<Q>(ruh, pp.lo, uhr);   // 128-bit conflict-free reads; not kept across iterations (registers)
-      const int ti = kCcSmem ? 0 : t;
-      if (kCcSmem) ld_priv<Q>(pp.wst, t, lane, cc[0]);
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         const double h = v[c] - phi[t][c];
-        q[c] = h + cc[ti][c];
+        q[c] = h + cc[t][c];
         const double wv = v[c] - uhr[c];
         const double ah = fabs(h);
         ge_tol[t] |= (ah >= tol);
@@ -342,12 +303,11 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         const double qr = (c < Q - 1) ? q[c + 1] : qR;
         const double vc = v[c], qc = q[c];
         phi[t][c] = fma(a0, vc, (up + um) * fma(-qs, up - um, e));
-        cc[ti][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
+        cc[t][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
         um = vc; ql = qc;
         if (t < NU) v[c] = vc - qc;
         else if (EMIT) q[c] = qc - (vc - uhr[c]);   // y
       }
-      if (kCcSmem) st_priv<Q>(pp.wst, t, lane, cc[0]);
       if (t < NU) { vL = vnL; vR = vnR; }
       else store_cells<Q>(so_y, pp.lo, q);
     }
@@ -590,8 +550,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;
   pp.xch = pp.orow + (size_t)4 * G::RP;
   pp.red = pp.xch + G::XCH;
-  pp.wst = pp.red + W * kRed + (size_t)w * (JT * Q * 32);
-  pp.bar0 = smem_u32(pp.red + W * kRed + (size_t)W * (JT * Q * 32));
+  pp.bar0 = smem_u32(pp.red + W * kRed);
   pp.phase = 0;
   pp.nst = A.nst; pp.lane = lane; pp.w = w; pp.bar_id = 1 + slot;
   pp.first = (w * 32 + lane) * Q;

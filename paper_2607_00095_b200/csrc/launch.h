@@ -32,7 +32,6 @@ struct Proj1dArgs {
 struct Plan1d {
   int q, wpc, nst, rp, warp_bytes, grid;
   int wps;       // fused path: warps per sample
-  int variant;   // fused path: tuning variant of the nx = 256 instantiation (0 = default)
   bool full;  // nx == 32 q: no bounds checks in the sweeps
   bool tma;   // every row start is 16-byte aligned: bulk (TMA) copies; otherwise plain loads/stores
   size_t smem;
@@ -47,7 +46,7 @@ int launch_project1d_fisher(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t 
 int launch_project1d_burgers_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
 int fused_row_pitch(int nx);   // padded shared-memory row pitch in doubles
 // (warps per sample, cells per lane, iterations per pass, max threads per CTA) of the instantiation for nx
-bool fused_variant(int nx, int variant, int& W, int& Q, int& JT, int& maxt);
+bool fused_variant(int nx, int& W, int& Q, int& JT, int& maxt);
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, cudaStream_t st);
 

@@ -348,8 +348,8 @@ def run_gpu(args):
                    "alg_bytes_per_projection": sum(alg_bytes_call) / (run.B * run.calls)},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_note": traffic_note,
-                     "kernel": {5: "project1d_fused_kernel<1,8,3,256>", 2: "project1d_fused_kernel<1,4,4,256>",
-                                3: "project1d_kernel<2,4,0,1> (Fisher, classic sweeps)", 4: "project2d_kernel",
+                     "kernel": {5: "project1d_fused_kernel<1,1,8,3,256>", 2: "project1d_fused_kernel<1,1,4,4,256>",
+                                3: "project1d_fused_kernel<2,1,4,3,256> (Fisher)", 4: "project2d_kernel",
                                 1: "heat_project_kernel"}[cfg],
                      "peak_source": peak_src, "alg_bytes_per_launch_mean": alg_total / (args.steps * run.calls),
                      "launch_ms_mean": 1e3 * kern_s / (args.steps * run.calls),

@@ -88,7 +88,7 @@ typedef struct {
   int pcg_max;        /* 2D: PCG iteration cap per solve                    (default 200)                     */
   int precond;        /* 2D: 0 none, 1 time-line, 2 time-line x ADI, 3 time-line x exact level solve (default 2) */
   int lambda_mode;    /* 0 = minimum-norm multiplier, 1 = basic (redundant multipliers = 0)    */
-  int gn_fuse;        /* Burgers kinds with nx in {32,64,128,256,512}: Gauss-Newton iterations carried by one
+  int gn_fuse;        /* Burgers kinds (nx in {32,...,512}) and Fisher (nx in {32,...,256}): Gauss-Newton iterations carried by one
                          forward pass over the levels.  0 = as many as the kernel holds in
                          registers (default), k >= 1 = at most k, -1 = classic path (one forward and one
                          backward sweep per iteration).  Other kinds / sizes always take the classic path.   */

@@ -73,7 +73,8 @@ bool plan_1d(const snap_problem* p, int batch, Plan1d& pl) {
 bool plan_fused(const snap_problem* p, int batch, Plan1d& pl) {
   const int nx = p->dp.nx;
   int W, Q, JT, maxt;
-  if (!fused_variant(nx, W, Q, JT, maxt)) return false;
+  const bool fisher = p->dp.kind == SNAP_FISHER1D_IE;
+  if (!(fisher ? fused_variant_fisher(nx, W, Q, JT, maxt) : fused_variant(nx, W, Q, JT, maxt))) return false;
   pl.wps = W;
   pl.q = Q; pl.full = true; pl.tma = true;
   pl.rp = fused_row_pitch(nx);
@@ -277,7 +278,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   // bulk (TMA) copies need every row start 16-byte aligned
   const bool bulk_ok = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
                        aligned16(lambda) && aligned16(a.bufA);
-  if (d.kind != SNAP_FISHER1D_IE && p->params.gn_fuse >= 0 && bulk_ok) {
+  if (p->params.gn_fuse >= 0 && bulk_ok) {
     Plan1d pf;
     if (plan_fused(p, batch, pf)) {
       const int box = d.nx / 16 / pf.wps;
@@ -290,7 +291,8 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
       if (ok) {
         a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
         p->launches++;
-        return launch_project1d_burgers_fused(a, pf, st);
+        return d.kind == SNAP_FISHER1D_IE ? launch_project1d_fisher_fused(a, pf, st)
+                                          : launch_project1d_burgers_fused(a, pf, st);
       }
     }
   }

@@ -26,6 +26,7 @@
 #include "device_utils.cuh"
 #include "launch.h"
 #include "snap_internal.h"
+#include "tridiag.cuh"
 
 namespace snap {
 
@@ -376,21 +377,175 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
 }
 
-// runtime (J, T) -> static instantiation
-template <int W, int Q, int JT>
+// ------------------------------------------------------------------------------------------------
+// Fisher-KPP (kind 2, W = 1): the same fused pass with the implicit level operator,
+//     q_0 = h_0 ,   T_k q_k = h_k + q_{k-1} ,   T_k = I - dt D Lap_h - dt rho diag(1 - 2 x[k])   (symmetric tridiagonal),
+//     h_k = x[k] - x[k-1] - dt (D Lap_h x[k] + rho x[k] (1 - x[k]))   with ghost-cell Neumann ends (R10).
+// State per iteration in flight: q_{k-1} and x_t[k-1] of the own cells.  The tridiagonal solve is the warp-level
+// partition + cyclic-reduction solver of tridiag.cuh; the level matrix depends on the current level only.
+// ------------------------------------------------------------------------------------------------
+template <int Q, int JT, int NU, bool EMIT>
+__device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x0, const Buf uh,
+                                         const double* __restrict__ u0, const Buf xout, const Buf yout,
+                                         FusedStats<JT>& S) {
+  constexpr int T = NU + (EMIT ? 1 : 0);
+  static_assert(T >= 1 && T <= JT, "iterations per pass");
+  RowPipe<1, Q> pp = pp_ref;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
+  const double fa = P.fi_a, fr = P.fi_dtrho;
+  const bool same = (x0.p == uh.p);
+  const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
+  const double tol = P.tol, skip = kPolishSkip * P.tol;
+
+  double qo[T][Q], xp[T][Q];   // q_{k-1} and x_t[k-1] of iteration t, own cells
+  double h1[T], wd[T], dd[T];
+  bool ge_tol[T], gt_skip[T];
+  double f2 = 0.0;
+  double u0r[Q];
+#pragma unroll
+  for (int c = 0; c < Q; ++c) u0r[c] = u0[first + c];
+#pragma unroll
+  for (int t = 0; t < T; ++t) {
+#pragma unroll
+    for (int c = 0; c < Q; ++c) { qo[t][c] = 0.0; xp[t][c] = 0.0; }
+    h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false;
+  }
+  const int npro = nst < nt ? nst : nt;
+  for (int k = 0; k < npro; ++k) pp.issue(k, k, x0.tm, tm_uh);
+
+  int s = 0;
+  for (int k = 0; k < nt; ++k) {
+    pp.wait(s);
+    double v[Q];
+    const double* r0 = pp.row(s, 0);
+    const double* ruh = same ? r0 : pp.row(s, 1);
+    load_cells<Q>(r0, pp.lo, v);
+    pp.out_ready();
+    double* so_u = pp.out(k & 1);
+    double* so_y = pp.out(2 + (k & 1));
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      double q[Q], uhr[Q], hv[Q];
+      load_cells<Q>(ruh, pp.lo, uhr);
+      if (k == 0) {
+#pragma unroll
+        for (int c = 0; c < Q; ++c) { hv[c] = v[c] - u0r[c]; q[c] = hv[c]; }
+      } else {
+        double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
+        if (lane == 0) vL = v[0];          // mirrored ghost cells (Neumann)
+        if (lane == 31) vR = v[Q - 1];
+        double a[Q], b[Q], cdiag[Q];
+#pragma unroll
+        for (int c = 0; c < Q; ++c) {
+          const double um = (c > 0) ? v[c - 1] : vL, up = (c < Q - 1) ? v[c + 1] : vR;
+          hv[c] = v[c] - xp[t][c] - fa * ((um - v[c]) + (up - v[c])) - fr * v[c] * (1.0 - v[c]);
+          q[c] = hv[c] + qo[t][c];
+        }
+        fisher_matrix<Q>(P, v, lane, a, b, cdiag);
+        warp_tridiag<Q>(a, b, cdiag, q, lane);
+      }
+#pragma unroll
+      for (int c = 0; c < Q; ++c) {
+        const double wv = v[c] - uhr[c];
+        const double ah = fabs(hv[c]);
+        ge_tol[t] |= (ah >= tol);
+        gt_skip[t] |= (ah > skip);
+        h1[t] += ah;
+        wd[t] = fma(wv, q[c], wd[t]);
+        dd[t] = fma(q[c], q[c], dd[t]);
+        if (t == 0) f2 = fma(wv, wv, f2);
+        qo[t][c] = q[c];
+        xp[t][c] = v[c];
+        if (t < NU) v[c] -= q[c];
+        else if (EMIT) q[c] = q[c] - wv;   // y
+      }
+      if (t >= NU) store_cells<Q>(so_y, pp.lo, q);
+    }
+    if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
+    pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
+    if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
+    if (++s == nst) s = 0;
+  }
+  pp.drain();
+  const double f2s = warp_sum(f2);
+  S.f0 = 0.5 * f2s;
+#pragma unroll
+  for (int t = 0; t < T; ++t) {
+    const double a = __any_sync(SNAP_FULL, ge_tol[t]) ? 2.0 : (__any_sync(SNAP_FULL, gt_skip[t]) ? 1.0 : 0.0);
+    const double b = warp_sum(h1[t]), c1 = -warp_sum(wd[t]), c2 = warp_sum(dd[t]);
+    S.hlev[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
+    S.bad[t] = !(finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(f2s));
+  }
+  pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
+}
+
+// Fisher multiplier solve at the final iterate:  T_k lam_k = y_k + lam_{k+1} (k >= 1) ,  lam_0 = y_0 + lam_1.
+template <int Q>
+__device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x, const Buf lam,
+                                           const CUtensorMap* ucopy) {
+  RowPipe<1, Q> pp = pp_ref;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst;
+  double lo[Q];
+#pragma unroll
+  for (int c = 0; c < Q; ++c) lo[c] = 0.0;
+  double chk = 0.0;
+  const int npro = nst < nt ? nst : nt;
+  for (int t = 0; t < npro; ++t) pp.issue(t, nt - 1 - t, lam.tm, x.tm);
+  int s = 0;
+  for (int t = 0; t < nt; ++t) {
+    const int k = nt - 1 - t;
+    pp.wait(s);
+    double l[Q], v[Q];
+    load_cells<Q>(pp.row(s, 0), pp.lo, l);
+    load_cells<Q>(pp.row(s, 1), pp.lo, v);
+    pp.out_ready();
+#pragma unroll
+    for (int c = 0; c < Q; ++c) l[c] += lo[c];
+    if (k > 0) {
+      double a[Q], b[Q], cdiag[Q];
+      fisher_matrix<Q>(P, v, lane, a, b, cdiag);
+      warp_tridiag<Q>(a, b, cdiag, l, lane);
+    }
+#pragma unroll
+    for (int c = 0; c < Q; ++c) { lo[c] = l[c]; chk += l[c]; }
+    double* so_l = pp.out(t & 1);
+    double* so_u = pp.out(2 + (t & 1));
+    store_cells<Q>(so_l, pp.lo, l);
+    if (ucopy) store_cells<Q>(so_u, pp.lo, v);
+    pp.store_rows(k, lam.tm, so_l, ucopy, so_u);
+    if (t + nst < nt) pp.issue(s, k - nst, lam.tm, x.tm);
+    if (++s == nst) s = 0;
+  }
+  pp.drain();
+  pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
+  return warp_sum(chk);
+}
+
+// runtime (J, T) -> static instantiation; KIND: KB_FUSED (Burgers family) or KF_FUSED (Fisher, W = 1)
+constexpr int KB_FUSED = 1, KF_FUSED = 2;
+
+template <int KIND, int W, int Q, int JT, int NU, bool EMIT>
+__device__ __forceinline__ void fused_fwd_kind(const DevParams& P, RowPipe<W, Q>& pp, const Buf x0, const Buf uh,
+                                               const double* u0, const Buf xout, const Buf yout, double M0,
+                                               FusedStats<JT>& S) {
+  if constexpr (KIND == KF_FUSED) fused_fwd_f<Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, S);
+  else fused_fwd<W, Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, M0, S);
+}
+
+template <int KIND, int W, int Q, int JT>
 __device__ __forceinline__ void fused_fwd_dispatch(const DevParams& P, RowPipe<W, Q>& pp, const Buf x0, const Buf uh,
                                                    const double* u0, const Buf xout, const Buf yout, int J, int T,
                                                    double M0, FusedStats<JT>& S) {
   if (T == J) {   // only the first pass: JT updates, no y
-    fused_fwd<W, Q, JT, JT, false>(P, pp, x0, uh, u0, xout, yout, M0, S);
+    fused_fwd_kind<KIND, W, Q, JT, JT, false>(P, pp, x0, uh, u0, xout, yout, M0, S);
     return;
   }
-  if (J == 0) fused_fwd<W, Q, JT, 0, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
-  else if (J == 1) fused_fwd<W, Q, JT, 1, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+  if (J == 0) fused_fwd_kind<KIND, W, Q, JT, 0, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+  else if (J == 1) fused_fwd_kind<KIND, W, Q, JT, 1, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
   else if (J == 2) {
-    if constexpr (JT >= 3) fused_fwd<W, Q, JT, 2, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+    if constexpr (JT >= 3) fused_fwd_kind<KIND, W, Q, JT, 2, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
   } else if (J == 3) {
-    if constexpr (JT >= 4) fused_fwd<W, Q, JT, 3, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
+    if constexpr (JT >= 4) fused_fwd_kind<KIND, W, Q, JT, 3, true>(P, pp, x0, uh, u0, xout, yout, M0, S);
   }
 }
 
@@ -528,7 +683,7 @@ __device__ __noinline__ void fused_min_norm(const DevParams& P, RowPipe<W, Q>& p
 // ------------------------------------------------------------------------------------------------
 // the persistent Gauss-Newton driver (a8, a9); every warp of a group runs it with identical values
 // ------------------------------------------------------------------------------------------------
-template <int W, int Q, int JT, int MAXT>
+template <int KIND, int W, int Q, int JT, int MAXT>
 __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_constant__ Proj1dArgs A) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   using G = RowGeom<W, Q>;
@@ -625,7 +780,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     if (J > JT - 1 && (sweeps > 0 || conv || jcap < JT)) J = JT - 1;
     if (J < 0) J = 0;
     const int T = (J < JT) ? J + 1 : J;
-    fused_fwd_dispatch<W, Q, JT>(P, pp, mk(x0), mk(uh), u0, mk(xo), mk(lam), J, T, M0, S);
+    fused_fwd_dispatch<KIND, W, Q, JT>(P, pp, mk(x0), mk(uh), u0, mk(xo), mk(lam), J, T, M0, S);
     ++sweeps;
 
     // ---- a pending step is judged by iteration 0 of this pass ---------------------------------------------
@@ -743,13 +898,15 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
   } else {
     if (status == SNAP_ST_LINESEARCH) {   // multiplier at the last accepted iterate (as the oracle returns it)
-      fused_fwd_dispatch<W, Q, JT>(P, pp, mk(cur), mk(uh), u0, Buf{nullptr, nullptr}, mk(lam), 0, 1, M0, S);
+      fused_fwd_dispatch<KIND, W, Q, JT>(P, pp, mk(cur), mk(uh), u0, Buf{nullptr, nullptr}, mk(lam), 0, 1, M0, S);
       ++sweeps;
       xfin = cur;
     }
     const bool want_sig = (P.kind == SNAP_BURGERS1D_LF_MASS) && (P.lambda_mode == 0);
-    const double chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), (xfin != ustar) ? &A.tm[TM_USTAR] : nullptr,
-                                       want_sig ? sig : nullptr);
+    const CUtensorMap* const tm_copy = (xfin != ustar) ? &A.tm[TM_USTAR] : nullptr;
+    double chk;
+    if constexpr (KIND == KF_FUSED) chk = fused_bwd_f<Q>(P, pp, mk(xfin), mk(lam), tm_copy);
+    else chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), tm_copy, want_sig ? sig : nullptr);
     ++sweeps;
     if (!finite_d(chk)) {
       status = SNAP_ST_NONFINITE;
@@ -758,7 +915,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
       for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
     } else if (P.has_mass) {
       if (want_sig) {
-        fused_min_norm<W, Q>(P, pp, mk(lam), sig, tt);
+        if constexpr (KIND == KB_FUSED) fused_min_norm<W, Q>(P, pp, mk(lam), sig, tt);
         ++sweeps;
       } else {
         for (int k = gtid; k < nt; k += GT) lam[n + k] = 0.0;
@@ -771,9 +928,9 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   }
 }
 
-template <int W, int Q, int JT, int MAXT>
+template <int KIND, int W, int Q, int JT, int MAXT>
 inline int launch_fused_variant(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
-  auto kern = project1d_fused_kernel<W, Q, JT, MAXT>;
+  auto kern = project1d_fused_kernel<KIND, W, Q, JT, MAXT>;
   if (pl.wpc * W * 32 > MAXT) return SNAP_EINVAL;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
     return SNAP_ECUDA;
@@ -782,8 +939,8 @@ inline int launch_fused_variant(const Proj1dArgs& a, const Plan1d& pl, cudaStrea
   if (err != cudaSuccess && getenv("SNAP_DEBUG")) {
     cudaFuncAttributes fa;
     cudaFuncGetAttributes(&fa, kern);
-    fprintf(stderr, "snap: fused<%d,%d,%d,%d> launch failed: %s; grid %d block %d smem %zu; regs %d maxThreads %d local %zu\n",
-            W, Q, JT, MAXT, cudaGetErrorString(err), pl.grid, pl.wpc * W * 32, pl.smem, fa.numRegs, fa.maxThreadsPerBlock,
+    fprintf(stderr, "snap: fused<%d,%d,%d,%d,%d> launch failed: %s; grid %d block %d smem %zu; regs %d maxThreads %d local %zu\n",
+            KIND, W, Q, JT, MAXT, cudaGetErrorString(err), pl.grid, pl.wpc * W * 32, pl.smem, fa.numRegs, fa.maxThreadsPerBlock,
             fa.localSizeBytes);
   }
   return err == cudaSuccess ? SNAP_OK : SNAP_ECUDA;

@@ -47,6 +47,9 @@ int launch_project1d_burgers_fused(const Proj1dArgs& a, const Plan1d& pl, cudaSt
 int fused_row_pitch(int nx);   // padded shared-memory row pitch in doubles
 // (warps per sample, cells per lane, iterations per pass, max threads per CTA) of the instantiation for nx
 bool fused_variant(int nx, int& W, int& Q, int& JT, int& maxt);
+// proj1d_fisher_fused.cu: same for kind 2
+int launch_project1d_fisher_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
+bool fused_variant_fisher(int nx, int& W, int& Q, int& JT, int& maxt);
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, cudaStream_t st);
 

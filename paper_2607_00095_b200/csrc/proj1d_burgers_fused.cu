@@ -20,12 +20,12 @@ int fused_row_pitch(int nx) { return nx < 128 ? 128 : nx; }
 
 int launch_project1d_burgers_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
   switch (a.P.nx) {
-    case 32: return launch_fused_variant<1, 1, 4, 256>(a, pl, st);
-    case 64: return launch_fused_variant<1, 2, 4, 256>(a, pl, st);
-    case 128: return launch_fused_variant<1, 4, 4, 256>(a, pl, st);
+    case 32: return launch_fused_variant<KB_FUSED, 1, 1, 4, 256>(a, pl, st);
+    case 64: return launch_fused_variant<KB_FUSED, 1, 2, 4, 256>(a, pl, st);
+    case 128: return launch_fused_variant<KB_FUSED, 1, 4, 4, 256>(a, pl, st);
     case 256:
-      return launch_fused_variant<1, 8, 3, 256>(a, pl, st);
-    case 512: return launch_fused_variant<2, 8, 3, 256>(a, pl, st);
+      return launch_fused_variant<KB_FUSED, 1, 8, 3, 256>(a, pl, st);
+    case 512: return launch_fused_variant<KB_FUSED, 2, 8, 3, 256>(a, pl, st);
   }
   return SNAP_EINVAL;
 }

@@ -306,9 +306,9 @@ def test_host_buffer_entry_point(S):
 
 
 # ------------------------------------------------------------------------------------------------
-# fused Gauss-Newton passes (Burgers kinds, nx = 32 * 2^j): every mode must reach the oracle's point
+# fused Gauss-Newton passes (Burgers and Fisher kinds, nx = 32 * 2^j): every mode must reach the oracle's point
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg", [2, 5])
+@pytest.mark.parametrize("cfg", [2, 3, 5])
 @pytest.mark.parametrize("gn_fuse", [-1, 1, 2, 0])
 def test_fused_pass_modes_agree_with_oracle(S, cfg, gn_fuse):
     """gn_fuse = -1 classic sweeps, 1 / 2 / 0 (= max) iterations per forward pass: same limit point."""

@@ -20,7 +20,10 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 bool is_1d(int kind) { return kind != SNAP_ALLENCAHN2D_IE; }
 
 // Green's function of the cyclic tridiagonal (-a, 1+2a, -a) of size N, truncated where it drops below
-// 1e-17 of its peak (exact to fp64 rounding); g[t], t = 0..K, applied symmetrically (t = -K..K).
+// kGreenTol of its peak; g[t], t = 0..K, applied symmetrically (t = -K..K).
+// taps of the ADI line solve below this fraction of the peak are dropped: the operator only preconditions,
+// and M^{-1} = Jt^{-T} Jt^{-1} stays symmetric positive definite because both sweeps use the same taps
+constexpr double kGreenTol = 1e-8;
 void circulant_green(double a, int N, std::vector<double>& g) {
   g.clear();
   if (a <= 0.0) { g.push_back(1.0); return; }
@@ -32,7 +35,7 @@ void circulant_green(double a, int N, std::vector<double>& g) {
   for (int t = 0; t <= Kmax; ++t) {
     const double v = (pow(rho, (double)t) + pow(rho, (double)(N - t))) / ((1.0 - rhoN) * disc);
     g.push_back(v);
-    if (t > 0 && v < 1e-17 * g[0]) break;
+    if (t > 0 && v < kGreenTol * g[0]) break;
   }
   const int K = (int)g.size() - 1;
   if (2 * K == N) g[K] *= 0.5;  // offset +K and -K are the same point on an even ring

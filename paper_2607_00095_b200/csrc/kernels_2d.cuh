@@ -61,6 +61,22 @@ __device__ __forceinline__ double blk_max(const Ctx2d& c, double v) {
   if ((c).active)                  \
     for (int j = (c).jr, cell = (c).jr * (c).nx + (c).i; j < (c).ny; j += (c).rpp, cell += (c).rpp * (c).nx)
 
+// A thread owns at most kCpt cells of a level (column i, rows jr, jr + rpp, ...).  The level passes first
+// gather all of a thread's global values into registers (independent loads in flight together) and only then
+// touch shared memory: a load-store-load chain per cell would expose the full memory latency kCpt times.
+constexpr int kCpt = 8;   // nx * ny <= 4096 cells over 512 threads
+__device__ __forceinline__ void gather(const Ctx2d& c, const double* __restrict__ src, double (&t)[kCpt]) {
+#pragma unroll
+  for (int u = 0; u < kCpt; ++u) {
+    const int j = c.jr + u * c.rpp;
+    t[u] = (c.active && j < c.ny) ? src[j * c.nx + c.i] : 0.0;
+  }
+}
+#define SNAP_FOR_OWN(c, u, cell, j)                                               \
+  _Pragma("unroll") for (int u = 0; u < kCpt; ++u)                                \
+    for (int j = (c).jr + u * (c).rpp, cell = j * (c).nx + (c).i, once_ = 1;      \
+         once_ && (c).active && j < (c).ny; once_ = 0)
+
 // T x at one cell, x in shared memory:  x - ax lap_x x - ay lap_y x + dt (3 w^2 - 1) x
 __device__ __forceinline__ double T_apply(const DevParams& P, const Ctx2d& c, const double* x, int j, int cell,
                                           double w) {
@@ -122,24 +138,30 @@ __device__ double schur_apply(const DevParams& P, const Ctx2d& c, const double* 
   double dot = 0.0;
   double* gcur = c.s1;
   double* gprev = c.s2;
+  double xn[kCpt], un[kCpt] = {}, xc[kCpt], uc[kCpt];
+  gather(c, x, xn);            // level 0 of x; u is not needed at level 0
   for (int k = 0; k < c.nt; ++k) {
-    const double* uk = u + (size_t)k * c.L;
-    const double* xk = x + (size_t)k * c.L;
+#pragma unroll
+    for (int t = 0; t < kCpt; ++t) { xc[t] = xn[t]; uc[t] = un[t]; }
+    if (k + 1 < c.nt) {        // next level's values travel while this level is computed
+      gather(c, x + (size_t)(k + 1) * c.L, xn);
+      gather(c, u + (size_t)(k + 1) * c.L, un);
+    }
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) c.s0[cell] = xk[cell];
+    SNAP_FOR_OWN(c, t, cell, j) c.s0[cell] = xc[t];
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      double g = (k == 0) ? c.s0[cell] : T_apply(P, c, c.s0, j, cell, uk[cell]);
-      if (k + 1 < c.nt) g -= xk[cell + c.L];
+    SNAP_FOR_OWN(c, t, cell, j) {
+      double g = (k == 0) ? xc[t] : T_apply(P, c, c.s0, j, cell, uc[t]);
+      if (k + 1 < c.nt) g -= xn[t];
       gcur[cell] = g;
     }
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      const double qq = (k == 0) ? gcur[cell] : T_apply(P, c, gcur, j, cell, uk[cell]) - gprev[cell];
+    SNAP_FOR_OWN(c, t, cell, j) {
+      const double qq = (k == 0) ? gcur[cell] : T_apply(P, c, gcur, j, cell, uc[t]) - gprev[cell];
       q[(size_t)k * c.L + cell] = qq;
-      dot = fma(c.s0[cell], qq, dot);
+      dot = fma(xc[t], qq, dot);
     }
-    double* t = gcur; gcur = gprev; gprev = t;
+    double* tp = gcur; gcur = gprev; gprev = tp;
   }
   return blk_sum(c, dot);
 }
@@ -182,28 +204,36 @@ __device__ double precond_apply(const DevParams& P, const Ctx2d& c, const double
     }
     return blk_sum(c, dot);
   }
-  // forward: y_0 = r_0 ; y_k = Tt^{-1} (r_k + y_{k-1})      (level kept in s0)
+  // forward: y_0 = r_0 ; y_k = Tt^{-1} (r_k + y_{k-1})      (level kept in s0; next level's r prefetched)
+  double vn[kCpt], vc[kCpt], rn[kCpt], rc[kCpt];
+  gather(c, r, vn);
   for (int k = 0; k < c.nt; ++k) {
+#pragma unroll
+    for (int t = 0; t < kCpt; ++t) vc[t] = vn[t];
+    if (k + 1 < c.nt) gather(c, r + (size_t)(k + 1) * c.L, vn);
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      const double v = r[(size_t)k * c.L + cell];
-      c.s0[cell] = (k == 0) ? v : v + c.s0[cell];
-    }
+    SNAP_FOR_OWN(c, t, cell, j) c.s0[cell] = (k == 0) ? vc[t] : vc[t] + c.s0[cell];
     if (k > 0 && P.precond == 2) adi_inverse(P, c, c.s0, c.s1);
-    SNAP_FOR_CELLS(c, cell, j) y[(size_t)k * c.L + cell] = c.s0[cell];
+    SNAP_FOR_OWN(c, t, cell, j) y[(size_t)k * c.L + cell] = c.s0[cell];
   }
   // backward: z_k = Tt^{-1} (y_k + z_{k+1}) ; z_0 = y_0 + z_1
+  __syncthreads();   // this thread's y values were written by itself: visible; the barrier orders shared memory
+  gather(c, y + (size_t)(c.nt - 1) * c.L, vn);
+  gather(c, r + (size_t)(c.nt - 1) * c.L, rn);
   for (int k = c.nt - 1; k >= 0; --k) {
-    __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      const double v = y[(size_t)k * c.L + cell];
-      c.s0[cell] = (k == c.nt - 1) ? v : v + c.s0[cell];
+#pragma unroll
+    for (int t = 0; t < kCpt; ++t) { vc[t] = vn[t]; rc[t] = rn[t]; }
+    if (k > 0) {
+      gather(c, y + (size_t)(k - 1) * c.L, vn);
+      gather(c, r + (size_t)(k - 1) * c.L, rn);
     }
+    __syncthreads();
+    SNAP_FOR_OWN(c, t, cell, j) c.s0[cell] = (k == c.nt - 1) ? vc[t] : vc[t] + c.s0[cell];
     if (k > 0 && P.precond == 2) adi_inverse(P, c, c.s0, c.s1);
-    SNAP_FOR_CELLS(c, cell, j) {
+    SNAP_FOR_OWN(c, t, cell, j) {
       const double zz = c.s0[cell];
       z[(size_t)k * c.L + cell] = zz;
-      dot = fma(r[(size_t)k * c.L + cell], zz, dot);
+      dot = fma(rc[t], zz, dot);
     }
   }
   return blk_sum(c, dot);
@@ -240,10 +270,11 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
 
 // ---- a6: PCG on S lam = b.  Returns 0 on success, 1 if pcg_max was hit ----------------------------------
 __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __restrict__ u, const double* __restrict__ b,
-                         double* __restrict__ x, double* r, double* z, double* p, double* q, double* y, bool warm,
-                         size_t n) {
+                         double* __restrict__ x, double* __restrict__ r, double* __restrict__ z, double* __restrict__ p,
+                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n) {
   const int tid = threadIdx.x;
   double bb = 0.0;
+#pragma unroll 8
   for (size_t i = tid; i < n; i += kT2) bb = fma(b[i], b[i], bb);
   bb = blk_sum(c, bb);
   const double bnorm = sqrt(bb);
@@ -268,6 +299,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
     const double alpha = rz / pq;
     __syncthreads();
     double rr = 0.0;
+#pragma unroll 8
     for (size_t i = tid; i < n; i += kT2) {
       x[i] = fma(alpha, p[i], x[i]);
       const double rn = fma(-alpha, q[i], r[i]);
@@ -295,6 +327,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
     const double beta = rz_new / rz;
     rz = rz_new;
     __syncthreads();
+#pragma unroll 8
     for (size_t i = tid; i < n; i += kT2) p[i] = fma(beta, p[i], z[i]);
   }
   return 1;

@@ -256,8 +256,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const DevParams& d = p->dp;
   if (d.kind == SNAP_HEAT1D_IC_MASS) {
-    const int wpc = 4;
-    heat_project_kernel<<<(batch + wpc - 1) / wpc, wpc * 32, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters);
+    heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters);
     return check_launch(p);
   }
   if (!workspace) return SNAP_EINVAL;

@@ -213,15 +213,19 @@ __global__ void __launch_bounds__(kMiscThreads) j_apply_kernel(const __grid_cons
 //   minimum norm   : lam -= N^T (N lam) / (N N^T),  N = (dx 1 on IC rows, -1 on mass row 0),  N N^T = 1 + nx dx^2
 // r = h - J (u - u_hat) = J u_hat - b does not depend on u, so one Gauss-Newton step is exact;
 // the full step satisfies the Armijo condition identically (1/2 |d|^2 = 1/2 lam^T h <= mu |h|_1 / 2.2).
-// One warp per sample; iters = 2 (step + the solve at the projected point) or 1 if u_hat is already feasible.
+// One CTA per sample; iters = 2 (step + the solve at the projected point) or 1 if u_hat is already feasible.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid_constant__ DevParams P, int batch,
                                                                     const double* __restrict__ u_hat,
                                                                     const double* __restrict__ cdata,
                                                                     double* __restrict__ u_star,
                                                                     double* __restrict__ lam, int* __restrict__ iters) {
-  const int lane = threadIdx.x & 31;
-  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  // One CTA per sample: the levels are independent (every non-redundant mass row has its own multiplier), so the
+  // warps of the CTA take the levels round-robin; only ||h||_inf and the non-finite flag are reduced over the CTA.
+  __shared__ double s_max[kMiscThreads / 32];
+  __shared__ int s_bad[kMiscThreads / 32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+  const int b = blockIdx.x;
   if (b >= batch) return;
   const int nx = P.nx, nt = P.nt;
   const double* uh = u_hat + (size_t)b * P.n;
@@ -231,12 +235,23 @@ __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid
   const double c = (double)nx * P.dx * P.dx;
   double s0 = 0.0;
   for (int i = lane; i < nx; i += 32) s0 += u0[i];
-  const double M0 = P.dx * warp_sum(s0);
+  const double M0 = P.dx * warp_sum(s0);   // same order in every warp: identical value
 
-  // solve 1 at u = u_hat: residual norms and the multipliers
+  auto block_max = [&](double v, int flag, int& flag_out) {
+    __syncthreads();
+    if (lane == 0) { s_max[warp] = v; s_bad[warp] = flag; }
+    __syncthreads();
+    double m = 0.0;
+    int f = 0;
+    for (int w2 = 0; w2 < nwarp; ++w2) { m = fmax(m, s_max[w2]); f |= s_bad[w2]; }
+    flag_out = f;
+    return m;
+  };
+
+  // solve 1 at u = u_hat: residual norms and the mass multipliers
   double hinf = 0.0;
   int bad = 0;
-  for (int k = 0; k < nt; ++k) {
+  for (int k = warp; k < nt; k += nwarp) {
     double sk = 0.0, dmax = 0.0;
     for (int i = lane; i < nx; i += 32) {
       const double v = uh[(size_t)k * nx + i];
@@ -253,48 +268,51 @@ __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid
     if (lane == 0) lb[nx + k] = (k == 0) ? 0.0 : rm / c;
   }
   bad = warp_or(bad);
+  hinf = block_max(hinf, bad, bad);
   if (bad) {  // R16
     if (us != uh)
-      for (size_t i = lane; i < (size_t)P.n; i += 32) us[i] = uh[i];
-    for (int i = lane; i < P.m; i += 32) lb[i] = 0.0;
-    if (lane == 0) iters[b] = SNAP_ST_NONFINITE;
+      for (size_t i = threadIdx.x; i < (size_t)P.n; i += blockDim.x) us[i] = uh[i];
+    __syncthreads();
+    for (int i = threadIdx.x; i < P.m; i += blockDim.x) lb[i] = 0.0;
+    if (threadIdx.x == 0) iters[b] = SNAP_ST_NONFINITE;
     return;
   }
   double dsum = 0.0;
   for (int i = lane; i < nx; i += 32) dsum += uh[i] - u0[i];
   dsum = warp_sum(dsum);
   const double lm0 = (P.lambda_mode == 0) ? P.dx * dsum / (1.0 + c) : 0.0;  // minimum-norm correction
-  __syncwarp();
   const bool feasible = hinf <= kPolishSkip * P.tol;
   int solves = 1;
-  for (int i = lane; i < nx; i += 32) lb[i] = (uh[i] - u0[i]) - P.dx * lm0;
-  if (lane == 0) lb[nx] = lm0;
+  // IC multipliers need u_hat[0]: computed before level 0 of u_star (which may alias u_hat) is overwritten
+  if (warp == 0) {
+    for (int i = lane; i < nx; i += 32) lb[i] = (uh[i] - u0[i]) - P.dx * lm0;
+    if (lane == 0) lb[nx] = lm0;
+  }
+  __syncthreads();
   if (feasible) {
     if (us != uh)
-      for (size_t i = lane; i < (size_t)P.n; i += 32) us[i] = uh[i];
+      for (size_t i = threadIdx.x; i < (size_t)P.n; i += blockDim.x) us[i] = uh[i];
   } else {
-    // full step u = u_hat - J^T lam:  level 0 -> u0 ; level k -> u_hat[k] - dx lam_mass,k
-    for (int k = 0; k < nt; ++k) {
-      const double sh = (k == 0) ? 0.0 : P.dx * lb[nx + k];
-      for (int i = lane; i < nx; i += 32)
-        us[(size_t)k * nx + i] = (k == 0) ? u0[i] : uh[(size_t)k * nx + i] - sh;
-    }
-    __syncwarp();
-    // solve 2 at the projected point: the residual there decides convergence; r (hence lam) is unchanged
+    // full step u = u_hat - J^T lam:  level 0 -> u0 ; level k -> u_hat[k] - dx lam_mass,k ; then solve 2 at the
+    // projected point: the residual there decides convergence; r (hence lam) is unchanged
     double h2 = 0.0;
-    for (int k = 0; k < nt; ++k) {
+    for (int k = warp; k < nt; k += nwarp) {
+      const double sh = (k == 0) ? 0.0 : P.dx * lb[nx + k];
       double sk = 0.0, dmax = 0.0;
       for (int i = lane; i < nx; i += 32) {
-        const double v = us[(size_t)k * nx + i];
+        const double v = (k == 0) ? u0[i] : uh[(size_t)k * nx + i] - sh;
+        us[(size_t)k * nx + i] = v;
         sk += v;
         if (k == 0) dmax = fmax(dmax, fabs(v - u0[i]));
       }
       h2 = fmax(h2, fmax(fabs(P.dx * warp_sum(sk) - M0), warp_max(dmax)));
     }
+    int dummy;
+    h2 = block_max(h2, 0, dummy);
     solves = 2;
     if (!(h2 < P.tol)) solves = SNAP_ST_MAXITER;
   }
-  if (lane == 0) iters[b] = solves;
+  if (threadIdx.x == 0) iters[b] = solves;
 }
 
 }  // namespace snap

@@ -235,12 +235,33 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, k, x0.tm, tm_uh);
 
+  // W == 1: the mass rows of level k are reduced over the lanes at the start of level k + 1 (branch-free, T
+  // butterflies interleaved), so that the shuffle latency hides behind that level's arithmetic
+  const double dxm = P.dx;
+  const bool mass_lane = has_mass && w == 0 && lane == 0;
+  auto mass_rows = [&](bool valid) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+      for (int t = 0; t < T; ++t) ms[t] += __shfl_xor_sync(SNAP_FULL, ms[t], o);
+    }
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      const double hm = fabs(fma(dxm, ms[t], -M0));
+      const bool on = mass_lane && valid;
+      ge_tol[t] |= on && (hm >= tol);
+      gt_skip[t] |= on && (hm > skip);
+      h1[t] += on ? hm : 0.0;
+    }
+  };
+
   int s = 0, par = 0;
   for (int k = 0; k < nt; ++k) {
     pp.wait(s);
     double v[Q];
     const double* r0 = pp.row(s, 0);
     const double* ruh = same ? r0 : pp.row(s, 1);   // u_hat cells are re-read where needed
+    if constexpr (W == 1) mass_rows(k > 0);
     load_cells<Q>(r0, pp.lo, v);
     double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
     if constexpr (W > 1) {
@@ -288,7 +309,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         }
         par ^= 1;
         if (has_mass && w == 0 && lane == 0) {
-          const double hm = fabs(fma(P.dx, mtot, -M0));
+          const double hm = fabs(fma(dxm, mtot, -M0));
           ge_tol[t] |= (hm >= tol);
           gt_skip[t] |= (hm > skip);
           h1[t] += hm;
@@ -312,30 +333,13 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
       if (t < NU) { vL = vnL; vR = vnR; }
       else store_cells<Q>(so_y, pp.lo, q);
     }
-    if constexpr (W == 1) {
-      if (has_mass) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-          for (int t = 0; t < T; ++t) ms[t] += __shfl_xor_sync(SNAP_FULL, ms[t], o);
-        }
-        if (lane == 0) {
-#pragma unroll
-          for (int t = 0; t < T; ++t) {
-            const double hm = fabs(fma(P.dx, ms[t], -M0));
-            ge_tol[t] |= (hm >= tol);
-            gt_skip[t] |= (hm > skip);
-            h1[t] += hm;
-          }
-        }
-      }
-    }
     if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
     pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
     // stage s is free: every warp loaded its cells before the first exchange barrier of this level
     if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
     if (++s == nst) s = 0;
   }
+  if constexpr (W == 1) mass_rows(true);   // last level
   pp.drain();
   // ---- reduce: lanes -> warp -> group (fixed order: identical in every warp, run-to-run deterministic) ----
   double part[4 * T + 1];

@@ -83,6 +83,17 @@ __device__ __forceinline__ void store_cells(double* row, const LaneOff<Q>& lo, c
   }
 }
 
+// a lane's Q contiguous cells straight to global memory (128-bit stores)
+template <int Q>
+__device__ __forceinline__ void store_cells_global(double* __restrict__ g, const double (&x)[Q]) {
+  if constexpr (Q == 1) {
+    g[0] = x[0];
+  } else {
+#pragma unroll
+    for (int c = 0; c < Q / 2; ++c) reinterpret_cast<double2*>(g)[c] = make_double2(x[2 * c], x[2 * c + 1]);
+  }
+}
+
 __device__ __forceinline__ double shfl_prev(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 31) & 31); }
 __device__ __forceinline__ double shfl_next(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 1) & 31); }
 
@@ -173,7 +184,8 @@ struct RowPipe {
   // all TMA stores of the group are complete and visible to later (TMA or generic) loads
   __device__ __forceinline__ void drain() {
     if (lane == 0) bulk_wait_all<0>();
-    fence_proxy_async_all();
+    __threadfence();           // generic stores to global (direct row stores) are performed ...
+    fence_proxy_async_all();   // ... and ordered before the async-proxy (TMA) loads of the next pass
     gsync();
   }
 };
@@ -268,7 +280,8 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
       if (lane == 0) vL = r0[cellL];
       if (lane == 31) vR = r0[cellR];
     }
-    pp.out_ready();
+    constexpr bool kDirect = (W == 1);   // W == 1: results go straight to global memory (no staging, no proxy fence)
+    if constexpr (!kDirect) pp.out_ready();
     double* so_u = pp.out(k & 1);
     double* so_y = pp.out(2 + (k & 1));
 #pragma unroll
@@ -331,10 +344,16 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         else if (EMIT) q[c] = qc - (vc - uhr[c]);   // y
       }
       if (t < NU) { vL = vnL; vR = vnR; }
+      else if constexpr (kDirect) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
       else store_cells<Q>(so_y, pp.lo, q);
     }
-    if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
-    pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
+    if constexpr (kDirect) {
+      if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
+      if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + (EMIT ? 1 : 0);
+    } else {
+      if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
+      pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
+    }
     // stage s is free: every warp loaded its cells before the first exchange barrier of this level
     if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
     if (++s == nst) s = 0;
@@ -561,8 +580,10 @@ __device__ __forceinline__ void fused_fwd_dispatch(const DevParams& P, RowPipe<W
 // ------------------------------------------------------------------------------------------------
 template <int W, int Q>
 __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x, const Buf lam,
-                                         const CUtensorMap* ucopy, double* __restrict__ sig) {
+                                         const CUtensorMap* ucopy, double* __restrict__ ucopy_p,
+                                         double* __restrict__ sig) {
   using G = RowGeom<W, Q>;
+  constexpr int nx = G::NX;
   RowPipe<W, Q> pp = pp_ref;
 
   const int nt = P.nt, lane = pp.lane, nst = pp.nst, w = pp.w, first = pp.first;
@@ -581,7 +602,7 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
     double yv[Q], v[Q], l[Q];
     load_cells<Q>(pp.row(s, 0), pp.lo, yv);
     load_cells<Q>(pp.row(s, 1), pp.lo, v);
-    pp.out_ready();
+    if constexpr (W > 1) pp.out_ready();
     double lsum = 0.0;
 #pragma unroll
     for (int c = 0; c < Q; ++c) {
@@ -610,11 +631,17 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
       chk += lsum;
     }
     if (sig && w == 0 && lane == 0) sig[k] = stot;
-    double* so_l = pp.out(t & 1);
-    double* so_u = pp.out(2 + (t & 1));
-    store_cells<Q>(so_l, pp.lo, l);
-    if (ucopy) store_cells<Q>(so_u, pp.lo, v);
-    pp.store_rows(k, lam.tm, so_l, ucopy, so_u);
+    if constexpr (W == 1) {   // straight to global memory (see fused_fwd)
+      store_cells_global<Q>(lam.p + (size_t)k * nx + first, l);
+      if (ucopy_p) store_cells_global<Q>(ucopy_p + (size_t)k * nx + first, v);
+      if (lane == 0) pp.rows_wr += ucopy_p ? 2 : 1;
+    } else {
+      double* so_l = pp.out(t & 1);
+      double* so_u = pp.out(2 + (t & 1));
+      store_cells<Q>(so_l, pp.lo, l);
+      if (ucopy) store_cells<Q>(so_u, pp.lo, v);
+      pp.store_rows(k, lam.tm, so_l, ucopy, so_u);
+    }
     if (t + nst < nt) pp.issue(s, k - nst, lam.tm, x.tm);
     if (++s == nst) s = 0;
   }
@@ -669,13 +696,18 @@ __device__ __noinline__ void fused_min_norm(const DevParams& P, RowPipe<W, Q>& p
     pp.wait(s);
     double l[Q];
     load_cells<Q>(pp.row(s, 0), pp.lo, l);
-    pp.out_ready();
+    if constexpr (W > 1) pp.out_ready();
     const double add = P.dx * sig[k];
 #pragma unroll
     for (int cidx = 0; cidx < Q; ++cidx) l[cidx] += add;
-    double* so = pp.out(k & 1);
-    store_cells<Q>(so, pp.lo, l);
-    pp.store_rows(k, lamb.tm, so, nullptr, nullptr);
+    if constexpr (W == 1) {
+      store_cells_global<Q>(lamb.p + (size_t)k * nx + first, l);
+      if (lane == 0) pp.rows_wr += 1;
+    } else {
+      double* so = pp.out(k & 1);
+      store_cells<Q>(so, pp.lo, l);
+      pp.store_rows(k, lamb.tm, so, nullptr, nullptr);
+    }
     if constexpr (W > 1) pp.gsync();   // every warp has read stage s
     if (k + nst < nt) pp.issue(s, k + nst, lamb.tm, nullptr);
     if (++s == nst) s = 0;
@@ -910,7 +942,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     const CUtensorMap* const tm_copy = (xfin != ustar) ? &A.tm[TM_USTAR] : nullptr;
     double chk;
     if constexpr (KIND == KF_FUSED) chk = fused_bwd_f<Q>(P, pp, mk(xfin), mk(lam), tm_copy);
-    else chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), tm_copy, want_sig ? sig : nullptr);
+    else chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), tm_copy, tm_copy ? ustar : nullptr, want_sig ? sig : nullptr);
     ++sweeps;
     if (!finite_d(chk)) {
       status = SNAP_ST_NONFINITE;

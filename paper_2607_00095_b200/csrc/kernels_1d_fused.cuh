@@ -414,6 +414,7 @@ __device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_r
   constexpr int T = NU + (EMIT ? 1 : 0);
   static_assert(T >= 1 && T <= JT, "iterations per pass");
   RowPipe<1, Q> pp = pp_ref;
+  constexpr int nx = 32 * Q;
   const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
   const double fa = P.fi_a, fr = P.fi_dtrho;
   const bool same = (x0.p == uh.p);
@@ -443,9 +444,6 @@ __device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_r
     const double* r0 = pp.row(s, 0);
     const double* ruh = same ? r0 : pp.row(s, 1);
     load_cells<Q>(r0, pp.lo, v);
-    pp.out_ready();
-    double* so_u = pp.out(k & 1);
-    double* so_y = pp.out(2 + (k & 1));
 #pragma unroll
     for (int t = 0; t < T; ++t) {
       double q[Q], uhr[Q], hv[Q];
@@ -482,10 +480,10 @@ __device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_r
         if (t < NU) v[c] -= q[c];
         else if (EMIT) q[c] = q[c] - wv;   // y
       }
-      if (t >= NU) store_cells<Q>(so_y, pp.lo, q);
+      if (t >= NU) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
     }
-    if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
-    pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
+    if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
+    if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + (EMIT ? 1 : 0);
     if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
     if (++s == nst) s = 0;
   }
@@ -505,9 +503,10 @@ __device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_r
 // Fisher multiplier solve at the final iterate:  T_k lam_k = y_k + lam_{k+1} (k >= 1) ,  lam_0 = y_0 + lam_1.
 template <int Q>
 __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x, const Buf lam,
-                                           const CUtensorMap* ucopy) {
+                                           double* __restrict__ ucopy) {
   RowPipe<1, Q> pp = pp_ref;
-  const int nt = P.nt, lane = pp.lane, nst = pp.nst;
+  constexpr int nx = 32 * Q;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
   double lo[Q];
 #pragma unroll
   for (int c = 0; c < Q; ++c) lo[c] = 0.0;
@@ -521,7 +520,6 @@ __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp
     double l[Q], v[Q];
     load_cells<Q>(pp.row(s, 0), pp.lo, l);
     load_cells<Q>(pp.row(s, 1), pp.lo, v);
-    pp.out_ready();
 #pragma unroll
     for (int c = 0; c < Q; ++c) l[c] += lo[c];
     if (k > 0) {
@@ -531,11 +529,9 @@ __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp
     }
 #pragma unroll
     for (int c = 0; c < Q; ++c) { lo[c] = l[c]; chk += l[c]; }
-    double* so_l = pp.out(t & 1);
-    double* so_u = pp.out(2 + (t & 1));
-    store_cells<Q>(so_l, pp.lo, l);
-    if (ucopy) store_cells<Q>(so_u, pp.lo, v);
-    pp.store_rows(k, lam.tm, so_l, ucopy, so_u);
+    store_cells_global<Q>(lam.p + (size_t)k * nx + first, l);
+    if (ucopy) store_cells_global<Q>(ucopy + (size_t)k * nx + first, v);
+    if (lane == 0) pp.rows_wr += ucopy ? 2 : 1;
     if (t + nst < nt) pp.issue(s, k - nst, lam.tm, x.tm);
     if (++s == nst) s = 0;
   }
@@ -738,8 +734,8 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) + (size_t)slot * A.warp_bytes;
   RowPipe<W, Q> pp;
   pp.stage = reinterpret_cast<double*>(base);
-  pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;
-  pp.xch = pp.orow + (size_t)4 * G::RP;
+  pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;           // output staging rows: only W > 1 uses them
+  pp.xch = pp.orow + (size_t)(W > 1 ? 4 : 0) * G::RP;
   pp.red = pp.xch + G::XCH;
   pp.bar0 = smem_u32(pp.red + W * kRed);
   pp.phase = 0;
@@ -941,7 +937,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     const bool want_sig = (P.kind == SNAP_BURGERS1D_LF_MASS) && (P.lambda_mode == 0);
     const CUtensorMap* const tm_copy = (xfin != ustar) ? &A.tm[TM_USTAR] : nullptr;
     double chk;
-    if constexpr (KIND == KF_FUSED) chk = fused_bwd_f<Q>(P, pp, mk(xfin), mk(lam), tm_copy);
+    if constexpr (KIND == KF_FUSED) chk = fused_bwd_f<Q>(P, pp, mk(xfin), mk(lam), tm_copy ? ustar : nullptr);
     else chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), tm_copy, tm_copy ? ustar : nullptr, want_sig ? sig : nullptr);
     ++sweeps;
     if (!finite_d(chk)) {

@@ -131,6 +131,7 @@ struct RowPipe {
   double* orow;    // [4][RP]
   double* xch;     // [2][W][8]
   double* red;     // [W][kRed] partial sums of a pass
+  double* aux;     // W = 1: min(nt, 512) doubles (suffix sums of the min-norm correction)
   uint32_t bar0, phase;
   int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
   LaneOff<Q> lo;
@@ -646,6 +647,96 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
   return (W > 1) ? chk : warp_sum(chk);
 }
 
+// W = 1 version of the min-norm correction below.  The nt x nt SPD tridiagonal system is solved by the whole warp
+// (QT contiguous rows per lane, partition + cyclic reduction, tridiag.cuh) instead of one lane running Thomas, the
+// suffix sums go to shared memory, and the rank-nt update lam_loc[j][.] += dx S_j is a plain coalesced
+// read-add-write stream (it is elementwise, so it needs neither the lane-contiguous layout nor TMA staging).
+template <int QT>
+__device__ __forceinline__ void min_norm_coeffs(const DevParams& P, int lane, const double* __restrict__ sig,
+                                                double* __restrict__ ssuf, double* __restrict__ lmass) {
+  const int nt = P.nt;
+  const double cdiag = (double)P.nx * P.dx * P.dx;
+  double a[QT], b[QT], c[QT], d[QT];
+#pragma unroll
+  for (int j = 0; j < QT; ++j) {
+    const int r = lane * QT + j;
+    const bool valid = r < nt;
+    const double s0 = valid ? sig[r] : 0.0, s1 = (r + 1 < nt) ? sig[r + 1] : 0.0;
+    a[j] = (valid && r > 0) ? -1.0 : 0.0;
+    c[j] = (r + 1 < nt) ? -1.0 : 0.0;
+    b[j] = valid ? ((r == nt - 1) ? 1.0 : 2.0) + cdiag : 1.0;
+    d[j] = valid ? -P.dx * (s0 - s1) : 0.0;
+  }
+  warp_tridiag<QT>(a, b, c, d, lane);   // d = t
+  // suffix sums S_r = sum_{k >= r} t_k : inside the lane, then over the lanes above
+  double suf[QT];
+  double run = 0.0;
+#pragma unroll
+  for (int j = QT - 1; j >= 0; --j) { run += d[j]; suf[j] = run; }
+  double incl = run;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const double v = __shfl_down_sync(SNAP_FULL, incl, o);
+    if (lane + o < 32) incl += v;
+  }
+  const double above = incl - run;
+#pragma unroll
+  for (int j = 0; j < QT; ++j) {
+    const int r = lane * QT + j;
+    if (r < nt) { ssuf[r] = suf[j] + above; lmass[r] = -d[j]; }
+  }
+}
+
+template <int Q>
+__device__ __noinline__ void fused_min_norm_w1(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf lamb,
+                                               const double* __restrict__ sig) {
+  constexpr int nx = 32 * Q;
+  RowPipe<1, Q>& pp = pp_ref;
+  const int nt = P.nt, lane = pp.lane;
+  double* ssuf = pp.aux;
+  double* lmass = lamb.p + (size_t)nt * nx;
+  __syncwarp();
+  if (nt <= 32) min_norm_coeffs<1>(P, lane, sig, ssuf, lmass);
+  else if (nt <= 64) min_norm_coeffs<2>(P, lane, sig, ssuf, lmass);
+  else if (nt <= 128) min_norm_coeffs<4>(P, lane, sig, ssuf, lmass);
+  else if (nt <= 256) min_norm_coeffs<8>(P, lane, sig, ssuf, lmass);
+  else min_norm_coeffs<16>(P, lane, sig, ssuf, lmass);
+  __syncwarp();
+  // lam_loc[k][.] += dx S_k, four levels in flight per lane
+  constexpr int V = (nx >= 64) ? nx / 64 : 1;   // double2 per lane and level (nx = 32: lanes 16..31 idle)
+  const double dxm = P.dx;
+  double2* base = reinterpret_cast<double2*>(lamb.p);
+  const bool act = (nx >= 64) || lane < 16;
+  int k = 0;
+  for (; k + 4 <= nt; k += 4) {
+    double2 x[4][V];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int j = 0; j < V; ++j)
+        if (act) x[u][j] = base[(size_t)(k + u) * (nx / 2) + lane + 32 * j];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const double add = dxm * ssuf[k + u];
+#pragma unroll
+      for (int j = 0; j < V; ++j)
+        if (act) base[(size_t)(k + u) * (nx / 2) + lane + 32 * j] = make_double2(x[u][j].x + add, x[u][j].y + add);
+    }
+  }
+  for (; k < nt; ++k) {
+    const double add = dxm * ssuf[k];
+#pragma unroll
+    for (int j = 0; j < V; ++j)
+      if (act) {
+        double2 x = base[(size_t)k * (nx / 2) + lane + 32 * j];
+        base[(size_t)k * (nx / 2) + lane + 32 * j] = make_double2(x.x + add, x.y + add);
+      }
+  }
+  if (lane == 0) { pp.rows_rd += nt; pp.rows_wr += nt; }
+  __threadfence();
+  __syncwarp();
+}
+
 // Minimum-norm multiplier for the linearly dependent mass rows of kind 4 (streaming
 // recipe): with level sums sigma_j of the basic solution (mass multipliers 0) and c = nx dx^2,
 //   (D^T D + c I) t = -dx D^T sigma ,  lam_mass[k] = -t_k ,  lam_loc[j][.] += dx sum_{k>=j} t_k
@@ -737,7 +828,8 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;           // output staging rows: only W > 1 uses them
   pp.xch = pp.orow + (size_t)(W > 1 ? 4 : 0) * G::RP;
   pp.red = pp.xch + G::XCH;
-  pp.bar0 = smem_u32(pp.red + W * kRed);
+  pp.aux = pp.red + W * kRed;
+  pp.bar0 = smem_u32(pp.aux + (W == 1 ? (nt < 512 ? nt : 512) : 0));
   pp.phase = 0;
   pp.nst = A.nst; pp.lane = lane; pp.w = w; pp.bar_id = 1 + slot;
   pp.first = (w * 32 + lane) * Q;
@@ -947,7 +1039,14 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
       for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
     } else if (P.has_mass) {
       if (want_sig) {
-        if constexpr (KIND == KB_FUSED) fused_min_norm<W, Q>(P, pp, mk(lam), sig, tt);
+        if constexpr (KIND == KB_FUSED) {
+          if constexpr (W == 1) {
+            if (nt <= 512) fused_min_norm_w1<Q>(P, pp, mk(lam), sig);
+            else fused_min_norm<W, Q>(P, pp, mk(lam), sig, tt);
+          } else {
+            fused_min_norm<W, Q>(P, pp, mk(lam), sig, tt);
+          }
+        }
         ++sweeps;
       } else {
         for (int k = gtid; k < nt; k += GT) lam[n + k] = 0.0;

@@ -33,7 +33,7 @@ import workloads as W  # noqa: E402
 METRIC = "projected samples/sec to ||h||inf<1e-10 (fp64, 1 B200); % of HBM roofline"
 UNIT = "projections/s"
 N_TAU = 50
-PROFILED_TRAFFIC_CFG5 = 5.855e9   # bytes, launch 0 of profiles/r01c_project1d_fused.md
+PROFILED_TRAFFIC_CFG5 = 5.796e9   # bytes, launch 0 of profiles/r01d_project1d_fused.md
 
 
 def load_peaks():
@@ -328,9 +328,9 @@ def run_gpu(args):
     alg_bytes_call = run.traffic_model()
     traffic, traffic_note = args.traffic, None
     if traffic is None and cfg == 5:
-        # ncu --set full capture of the first two launches of the timed step (tau = 1/50, 2/50), profiles/r01c_*.md
+        # ncu --set full capture of the first two launches of the timed step (tau = 1/50, 2/50), profiles/r01d_*.md
         traffic = PROFILED_TRAFFIC_CFG5
-        traffic_note = ("dram__bytes_read.sum + dram__bytes_write.sum of launch 0 (tau=1/50), profiles/r01c_project1d_fused.md; "
+        traffic_note = ("dram__bytes_read.sum + dram__bytes_write.sum of launch 0 (tau=1/50), profiles/r01d_project1d_fused.md; "
                         f"algorithmic bytes of that launch: {alg_bytes_call[0]:.4g}")
     kern_s = sum(sum(k) for k in kern_ms) * 1e-3
     alg_total = sum(alg_bytes_call) * args.steps

@@ -228,7 +228,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
   double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
   double h1[T], wd[T], dd[T];              // per-lane partial sums (thread 0 of the group also takes the mass rows)
   bool ge_tol[T], gt_skip[T];              // some |h| >= tol / > kPolishSkip tol seen (all ||h||_inf is needed for)
-  double ms[T];                            // per-lane sum of the iterate's cells (mass rows)
+  double ms[T], msp[T];                    // per-lane sum of the iterate's cells (mass rows): this level, previous level
   const double tol = P.tol, skip = kPolishSkip * P.tol;
   double f2 = 0.0;
   {
@@ -242,7 +242,7 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         phi[t][c] = u0r[c];   // level 0: h_0 = x[0] - u0
         cc[t][c] = 0.0;
       }
-      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false; ms[t] = 0.0;
+      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false; ms[t] = 0.0; msp[t] = 0.0;
     }
   }
   const int npro = nst < nt ? nst : nt;
@@ -256,11 +256,11 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
-      for (int t = 0; t < T; ++t) ms[t] += __shfl_xor_sync(SNAP_FULL, ms[t], o);
+      for (int t = 0; t < T; ++t) msp[t] += __shfl_xor_sync(SNAP_FULL, msp[t], o);
     }
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-      const double hm = fabs(fma(dxm, ms[t], -M0));
+      const double hm = fabs(fma(dxm, msp[t], -M0));
       const bool on = mass_lane && valid;
       ge_tol[t] |= on && (hm >= tol);
       gt_skip[t] |= on && (hm > skip);
@@ -274,7 +274,6 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
     double v[Q];
     const double* r0 = pp.row(s, 0);
     const double* ruh = same ? r0 : pp.row(s, 1);   // u_hat cells are re-read where needed
-    if constexpr (W == 1) mass_rows(k > 0);
     load_cells<Q>(r0, pp.lo, v);
     double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
     if constexpr (W > 1) {
@@ -302,6 +301,9 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
         wd[t] = fma(wv, q[c], wd[t]);
         dd[t] = fma(q[c], q[c], dd[t]);
         if (t == 0) f2 = fma(wv, wv, f2);
+      }
+      if constexpr (W == 1) {
+        if (t == 0) mass_rows(k > 0);   // previous level's mass rows: independent of this level's arithmetic
       }
       // end values of the next iterate (only the two ends are exchanged; the rest is updated in place below)
       const double vn0 = (t < NU) ? v[0] - q[0] : v[0], vnE = (t < NU) ? v[Q - 1] - q[Q - 1] : v[Q - 1];
@@ -348,6 +350,8 @@ __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref
       else if constexpr (kDirect) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
       else store_cells<Q>(so_y, pp.lo, q);
     }
+#pragma unroll
+    for (int t = 0; t < T; ++t) msp[t] = ms[t];
     if constexpr (kDirect) {
       if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
       if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + (EMIT ? 1 : 0);

@@ -112,6 +112,10 @@ __device__ __forceinline__ double tree_sum(const double (&x)[Q]) {
   }
 }
 
+#ifndef SNAP_INLINE_HOT
+#define SNAP_INLINE_HOT 1
+#endif
+
 constexpr int kRed = 24;   // doubles per warp in the reduction scratch (>= 4 JT + 1)
 
 // a global buffer of the path: its tensor map (rows as TMA boxes) and the sample's base pointer (generic access)
@@ -208,7 +212,7 @@ struct FusedStats {
 // `xout` when NU > 0.
 // ------------------------------------------------------------------------------------------------
 template <int W, int Q, int JT, int NU, bool EMIT>
-__device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
+__device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
                                        const double* __restrict__ u0, const Buf xout, const Buf yout, const double M0,
                                        FusedStats<JT>& S) {
   using G = RowGeom<W, Q>;
@@ -548,11 +552,22 @@ __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp
 // runtime (J, T) -> static instantiation; KIND: KB_FUSED (Burgers family) or KF_FUSED (Fisher, W = 1)
 constexpr int KB_FUSED = 1, KF_FUSED = 2;
 
+// out-of-line copy for the rarely used pass shapes; the two shapes every projection runs (JT updates; JT - 1 updates
+// + y) are inlined into the kernel so that the grid constants stay constant-bank operands instead of registers
+template <int W, int Q, int JT, int NU, bool EMIT>
+__device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
+                                       const double* __restrict__ u0, const Buf xout, const Buf yout, const double M0,
+                                       FusedStats<JT>& S) {
+  fused_fwd_body<W, Q, JT, NU, EMIT>(P, pp_ref, x0, uh, u0, xout, yout, M0, S);
+}
+
 template <int KIND, int W, int Q, int JT, int NU, bool EMIT>
 __device__ __forceinline__ void fused_fwd_kind(const DevParams& P, RowPipe<W, Q>& pp, const Buf x0, const Buf uh,
                                                const double* u0, const Buf xout, const Buf yout, double M0,
                                                FusedStats<JT>& S) {
   if constexpr (KIND == KF_FUSED) fused_fwd_f<Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, S);
+  else if constexpr (SNAP_INLINE_HOT && W == 1 && ((NU == JT && !EMIT) || (NU == JT - 1 && EMIT)))
+    fused_fwd_body<W, Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, M0, S);
   else fused_fwd<W, Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, M0, S);
 }
 

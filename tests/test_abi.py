@@ -58,9 +58,16 @@ def test_create_validates_arguments(lib):
         with pytest.raises(lib.SnapError):
             lib.snap_problem_create(bad["kind"], bad["nx"], bad["ny"], bad["nt"], ok)
     for badp in [dict(dx=0.0, dt=1e-3), dict(dx=0.1, dt=-1.0), dict(dx=0.1, dt=1e-3, tol=0.0),
-                 dict(dx=0.1, dt=1e-3, ls_shrink=1.5), dict(dx=0.1, dt=1e-3, lambda_mode=3)]:
+                 dict(dx=0.1, dt=1e-3, ls_shrink=1.5), dict(dx=0.1, dt=1e-3, lambda_mode=3),
+                 dict(dx=0.1, dt=1e-3, gn_fuse=-2), dict(dx=0.1, dt=1e-3, gn_fuse=65)]:
         with pytest.raises(lib.SnapError):
             lib.snap_problem_create(lib.BURGERS1D_LF, 32, 1, 16, badp)
+    for fuse in (-1, 0, 1, 3):                 # classic path, default, capped
+        lib.snap_problem_create(lib.BURGERS1D_LF, 32, 1, 16, dict(ok, gn_fuse=fuse)).destroy()
+    # the workspace carries the per-sample work counters of snap_project_stats
+    p = lib.snap_problem_create(lib.FISHER1D_IE, 64, 1, 16, ok)
+    assert lib.snap_workspace_bytes(p, 3) >= 2 * 3 * p.n * 8 + 3 * 2 * 16 * 8 + 3 * 32
+    p.destroy()
     assert "invalid" in lib.snap_strerror(-1)
 
 

@@ -417,7 +417,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
 // partition + cyclic-reduction solver of tridiag.cuh; the level matrix depends on the current level only.
 // ------------------------------------------------------------------------------------------------
 template <int Q, int JT, int NU, bool EMIT>
-__device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x0, const Buf uh,
+__device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x0, const Buf uh,
                                          const double* __restrict__ u0, const Buf xout, const Buf yout,
                                          FusedStats<JT>& S) {
   constexpr int T = NU + (EMIT ? 1 : 0);
@@ -509,6 +509,13 @@ __device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_r
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
 }
 
+template <int Q, int JT, int NU, bool EMIT>
+__device__ __noinline__ void fused_fwd_f(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x0, const Buf uh,
+                                         const double* __restrict__ u0, const Buf xout, const Buf yout,
+                                         FusedStats<JT>& S) {
+  fused_fwd_f_body<Q, JT, NU, EMIT>(P, pp_ref, x0, uh, u0, xout, yout, S);
+}
+
 // Fisher multiplier solve at the final iterate:  T_k lam_k = y_k + lam_{k+1} (k >= 1) ,  lam_0 = y_0 + lam_1.
 template <int Q>
 __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x, const Buf lam,
@@ -565,7 +572,11 @@ template <int KIND, int W, int Q, int JT, int NU, bool EMIT>
 __device__ __forceinline__ void fused_fwd_kind(const DevParams& P, RowPipe<W, Q>& pp, const Buf x0, const Buf uh,
                                                const double* u0, const Buf xout, const Buf yout, double M0,
                                                FusedStats<JT>& S) {
-  if constexpr (KIND == KF_FUSED) fused_fwd_f<Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, S);
+  if constexpr (KIND == KF_FUSED) {
+    if constexpr (SNAP_INLINE_HOT && ((NU == JT && !EMIT) || (NU == JT - 1 && EMIT)))
+      fused_fwd_f_body<Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, S);
+    else fused_fwd_f<Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, S);
+  }
   else if constexpr (SNAP_INLINE_HOT && W == 1 && ((NU == JT && !EMIT) || (NU == JT - 1 && EMIT)))
     fused_fwd_body<W, Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, M0, S);
   else fused_fwd<W, Q, JT, NU, EMIT>(P, pp, x0, uh, u0, xout, yout, M0, S);

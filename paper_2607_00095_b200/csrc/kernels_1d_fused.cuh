@@ -219,6 +219,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
   constexpr int nx = G::NX;
   constexpr int T = NU + (EMIT ? 1 : 0);
   static_assert(T >= 1 && T <= JT, "iterations per pass");
+  constexpr bool kFirstPass = (NU == JT && !EMIT);   // this shape is only planned as the first pass: x_0 == u_hat
   RowPipe<W, Q> pp = pp_ref;   // registers; the mutable fields are written back at the end
   const int nt = P.nt, lane = pp.lane, nst = pp.nst, w = pp.w, first = pp.first;
   const double a0 = P.bs_a0, e = P.bs_e, qs = P.bs_qs, hs = P.bs_hs;
@@ -292,19 +293,21 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     for (int t = 0; t < T; ++t) {
       double q[Q], uhr[Q];
       const double msum = tree_sum<Q>(v);
-      load_cells<Q>(ruh, pp.lo, uhr);   // 128-bit conflict-free reads; not kept across iterations (registers)
+      if (!(kFirstPass && t == 0)) load_cells<Q>(ruh, pp.lo, uhr);   // 128-bit conflict-free reads; not kept across iterations
 #pragma unroll
       for (int c = 0; c < Q; ++c) {
         const double h = v[c] - phi[t][c];
         q[c] = h + cc[t][c];
-        const double wv = v[c] - uhr[c];
         const double ah = fabs(h);
         ge_tol[t] |= (ah >= tol);
         gt_skip[t] |= (ah > skip);
         h1[t] += ah;
-        wd[t] = fma(wv, q[c], wd[t]);
         dd[t] = fma(q[c], q[c], dd[t]);
-        if (t == 0) f2 = fma(wv, wv, f2);
+        if (!(kFirstPass && t == 0)) {   // the first pass starts at x_0 = u_hat: w = 0 there
+          const double wv = v[c] - uhr[c];
+          wd[t] = fma(wv, q[c], wd[t]);
+          if (t == 0) f2 = fma(wv, wv, f2);
+        }
       }
       if constexpr (W == 1) {
         if (t == 0) mass_rows(k > 0);   // previous level's mass rows: independent of this level's arithmetic
@@ -931,7 +934,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
       const int budget = P.max_iter - steps - (pend ? 1 : 0);
       if (J > budget) J = budget;
     }
-    if (J > JT - 1 && (sweeps > 0 || conv || jcap < JT)) J = JT - 1;
+    if (J > JT - 1 && (sweeps > 0 || conv || jcap < JT || x0 != uh)) J = JT - 1;   // the JT-update shape assumes x_0 == u_hat
     if (J < 0) J = 0;
     const int T = (J < JT) ? J + 1 : J;
     fused_fwd_dispatch<KIND, W, Q, JT>(P, pp, mk(x0), mk(uh), u0, mk(xo), mk(lam), J, T, M0, S);

@@ -377,3 +377,40 @@ def test_project_stats_counts_the_rows_moved(S):
     assert (st[:, 2] >= 5 * nt).all() and (st[:, 3] >= 4 * nt).all()
     assert (st[:, 1] >= 4).all()
     p.destroy()
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_fused_path_edge_shapes_and_params(S, cfg):
+    """Fused path at the edges: fewer levels than ring stages, nt not a multiple of the unroll factors, polish 0 / 2,
+    a loose tolerance, max_iter = 0, and batch sizes that give 1, 2 and 8 samples per CTA."""
+    for kw, prm in [(dict(batch=2, nx=32, nt=2), {}), (dict(batch=2, nx=64, nt=3), {}), (dict(batch=3, nx=32, nt=7), {}),
+                    (dict(batch=2, nx=64, nt=21), dict(polish=0)), (dict(batch=2, nx=64, nt=21), dict(polish=2)),
+                    (dict(batch=2, nx=128, nt=10), dict(tol=1e-4, polish=0))]:
+        wl = W.make_workload(cfg, **kw)
+        g = gpu_project(S, wl, wl.u_hat, params=prm)
+        p = dict(wl.params, **prm)
+        for b in range(wl.batch):
+            o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), p)
+            assert o["status"] == 0 and g["iters"][b] > 0, (kw, prm, int(g["iters"][b]))
+            # with a loose tolerance / no polish both sides stop early at slightly different iterates
+            tol_u = 1e-9 if not prm.get("tol") else 50 * prm["tol"]
+            ru = np.abs(g["u"][b] - o["u"]).max() / np.abs(o["u"]).max()
+            assert ru <= tol_u, (kw, prm, ru)
+            if not prm.get("tol"):
+                assert rel_lam(g["lam"][b], o["lam"]) <= (1e-8 if prm.get("polish", 1) else 1e-6), (kw, prm)
+        assert g["norms"][:, 0].max() < p.get("tol", 1e-10)
+    wl = W.make_workload(cfg, batch=2, nx=64, nt=12)
+    g = gpu_project(S, wl, wl.u_hat, params=dict(max_iter=0))
+    assert (g["iters"] == -1).all()
+    o = O.project(wl.kind, wl.u_hat[0].numpy(), wl.cdata[0].numpy(), dict(wl.params, max_iter=0))
+    np.testing.assert_array_equal(g["u"][0], o["u"])                    # no step taken: u* = u_hat
+    np.testing.assert_allclose(g["lam"][0], o["lam"], rtol=0, atol=1e-9 * max(1.0, np.abs(o["lam"]).max()))
+    # samples per CTA: 149 -> 2, 1200 -> 8 (more CTAs than SMs); every sample must equal the same sample run alone
+    for B in (149, 1200):
+        wl = W.make_workload(cfg, batch=B, nx=32, nt=9)
+        g = gpu_project(S, wl, wl.u_hat)
+        assert (g["iters"] > 0).all() and g["norms"][:, 0].max() < 1e-10
+        for b in (0, B // 2, B - 1):
+            one = gpu_project(S, wl, wl.u_hat[b:b + 1].clone(), cdata=wl.cdata[b:b + 1])
+            np.testing.assert_array_equal(one["u"][0], g["u"][b])
+            np.testing.assert_array_equal(one["lam"][0], g["lam"][b])

@@ -86,7 +86,7 @@ typedef struct {
   int ls_max;         /* maximum number of reductions per step              (default 20)                      */
   double pcg_rtol;    /* 2D: PCG stops at ||r - S lam||_2 <= pcg_rtol ||r||_2 (default 1e-13)  */
   int pcg_max;        /* 2D: PCG iteration cap per solve                    (default 200)                     */
-  int precond;        /* 2D: 0 none, 1 time-line, 2 time-line x ADI, 3 time-line x exact level solve (default 2) */
+  int precond;        /* 2D: 0 none, 1 time-line, 2 time-line x ADI         (default 2)                       */
   int lambda_mode;    /* 0 = minimum-norm multiplier, 1 = basic (redundant multipliers = 0)    */
   int gn_fuse;        /* Burgers kinds (nx in {32,...,512}) and Fisher (nx in {32,...,256}): Gauss-Newton iterations carried by one
                          forward pass over the levels.  0 = as many as the kernel holds in

@@ -622,7 +622,7 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
   double lo[Q];
 #pragma unroll
   for (int c = 0; c < Q; ++c) lo[c] = 0.0;
-  double lL = 0.0, lR = 0.0, chk = 0.0;
+  double lL = 0.0, lR = 0.0, chk = 0.0, lsum_prev = 0.0;
   const int npro = nst < nt ? nst : nt;
   for (int t = 0; t < npro; ++t) pp.issue(t, nt - 1 - t, lam.tm, x.tm);
   int s = 0, par = 0;
@@ -633,6 +633,12 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
     load_cells<Q>(pp.row(s, 0), pp.lo, yv);
     load_cells<Q>(pp.row(s, 1), pp.lo, v);
     if constexpr (W > 1) pp.out_ready();
+    if constexpr (W == 1) {   // level sum of the previous step: the butterfly overlaps this level's arithmetic
+      if (sig) {
+        const double sp = warp_sum(lsum_prev);
+        if (lane == 0 && t > 0) sig[k + 1] = sp;
+      }
+    }
     double lsum = 0.0;
 #pragma unroll
     for (int c = 0; c < Q; ++c) {
@@ -644,8 +650,9 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
     for (int c = 0; c < Q; ++c) lo[c] = l[c];
     lL = shfl_prev(l[Q - 1], lane);
     lR = shfl_next(l[0], lane);
-    double stot = (sig || W > 1) ? warp_sum(lsum) : 0.0;
+    double stot = 0.0;
     if constexpr (W > 1) {
+      stot = warp_sum(lsum);
       double* xs = pp.xch + (size_t)par * (W * 8);
       if (lane == 0) { xs[w * 8 + 0] = l[0]; xs[w * 8 + 4] = stot; }
       if (lane == 31) xs[w * 8 + 1] = l[Q - 1];
@@ -657,10 +664,11 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
       for (int i = 0; i < W; ++i) stot += xs[i * 8 + 4];
       par ^= 1;
       chk += stot;
+      if (sig && w == 0 && lane == 0) sig[k] = stot;
     } else {
       chk += lsum;
+      lsum_prev = lsum;
     }
-    if (sig && w == 0 && lane == 0) sig[k] = stot;
     if constexpr (W == 1) {   // straight to global memory (see fused_fwd)
       store_cells_global<Q>(lam.p + (size_t)k * nx + first, l);
       if (ucopy_p) store_cells_global<Q>(ucopy_p + (size_t)k * nx + first, v);
@@ -674,6 +682,12 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
     }
     if (t + nst < nt) pp.issue(s, k - nst, lam.tm, x.tm);
     if (++s == nst) s = 0;
+  }
+  if constexpr (W == 1) {
+    if (sig) {
+      const double sp = warp_sum(lsum_prev);
+      if (lane == 0) sig[0] = sp;
+    }
   }
   pp.drain();
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;

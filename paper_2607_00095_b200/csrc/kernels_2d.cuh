@@ -13,7 +13,7 @@
 
 namespace snap {
 
-constexpr int kT2 = 512;          // threads per CTA (one CTA per sample)
+constexpr int kT2 = 1024;         // threads per CTA (one CTA per sample)
 
 struct Proj2dArgs {
   DevParams P;
@@ -64,7 +64,7 @@ __device__ __forceinline__ double blk_max(const Ctx2d& c, double v) {
 // A thread owns at most kCpt cells of a level (column i, rows jr, jr + rpp, ...).  The level passes first
 // gather all of a thread's global values into registers (independent loads in flight together) and only then
 // touch shared memory: a load-store-load chain per cell would expose the full memory latency kCpt times.
-constexpr int kCpt = 8;   // nx * ny <= 4096 cells over 512 threads
+constexpr int kCpt = 4;   // nx * ny <= 4096 cells over 1024 threads
 __device__ __forceinline__ void gather(const Ctx2d& c, const double* __restrict__ src, double (&t)[kCpt]) {
 #pragma unroll
   for (int u = 0; u < kCpt; ++u) {

@@ -116,6 +116,19 @@ __device__ __forceinline__ double tree_sum(const double (&x)[Q]) {
 #define SNAP_INLINE_HOT 1
 #endif
 
+// ||h||_inf is only ever compared with two thresholds (tol, kPolishSkip tol).  The passes therefore keep, per lane,
+// the maximum of the UPPER 32 bits of |h| (one integer max per cell on the ALU pipe instead of two FP64 compares;
+// for non-negative doubles the upper word orders like the value, NaN/Inf sort above everything), and a residual
+// counts as below a threshold only if its upper word is below the threshold's upper word.  That is the test
+// "||h||_inf < threshold rounded down to 21 significant bits": conservative, it never accepts a residual >= tol.
+// Returns 0: below kPolishSkip tol, 1: below tol, 2: not below tol.
+__device__ __forceinline__ double hinf_level(int hmx_lane, double tol, double skip) {
+  int m = hmx_lane;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(SNAP_FULL, m, o));
+  return (m >= __double2hiint(tol)) ? 2.0 : ((m >= __double2hiint(skip)) ? 1.0 : 0.0);
+}
+
 constexpr int kRed = 24;   // doubles per warp in the reduction scratch (>= 4 JT + 1)
 
 // a global buffer of the path: its tensor map (rows as TMA boxes) and the sample's base pointer (generic access)
@@ -232,7 +245,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
 
   double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
   double h1[T], wd[T], dd[T];              // per-lane partial sums (thread 0 of the group also takes the mass rows)
-  bool ge_tol[T], gt_skip[T];              // some |h| >= tol / > kPolishSkip tol seen (all ||h||_inf is needed for)
+  int hmx[T];                              // max over the upper 32 bits of |h| (see hinf_level)
   double ms[T], msp[T];                    // per-lane sum of the iterate's cells (mass rows): this level, previous level
   const double tol = P.tol, skip = kPolishSkip * P.tol;
   double f2 = 0.0;
@@ -247,7 +260,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
         phi[t][c] = u0r[c];   // level 0: h_0 = x[0] - u0
         cc[t][c] = 0.0;
       }
-      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false; ms[t] = 0.0; msp[t] = 0.0;
+      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; hmx[t] = 0; ms[t] = 0.0; msp[t] = 0.0;
     }
   }
   const int npro = nst < nt ? nst : nt;
@@ -267,8 +280,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     for (int t = 0; t < T; ++t) {
       const double hm = fabs(fma(dxm, msp[t], -M0));
       const bool on = mass_lane && valid;
-      ge_tol[t] |= on && (hm >= tol);
-      gt_skip[t] |= on && (hm > skip);
+      hmx[t] = max(hmx[t], on ? __double2hiint(hm) : 0);
       h1[t] += on ? hm : 0.0;
     }
   };
@@ -299,8 +311,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
         const double h = v[c] - phi[t][c];
         q[c] = h + cc[t][c];
         const double ah = fabs(h);
-        ge_tol[t] |= (ah >= tol);
-        gt_skip[t] |= (ah > skip);
+        hmx[t] = max(hmx[t], __double2hiint(ah));
         h1[t] += ah;
         dd[t] = fma(q[c], q[c], dd[t]);
         if (!(kFirstPass && t == 0)) {   // the first pass starts at x_0 = u_hat: w = 0 there
@@ -333,8 +344,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
         par ^= 1;
         if (has_mass && w == 0 && lane == 0) {
           const double hm = fabs(fma(dxm, mtot, -M0));
-          ge_tol[t] |= (hm >= tol);
-          gt_skip[t] |= (hm > skip);
+          hmx[t] = max(hmx[t], __double2hiint(hm));
           h1[t] += hm;
         }
       } else {
@@ -376,7 +386,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
   double part[4 * T + 1];
 #pragma unroll
   for (int t = 0; t < T; ++t) {
-    part[4 * t + 0] = __any_sync(SNAP_FULL, ge_tol[t]) ? 2.0 : (__any_sync(SNAP_FULL, gt_skip[t]) ? 1.0 : 0.0);
+    part[4 * t + 0] = hinf_level(hmx[t], tol, skip);
     part[4 * t + 1] = warp_sum(h1[t]);
     part[4 * t + 2] = warp_sum(wd[t]);
     part[4 * t + 3] = warp_sum(dd[t]);
@@ -435,7 +445,7 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
 
   double qo[T][Q], xp[T][Q];   // q_{k-1} and x_t[k-1] of iteration t, own cells
   double h1[T], wd[T], dd[T];
-  bool ge_tol[T], gt_skip[T];
+  int hmx[T];
   double f2 = 0.0;
   double u0r[Q];
 #pragma unroll
@@ -444,7 +454,7 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
   for (int t = 0; t < T; ++t) {
 #pragma unroll
     for (int c = 0; c < Q; ++c) { qo[t][c] = 0.0; xp[t][c] = 0.0; }
-    h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; ge_tol[t] = false; gt_skip[t] = false;
+    h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; hmx[t] = 0;
   }
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, k, x0.tm, tm_uh);
@@ -481,8 +491,7 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
       for (int c = 0; c < Q; ++c) {
         const double wv = v[c] - uhr[c];
         const double ah = fabs(hv[c]);
-        ge_tol[t] |= (ah >= tol);
-        gt_skip[t] |= (ah > skip);
+        hmx[t] = max(hmx[t], __double2hiint(ah));
         h1[t] += ah;
         wd[t] = fma(wv, q[c], wd[t]);
         dd[t] = fma(q[c], q[c], dd[t]);
@@ -504,7 +513,7 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
   S.f0 = 0.5 * f2s;
 #pragma unroll
   for (int t = 0; t < T; ++t) {
-    const double a = __any_sync(SNAP_FULL, ge_tol[t]) ? 2.0 : (__any_sync(SNAP_FULL, gt_skip[t]) ? 1.0 : 0.0);
+    const double a = hinf_level(hmx[t], tol, skip);
     const double b = warp_sum(h1[t]), c1 = -warp_sum(wd[t]), c2 = warp_sum(dd[t]);
     S.hlev[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
     S.bad[t] = !(finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(f2s));

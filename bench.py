@@ -33,7 +33,7 @@ import workloads as W  # noqa: E402
 METRIC = "projected samples/sec to ||h||inf<1e-10 (fp64, 1 B200); % of HBM roofline"
 UNIT = "projections/s"
 N_TAU = 50
-PROFILED_TRAFFIC_CFG5 = 5.760e9   # bytes, launch 0 of profiles/r01d_project1d_fused.md
+PROFILED_TRAFFIC_CFG5 = 5.761e9   # bytes, launch 0 of profiles/r01d_project1d_fused.md
 
 
 def load_peaks():

@@ -271,7 +271,7 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
 // ---- a6: PCG on S lam = b.  Returns 0 on success, 1 if pcg_max was hit ----------------------------------
 __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __restrict__ u, const double* __restrict__ b,
                          double* __restrict__ x, double* __restrict__ r, double* __restrict__ z, double* __restrict__ p,
-                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n) {
+                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n, const double rtol) {
   const int tid = threadIdx.x;
   double bb = 0.0;
 #pragma unroll 8
@@ -308,7 +308,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
     }
     rr = blk_sum(c, rr);
     if (!finite_d(rr)) return 2;
-    if (sqrt(rr) <= P.pcg_rtol * bnorm) {
+    if (sqrt(rr) <= rtol * bnorm) {
       // exit test on the true residual, recomputed
       __syncthreads();
       schur_apply(P, c, u, x, q);
@@ -320,7 +320,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
         tr = fma(rn, rn, tr);
       }
       tr = blk_sum(c, tr);
-      if (sqrt(tr) <= P.pcg_rtol * bnorm) return 0;
+      if (sqrt(tr) <= rtol * bnorm) return 0;
     }
     __syncthreads();
     const double rz_new = precond_apply(P, c, r, z, y);
@@ -418,7 +418,11 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     }
     ++solves;
     __syncthreads();
-    const int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n);
+    // Inexact Gauss-Newton: a step taken from a point that is still far from feasible does not need the Schur
+    // system solved to pcg_rtol; the forcing term shrinks with ||h||_inf, and every solve whose multiplier is
+    // returned or used for the polish step (||h||_inf < tol) runs to the full pcg_rtol (R15).
+    const double rt = (polishing || hinf < P.tol) ? P.pcg_rtol : fmax(P.pcg_rtol, fmin(1e-4, 1e-3 * hinf));
+    const int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n, rt);
     have_lam = true;
     __syncthreads();
     if (prc == 2) { status = SNAP_ST_NONFINITE; break; }

@@ -414,3 +414,22 @@ def test_fused_path_edge_shapes_and_params(S, cfg):
             one = gpu_project(S, wl, wl.u_hat[b:b + 1].clone(), cdata=wl.cdata[b:b + 1])
             np.testing.assert_array_equal(one["u"][0], g["u"][b])
             np.testing.assert_array_equal(one["lam"][0], g["lam"][b])
+
+
+def test_host_entry_point_chunked_pipeline_matches_device_path(S):
+    """snap_project_host cuts batches >= 128 into chunks that flow through three streams; the result must be
+    the one of a single device-side call (samples are independent blocks)."""
+    for cfg, B in ((5, 130), (3, 515)):
+        wl = W.make_workload(cfg, batch=B, nx=32, nt=9)
+        ref = gpu_project(S, wl, wl.u_hat)
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        uh = wl.u_hat.contiguous().pin_memory()
+        us = torch.empty_like(uh).pin_memory()
+        lam = torch.zeros(B, p.m, dtype=torch.float64).pin_memory()
+        it = torch.empty(B, dtype=torch.int32).pin_memory()
+        for warm in (False, True):                       # second call: warm = copies lam in as well
+            S.snap_project_host(p, B, uh, wl.cdata.contiguous(), us, lam, it, warm=warm)
+            np.testing.assert_array_equal(us.numpy(), ref["u"])
+            np.testing.assert_array_equal(lam.numpy(), ref["lam"])
+            np.testing.assert_array_equal(it.numpy(), ref["iters"])
+        p.destroy()

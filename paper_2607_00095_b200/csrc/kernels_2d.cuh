@@ -92,30 +92,35 @@ __device__ void rhs_pass(const DevParams& P, const Ctx2d& c, const double* __res
                          const double* __restrict__ uh, const double* __restrict__ u0, double* __restrict__ b,
                          double& hinf, double& h1, double& f, int& bad) {
   double a_inf = 0.0, a_1 = 0.0, a_f = 0.0;
+  double vn[kCpt], hn[kCpt], vc[kCpt], hc[kCpt], vp[kCpt] = {}, wp[kCpt] = {}, u0r[kCpt];
+  gather(c, u0, u0r);
+  gather(c, u, vn);
+  gather(c, uh, hn);
   for (int k = 0; k < c.nt; ++k) {
-    const double* uk = u + (size_t)k * c.L;
-    const double* uhk = uh + (size_t)k * c.L;
-    __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      const double v = uk[cell];
-      c.s0[cell] = v;
-      c.s1[cell] = v - uhk[cell];
+#pragma unroll
+    for (int t = 0; t < kCpt; ++t) { vc[t] = vn[t]; hc[t] = hn[t]; }
+    if (k + 1 < c.nt) {        // next level's values travel while this level is computed
+      gather(c, u + (size_t)(k + 1) * c.L, vn);
+      gather(c, uh + (size_t)(k + 1) * c.L, hn);
     }
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      const double v = c.s0[cell], w = c.s1[cell];
+    SNAP_FOR_OWN(c, t, cell, j) {
+      c.s0[cell] = vc[t];
+      c.s1[cell] = vc[t] - hc[t];
+    }
+    __syncthreads();
+    SNAP_FOR_OWN(c, t, cell, j) {
+      const double v = vc[t], w = v - hc[t];
       double h, bb;
       if (k == 0) {
-        h = v - u0[cell];
+        h = v - u0r[t];
         bb = h - w;
       } else {
         const int row = j * c.nx;
         const int yp = ((j + 1 == c.ny) ? 0 : j + 1) * c.nx + c.i, ym = ((j == 0) ? c.ny - 1 : j - 1) * c.nx + c.i;
-        const double vprev = uk[cell - c.L];
-        const double wprev = vprev - uhk[cell - c.L];
-        h = v - vprev - P.ac_ax * ((c.s0[row + c.ip] - v) + (c.s0[row + c.im] - v)) -
+        h = v - vp[t] - P.ac_ax * ((c.s0[row + c.ip] - v) + (c.s0[row + c.im] - v)) -
             P.ac_ay * ((c.s0[yp] - v) + (c.s0[ym] - v)) + P.dt * (v * v * v - v);
-        bb = h - (T_apply(P, c, c.s1, j, cell, v) - wprev);
+        bb = h - (T_apply(P, c, c.s1, j, cell, v) - wp[t]);
       }
       b[(size_t)k * c.L + cell] = bb;
       const double ah = fabs(h);
@@ -123,6 +128,8 @@ __device__ void rhs_pass(const DevParams& P, const Ctx2d& c, const double* __res
       a_inf = fmax(a_inf, ah);
       a_1 += ah;
       a_f = fma(w, w, a_f);
+      vp[t] = v;
+      wp[t] = w;
     }
   }
   hinf = blk_max(c, a_inf);
@@ -244,21 +251,30 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
                           const double* __restrict__ uh, const double* __restrict__ lam, double* __restrict__ trial,
                           double& linf, double& wd, double& dd) {
   double a_inf = 0.0, a_wd = 0.0, a_dd = 0.0;
+  double ln[kCpt], lc[kCpt], un[kCpt], uc[kCpt], hn[kCpt], hc[kCpt];
+  gather(c, lam, ln);
+  gather(c, u, un);
+  gather(c, uh, hn);
   for (int k = 0; k < c.nt; ++k) {
-    const double* uk = u + (size_t)k * c.L;
-    const double* lk = lam + (size_t)k * c.L;
+#pragma unroll
+    for (int t = 0; t < kCpt; ++t) { lc[t] = ln[t]; uc[t] = un[t]; hc[t] = hn[t]; }
+    if (k + 1 < c.nt) {
+      gather(c, lam + (size_t)(k + 1) * c.L, ln);
+      gather(c, u + (size_t)(k + 1) * c.L, un);
+      gather(c, uh + (size_t)(k + 1) * c.L, hn);
+    }
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) c.s0[cell] = lk[cell];
+    SNAP_FOR_OWN(c, t, cell, j) c.s0[cell] = lc[t];
     __syncthreads();
-    SNAP_FOR_CELLS(c, cell, j) {
-      const double v = uk[cell], hh = uh[(size_t)k * c.L + cell];
-      double g = (k == 0) ? c.s0[cell] : T_apply(P, c, c.s0, j, cell, v);
-      if (k + 1 < c.nt) g -= lk[cell + c.L];
+    SNAP_FOR_OWN(c, t, cell, j) {
+      const double v = uc[t], hh = hc[t];
+      double g = (k == 0) ? lc[t] : T_apply(P, c, c.s0, j, cell, v);
+      if (k + 1 < c.nt) g -= ln[t];
       const double tr = hh - g;
       trial[(size_t)k * c.L + cell] = tr;
       a_wd = fma(v - hh, tr - v, a_wd);
       a_dd = fma(tr - v, tr - v, a_dd);
-      const double al = fabs(c.s0[cell]);
+      const double al = fabs(lc[t]);
       if (!finite_d(al)) a_inf = 1.7976931348623157e308 * 2.0;
       a_inf = fmax(a_inf, al);
     }
@@ -309,6 +325,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
     rr = blk_sum(c, rr);
     if (!finite_d(rr)) return 2;
     if (sqrt(rr) <= rtol * bnorm) {
+      if (rtol > P.pcg_rtol) return 0;   // inexact (forcing-term) solve: the recurred residual is good enough
       // exit test on the true residual, recomputed
       __syncthreads();
       schur_apply(P, c, u, x, q);

@@ -11,7 +11,11 @@ step" in that order and notation:
        u_full <- u_hat - J^T lam+ ;  d <- u_full - u
        if ||h||_inf < tol:  polish (R4) and return
        mu <- max(mu, 1e-3, ((u - u_hat)^T d + 1/2 ||d||^2) / ((1 - rho) ||h||_1)),  rho = 1/2
-                                                   (N&W Eq. 18.36 with sigma = 1, Hessian of f = I; ref [15] L275)
+                                                   (mu_rule "nw18_36", default: N&W Eq. 18.36 with sigma = 1,
+                                                    Hessian of f = I; ref [15] L275)
+         or  mu <- max(mu, 1.1 ||lam+||_inf + 1e-3)     (mu_rule "lam_inf": SURVEY.md §8(c) algorithm listing)
+       -- the paper fixes no merit rule (only "filter line search", ref [29] L289); both are textbook choices
+          for the l1 exact penalty and tests/test_oracle_pins.py pins that the limit point is the same.
        Armijo back-tracking on phi(v) = 1/2 ||v - u_hat||^2 + mu ||h(v)||_1     (N&W ch. 18, ref [15] L275)
        u <- u + alpha d
 
@@ -77,6 +81,9 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     c1 = p.get("ls_c1", 1e-4)
     shrink = p.get("ls_shrink", 0.5)
     ls_max = int(p.get("ls_max", 20))
+    mu_rule = p.get("mu_rule", "nw18_36")
+    if mu_rule not in ("nw18_36", "lam_inf"):
+        raise ValueError(f"unknown mu_rule {mu_rule!r}")
     cg_state = {"rtol": 1e-13, "maxiter": 20000, "iters": 0}
     uh = u_hat.ravel()
     shape = u_hat.shape
@@ -130,9 +137,13 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
             break
         d = u_full - u
         h1 = float(np.abs(h).sum())
-        # penalty parameter from the predicted decrease of the quadratic model (N&W Eq. 18.36, sigma = 1):
-        # needs no multiplier, so an implementation may postpone the multiplier solve (R2)
-        mu = max(mu, MU_FLOOR, (float((u - uh) @ d) + 0.5 * float(d @ d)) / ((1.0 - MU_RHO) * h1))
+        if mu_rule == "nw18_36":
+            # penalty parameter from the predicted decrease of the quadratic model (N&W Eq. 18.36, sigma = 1):
+            # needs no multiplier, so an implementation may postpone the multiplier solve (R2)
+            mu = max(mu, MU_FLOOR, (float((u - uh) @ d) + 0.5 * float(d @ d)) / ((1.0 - MU_RHO) * h1))
+        else:
+            # mu >= 1.1 ||lam+||_inf (+ floor) makes the l1 penalty exact (N&W Thm 17.3)
+            mu = max(mu, 1.1 * float(np.abs(lam).max()) + MU_FLOOR)
         phi0 = 0.5 * float((u - uh) @ (u - uh)) + mu * h1
         Dphi = float((u - uh) @ d) - mu * h1
         alpha = 1.0

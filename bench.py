@@ -33,7 +33,18 @@ import workloads as W  # noqa: E402
 METRIC = "projected samples/sec to ||h||inf<1e-10 (fp64, 1 B200); % of HBM roofline"
 UNIT = "projections/s"
 N_TAU = 50
-PROFILED_TRAFFIC_CFG5 = 5.761e9   # bytes, launch 0 of profiles/r01d_project1d_fused.md
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic.json")   # written next to the ncu summaries it quotes
+
+
+def profiled_traffic(cfg: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the latest
+    `ncu --set full` capture summarised under profiles/ (profiles/traffic.json names the summary it comes from).
+    None if no capture of this workload is recorded."""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            return json.load(f).get(f"cfg{cfg}")
+    except Exception:
+        return None
 
 
 def load_peaks():
@@ -46,25 +57,15 @@ def load_peaks():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def a_solve_bytes(n: int, m: int) -> int:
-    """Classic path (Fisher, 2D outer loop, odd sizes): algorithmic bytes of one Gauss-Newton linear solve per
-    sample: forward sweep reads u, u_hat (16 n) and writes y (8 m); backward sweep reads
-    y, u, u_hat (8 m + 16 n) and writes lam, u+ (8 m + 8 n)  =>  40 n + 24 m."""
-    return 40 * n + 24 * m
-
-
-def algorithmic_bytes(run, iters_row):
-    """Bytes one snap_project launch must move.  Fused Burgers path: the rows of nx doubles
-    each pass over the levels reads and writes, counted per sample by the kernel itself (snap_project_stats:
-    u_hat / iterate / y rows in, iterate / y / lam rows out) -- the traffic of THIS variant, not of the 64 n
-    per-iteration model of SURVEY.md §8(d).  Classic path: solves x (40 n + 24 m)."""
+def algorithmic_bytes(run):
+    """Bytes one snap_project launch must move, from the kernel's own per-sample work counters
+    (snap_project_stats): (rows read + rows written) x doubles per row x 8.  A "row" is one time level of one
+    field; the counters describe the traffic of the variant that actually ran, e.g. 88 n bytes for
+    a typical cfg-5 projection on the fused path -- not the 64 n per iteration model of SURVEY.md §8(d)."""
     st = run.stats.cpu()
-    rows = int(st[:, 2].sum() + st[:, 3].sum())
-    if rows > 0:
-        return float(rows) * run.wl.nx * 8.0
-    if run.cfg == 1:
-        return float(run.B * (16 * run.wl.n + 8 * run.p.m))
-    return float(iters_row.clamp(min=0).sum()) * a_solve_bytes(run.wl.n, run.p.m)
+    S = run.S
+    rows = (st[:, S.STAT_ROWS_READ] + st[:, S.STAT_ROWS_WRITTEN]).to(torch.float64)
+    return float((rows * st[:, S.STAT_ROW_DOUBLES].to(torch.float64)).sum() * 8.0)
 
 
 class ClockSampler:
@@ -122,22 +123,34 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------------
 # reference arm = the oracle, as it stands, on the host cores (bounded sample)
 # ------------------------------------------------------------------------------------------------------
-def oracle_sample(cfg: int, n_samples: int, workers: int, tau_j: int = 25):
-    """Time the CPU oracle on `n_samples` problems of workload `cfg`; returns (projections/s, seconds, desc)."""
+def oracle_sample(cfg: int, n_samples: int, workers: int, taus=(25,)):
+    """Time the CPU oracle, as it stands, on `n_samples` problems of workload `cfg` (for cfg 5: at each flow time
+    tau_j, j in `taus`).  Returns (projections/s, seconds, description, workers used)."""
     import oracle as O
+    total_t, total_n, ok = 0.0, 0, True
+    used = workers
     if cfg == 5:
         wl = W.make_workload(5, batch=n_samples, with_u_hat=False)
-        uh = W.burgers_tau_input(wl, tau_j)
-        desc = f"{n_samples} samples of cfg5 (256x256, Burgers-LF + mass rows) at tau={tau_j}/{N_TAU}"
+        for j in taus:
+            uh = W.burgers_tau_input(wl, j)
+            t0 = time.perf_counter()
+            out = O.project_batch(wl.kind, uh.numpy(), wl.cdata.numpy(), wl.params, workers=workers)
+            total_t += time.perf_counter() - t0
+            total_n += n_samples
+            ok = ok and bool((out["iters"] > 0).all())
+            used = out["workers"]
+        desc = (f"{n_samples} samples of cfg5 (256x256, Burgers-LF + mass rows) at each of tau in "
+                f"{{{', '.join(f'{j}/{N_TAU}' for j in taus)}}}")
     else:
         wl = W.make_workload(cfg, batch=n_samples)
-        uh = wl.u_hat
+        t0 = time.perf_counter()
+        out = O.project_batch(wl.kind, wl.u_hat.numpy(), wl.cdata.numpy(), wl.params, workers=workers)
+        total_t = time.perf_counter() - t0
+        total_n = n_samples
+        ok = bool((out["iters"] > 0).all())
+        used = out["workers"]
         desc = f"{n_samples} samples of cfg{cfg}"
-    t0 = time.perf_counter()
-    out = O.project_batch(wl.kind, uh.numpy(), wl.cdata.numpy(), wl.params, workers=workers)
-    dt = time.perf_counter() - t0
-    ok = bool((out["iters"] > 0).all())
-    return n_samples / dt, dt, desc + ("" if ok else " [oracle reported non-convergence]"), out["workers"]
+    return total_n / total_t, total_t, desc + ("" if ok else " [oracle reported non-convergence]"), used
 
 
 def run_reference(args):
@@ -151,7 +164,7 @@ def run_reference(args):
     times = []
     desc = ""
     for s in range(args.warmup + args.steps):
-        v, dt, desc, used = oracle_sample(cfg, n_samples, workers, tau_j=25)
+        v, dt, desc, used = oracle_sample(cfg, n_samples, workers, taus=(25,))
         if s >= args.warmup:
             times.append(dt)
     total = sum(times)
@@ -161,7 +174,8 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "reference": "CPU oracle (oracle/, numpy/scipy), one step = a bounded sample"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": desc + " per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "host_cpu_count": cores, "kind": "oracle",
+                         "sample": desc + " per step"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -202,7 +216,7 @@ class GpuRun:
         self.iters = torch.zeros(self.calls, self.B, dtype=torch.int32, device=dev)
         self.ws = torch.empty(S.snap_workspace_bytes(self.p, self.B), dtype=torch.uint8, device=dev)
         self.norms = torch.empty(self.B, 4, dtype=torch.float64, device=dev)
-        self.stats = torch.zeros(self.B, 4, dtype=torch.int64, device=dev)
+        self.stats = torch.zeros(self.B, S.STAT_COUNT, dtype=torch.int64, device=dev)
 
     def step(self, events=None):
         """The whole hot path over one batch of input: `calls` back-to-back snap_project launches."""
@@ -223,7 +237,8 @@ class GpuRun:
                                 warm=(self.cfg == 5 and c > 0), workspace=self.ws)
             self.S.snap_project_stats(self.p, self.B, self.ws, self.stats)
             torch.cuda.synchronize()
-            out.append(algorithmic_bytes(self, self.iters[c].cpu()))
+            out.append(algorithmic_bytes(self))
+        self.variants = sorted(set(self.stats[:, self.S.STAT_VARIANT].cpu().tolist()))
         return out
 
     def check(self):
@@ -292,15 +307,51 @@ def e2e_steps(run: GpuRun, steps: int, warmup: int):
     return run.projections_per_step() * steps / dt, h2d, d2h, ok
 
 
+KERNEL_NAMES = {5: "project1d_fused_kernel<KB,1,8,3> (Burgers family, nx=256)", 2: "project1d_fused_kernel<KB,1,4,4> (nx=128)",
+                3: "project1d_fused_kernel<KF,1,4,3> (Fisher, nx=128)", 4: "project2d kernel (see variant)",
+                1: "heat_project_kernel"}
+
+
+def roofline_of(run, cfg, kern_s, alg_bytes_call, steps, peak, peak_src):
+    """HBM roofline of the workload's (single) kernel: algorithmic bytes per launch / live CUDA-event duration."""
+    alg_total = sum(alg_bytes_call) * steps
+    achieved = alg_total / kern_s / 1e9
+    prof = profiled_traffic(cfg)
+    out = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "traffic": None, "kernel": KERNEL_NAMES[cfg], "variants": getattr(run, "variants", None),
+           "peak_source": peak_src, "alg_bytes_per_launch_mean": alg_total / (steps * run.calls),
+           "launch_ms_mean": 1e3 * kern_s / (steps * run.calls), "frac_of_8TBs_spec": achieved / 8000.0,
+           "achieved_is": "model-based: the kernel's own row counters x row bytes / CUDA-event time"}
+    if prof is not None:
+        out["traffic"] = prof["dram_bytes_per_launch"]
+        out["traffic_note"] = prof.get("note")
+        # the same fraction on measured DRAM bytes: scale by the profiled launch's DRAM / algorithmic ratio
+        ratio = prof["dram_bytes_per_launch"] / prof["alg_bytes_per_launch"]
+        out["frac_dram"] = achieved * ratio / peak
+        out["dram_over_alg"] = ratio
+    return out
+
+
 def run_gpu(args):
+    from paper_2607_00095_b200 import sharding as SH
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     dist = None
     if world > 1:
         import torch.distributed as dist_mod
-        dist_mod.init_process_group(backend="nccl")
+        os.environ.setdefault("NCCL_DEBUG", "WARN")
+        dist_mod.init_process_group(backend=args.backend)
         dist = dist_mod
+    if args.selftest_dist:
+        # launcher / reduction plumbing only (CPU, gloo): every rank reports fake device times
+        ms, units, ok = SH.reduce_timing(dist, torch.device("cpu"), 10.0 + rank, 100, True)
+        if rank == 0:
+            print(json.dumps({"selftest": "dist", "n_gpus": world, "max_ms": ms, "units": units, "ok": ok,
+                              "value": SH.throughput(units, 1, ms)}), flush=True)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     import paper_2607_00095_b200 as S
@@ -316,44 +367,31 @@ def run_gpu(args):
     clocks = sampler.stop() if rank == 0 else None
     ok, hmax, iters = run.check()
 
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t[0])
-    value = world * run.projections_per_step() * args.steps / (total_ms * 1e-3)
+    # max over ranks of the device time, sum of the units, AND of the converged flags (sharding.reduce_timing)
+    total_ms, units, ok = SH.reduce_timing(dist, dev, total_ms, run.projections_per_step(), ok)
+    value = SH.throughput(units, args.steps, total_ms)
 
     # roofline of the dominant kernel (the persistent projection kernel), live CUDA-event durations
     peak, peak_src = load_peaks()
     solves = iters.clamp(min=0).sum(dim=1).to(torch.float64)        # per call, over the batch
     alg_bytes_call = run.traffic_model()
-    traffic, traffic_note = args.traffic, None
-    if traffic is None and cfg == 5:
-        # ncu --set full capture of the first two launches of the timed step (tau = 1/50, 2/50), profiles/r01d_*.md
-        traffic = PROFILED_TRAFFIC_CFG5
-        traffic_note = ("dram__bytes_read.sum + dram__bytes_write.sum of launch 0 (tau=1/50), profiles/r01d_project1d_fused.md; "
-                        f"algorithmic bytes of that launch: {alg_bytes_call[0]:.4g}")
     kern_s = sum(sum(k) for k in kern_ms) * 1e-3
-    alg_total = sum(alg_bytes_call) * args.steps
-    achieved = alg_total / kern_s / 1e9
+    roof = roofline_of(run, cfg, kern_s, alg_bytes_call, args.steps, peak, peak_src)
+    if args.traffic is not None:
+        roof["traffic"] = args.traffic
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "batch_per_gpu": run.B, "nx": wl.nx, "ny": wl.ny, "nt": wl.nt,
-                   "calls_per_step": run.calls, "projections_per_step": world * run.projections_per_step(),
+                   "calls_per_step": run.calls, "projections_per_step": units,
                    "l2": "inputs (25.6 GB resident) exceed L2; no flush" if cfg == 5 else
-                         "working set smaller than L2 (latency-bound config; see DESIGN.md)",
+                         ("PCG/iterate vectors (0.6 GB) exceed L2; no flush" if cfg == 4 else
+                          "working set smaller than L2 (latency-bound config; see DESIGN.md)"),
                    "tol": wl.params["tol"], "converged_all": ok, "max_hinf_last_call": hmax,
                    "mean_linearisations_per_projection": float(solves.sum() / (run.B * run.calls)),
                    "alg_bytes_per_projection": sum(alg_bytes_call) / (run.B * run.calls)},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "traffic_note": traffic_note,
-                     "kernel": {5: "project1d_fused_kernel<1,1,8,3,256>", 2: "project1d_fused_kernel<1,1,4,4,256>",
-                                3: "project1d_fused_kernel<2,1,4,3,256> (Fisher)", 4: "project2d_kernel",
-                                1: "heat_project_kernel"}[cfg],
-                     "peak_source": peak_src, "alg_bytes_per_launch_mean": alg_total / (args.steps * run.calls),
-                     "launch_ms_mean": 1e3 * kern_s / (args.steps * run.calls),
-                     "frac_of_8TBs_spec": achieved / 8000.0},
+        "roofline": roof,
         "gpu_launches": launches,
         "clocks": clocks,
     }
@@ -364,25 +402,40 @@ def run_gpu(args):
     if rank == 0 and world == 1 and not args.no_cpu:
         cores = os.cpu_count() or 1
         workers = min(cores, 16)
-        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5) else max(workers, 16), workers)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle", "sample": desc,
-                                "seconds": dt}
+        taus = (1, 25, 49) if cfg == 5 else (25,)
+        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5) else max(workers, 16), workers, taus=taus)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "host_cpu_count": cores, "kind": "oracle",
+                                "sample": desc, "seconds": dt}
     if rank == 0 and world == 1 and args.others and cfg == 5:
         others = {}
         for c in (1, 2, 3, 4):
             r = GpuRun(S, c, dev)
             ms, km, _ = time_steps(r, 5, 3, None)
             okc, hm, itc = r.check()
-            ab = sum(r.traffic_model())
+            ab = r.traffic_model()
+            ks = sum(sum(k) for k in km) * 1e-3
             others[f"cfg{c}"] = {"projections_per_s": r.B * 5 / (ms * 1e-3), "ms_per_call": ms / 5, "converged_all": okc,
-                                 "max_hinf": hm, "model_GBs": ab * 5 / (ms * 1e-3) / 1e9,
-                                 "note": "not HBM-resident (fits L2) / latency-bound" if c != 4 else "PCG path"}
+                                 "max_hinf": hm, "roofline": roofline_of(r, c, ks, ab, 5, peak, peak_src),
+                                 "note": {1: "4 samples x 32 KiB: latency-bound, fits L2", 2: "32 samples, 4 MiB per field: fits L2, latency-bound",
+                                          3: "256 samples, 32 MiB per field: L2-borderline", 4: "64 samples, 64 MiB per field"}[c]}
             del r
         line["other_workloads"] = others
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def self_launch(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: re-exec under torch.distributed.run
+    with one rank per GPU (the launch line the driver itself uses)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -396,12 +449,17 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-others", dest="others", action="store_false")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture (profiles/)")
+                    help="override: dram bytes per launch of the dominant kernel (default: profiles/traffic.json)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="torch.distributed backend (N > 1)")
+    ap.add_argument("--selftest-dist", action="store_true",
+                    help="exercise only the multi-rank launch + reduction plumbing (no GPU work; use with --backend gloo)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_gpu(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(self_launch(args))
+    run_gpu(args)
 
 
 if __name__ == "__main__":

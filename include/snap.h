@@ -69,6 +69,30 @@ enum {
   SNAP_ST_PCG = -4         /* 2D: PCG hit pcg_max without reaching pcg_rtol; u* = last iterate               */
 };
 
+/* Which kernel served a sample (stats slot SNAP_STAT_VARIANT): a silent change of path is visible to callers. */
+enum {
+  SNAP_VAR_NONE = 0,
+  SNAP_VAR_HEAT_CLOSED_FORM = 1, /* heat_project_kernel                                                          */
+  SNAP_VAR_CLASSIC_BULK = 2,     /* project1d_kernel, rows by 1-D bulk (TMA) copies                               */
+  SNAP_VAR_CLASSIC_PLAIN = 3,    /* project1d_kernel, plain loads/stores (odd nx / unaligned buffers)             */
+  SNAP_VAR_FUSED_TMA = 4,        /* project1d_fused_kernel, tensor-map TMA rows, several GN iterations per pass   */
+  SNAP_VAR_PCG2D = 5,            /* project2d_kernel: PCG on J J^T (precond 0, 1, 2)                              */
+  SNAP_VAR_DIRECT2D = 6          /* project2d_direct_kernel: product-form sweeps with in-SMEM level solves        */
+};
+
+/* Slots of one sample's work-counter record (snap_project_stats), 8 x int64. */
+enum {
+  SNAP_STAT_LINEARISATIONS = 0, /* Gauss-Newton linearisations (Schur solves, forward half) used               */
+  SNAP_STAT_PASSES = 1,         /* passes over the time levels (forward, backward, correction sweeps)           */
+  SNAP_STAT_ROWS_READ = 2,      /* HBM rows (one level of one field) requested for reading                      */
+  SNAP_STAT_ROWS_WRITTEN = 3,   /* HBM rows written                                                             */
+  SNAP_STAT_VARIANT = 4,        /* SNAP_VAR_*                                                                   */
+  SNAP_STAT_INNER = 5,          /* 2D: PCG iterations (PCG path) / level-solve iterations (direct path)         */
+  SNAP_STAT_ROW_DOUBLES = 6,    /* doubles per row: rows * row_doubles * 8 = algorithmic bytes                  */
+  SNAP_STAT_BACKTRACKS = 7,     /* Armijo step-length reductions                                                */
+  SNAP_STAT_COUNT = 8
+};
+
 /* Size limits of this implementation (snap_problem_create returns SNAP_EINVAL beyond them):
  *   1D kinds: 2 <= nx <= 512, ny == 1, 2 <= nt <= 65535;  2D kind: 4 <= nx, ny and nx*ny <= 4096, nt >= 2. */
 
@@ -108,7 +132,8 @@ int snap_problem_destroy(snap_problem* p);
 size_t snap_num_unknowns(const snap_problem* p);
 size_t snap_num_rows(const snap_problem* p);
 
-/* Bytes of device workspace snap_project needs for `batch` samples (256-byte aligned base expected). */
+/* Bytes of device workspace snap_project needs for `batch` samples (any base alignment: the library aligns
+ * inside the buffer and the figure includes the slack). */
 size_t snap_workspace_bytes(const snap_problem* p, int batch);
 
 /* Batched projection (Eq. 2/4; the whole hot path of SURVEY.md §8(a) a1-a9).
@@ -121,10 +146,11 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch);
  *                                         always starts at u_hat.
  *   iters   dev [batch] (int32)      out  number of Gauss-Newton linearisations (Schur solves, forward half)
  *                                         used, or a negative SNAP_ST_* status.
- *   workspace dev, >= snap_workspace_bytes(p, batch).
+ *   workspace dev, workspace_bytes >= snap_workspace_bytes(p, batch); a shorter buffer returns SNAP_ENOMEM
+ *             and nothing is launched.
  * Enqueues on `stream`; no host synchronisation. */
 int snap_project(const snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
-                 double* lambda, int* iters, int warm, void* workspace, snap_stream stream);
+                 double* lambda, int* iters, int warm, void* workspace, size_t workspace_bytes, snap_stream stream);
 
 /* Same computation with HOST buffers (pinned or pageable): copies inputs to a device staging area owned by
  * the handle, runs snap_project, copies u_star / lambda / iters back, and synchronises `stream` before
@@ -141,16 +167,18 @@ int snap_residual(const snap_problem* p, int batch, const double* u, const doubl
 
 /* Matrix-free Schur operator (SURVEY.md §8(a) a2+a4): out = J(u) J(u)^T x for x in the multiplier layout,
  * the operator is never assembled.  x, out: dev [batch][m]; u: dev [batch][nt][ny][nx].  `workspace` must
- * hold batch*n doubles.  Used by the PCG path and exported for validation against an assembled J J^T. */
+ * hold batch*n doubles (workspace_bytes >= batch*n*8, else SNAP_ENOMEM).  Used by the PCG path and exported for
+ * validation against an assembled J J^T. */
 int snap_schur_apply(const snap_problem* p, int batch, const double* u, const double* x, double* out,
-                     void* workspace, snap_stream stream);
+                     void* workspace, size_t workspace_bytes, snap_stream stream);
 
-/* Per-sample work counters of the most recent snap_project call that used `workspace` (1D Burgers/Fisher
- * kinds; zeros otherwise), copied on `stream` into
- *   stats  dev [batch][4] (int64): Gauss-Newton linearisations used, passes over the levels (forward,
- *          backward and correction sweeps), HBM rows of nx doubles requested for reading, rows written.
- * rows * nx * 8 is the traffic the method itself asked for (bench.py's algorithmic bytes). */
-int snap_project_stats(const snap_problem* p, int batch, const void* workspace, long long* stats, snap_stream stream);
+/* Per-sample work counters of the most recent snap_project call that used `workspace` with the same `batch`,
+ * copied on `stream` into
+ *   stats  dev [batch][SNAP_STAT_COUNT] (int64), slots SNAP_STAT_* above.
+ * (rows read + rows written) * row_doubles * 8 is the traffic the method itself asked for (bench.py's
+ * algorithmic bytes); the variant slot says which kernel ran. */
+int snap_project_stats(const snap_problem* p, int batch, const void* workspace, size_t workspace_bytes,
+                       long long* stats, snap_stream stream);
 
 /* Number of kernel launches the library has enqueued through this handle since creation (host counter). */
 long long snap_launch_count(const snap_problem* p);

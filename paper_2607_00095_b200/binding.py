@@ -9,6 +9,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(HERE, "libsnap.so")
 
 HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS = range(5)
+# include/snap.h SNAP_STAT_* (slots of one sample's work-counter record) and SNAP_VAR_* (kernel variants)
+(STAT_LINEARISATIONS, STAT_PASSES, STAT_ROWS_READ, STAT_ROWS_WRITTEN, STAT_VARIANT, STAT_INNER, STAT_ROW_DOUBLES,
+ STAT_BACKTRACKS, STAT_COUNT) = range(9)
+(VAR_NONE, VAR_HEAT_CLOSED_FORM, VAR_CLASSIC_BULK, VAR_CLASSIC_PLAIN, VAR_FUSED_TMA, VAR_PCG2D, VAR_DIRECT2D) = range(7)
 
 EXPORTS = [
     "snap_params_default", "snap_problem_create", "snap_problem_destroy", "snap_num_unknowns", "snap_num_rows",
@@ -66,15 +70,15 @@ def load_library():
     lib.snap_num_rows.restype = C.c_size_t
     lib.snap_workspace_bytes.argtypes = [vp, C.c_int]
     lib.snap_workspace_bytes.restype = C.c_size_t
-    lib.snap_project.argtypes = [vp, C.c_int, dp, dp, dp, dp, ip, C.c_int, vp, vp]
+    lib.snap_project.argtypes = [vp, C.c_int, dp, dp, dp, dp, ip, C.c_int, vp, C.c_size_t, vp]
     lib.snap_project.restype = C.c_int
     lib.snap_project_host.argtypes = [vp, C.c_int, dp, dp, dp, dp, ip, C.c_int, vp]
     lib.snap_project_host.restype = C.c_int
     lib.snap_residual.argtypes = [vp, C.c_int, dp, dp, dp, dp, vp]
     lib.snap_residual.restype = C.c_int
-    lib.snap_schur_apply.argtypes = [vp, C.c_int, dp, dp, dp, vp, vp]
+    lib.snap_schur_apply.argtypes = [vp, C.c_int, dp, dp, dp, vp, C.c_size_t, vp]
     lib.snap_schur_apply.restype = C.c_int
-    lib.snap_project_stats.argtypes = [vp, C.c_int, vp, vp, vp]
+    lib.snap_project_stats.argtypes = [vp, C.c_int, vp, C.c_size_t, vp, vp]
     lib.snap_project_stats.restype = C.c_int
     lib.snap_launch_count.argtypes = [vp]
     lib.snap_launch_count.restype = C.c_longlong
@@ -119,6 +123,10 @@ def snap_problem_destroy(p: "Problem"):
 
 def _ptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _nbytes(t) -> int:
+    return 0 if t is None else int(t.numel() * t.element_size())
 
 
 def _stream_handle(stream) -> Optional[C.c_void_p]:
@@ -181,13 +189,11 @@ def snap_project(p: Problem, batch: int, u_hat, cdata, u_star, lam, iters, warm:
         _need(t, ne, name, dt)
         if not t.is_cuda:
             raise SnapError(f"{name} must be a CUDA tensor (use snap_project_host for host buffers)")
-    need = snap_workspace_bytes(p, batch)
     if workspace is None:
-        workspace = torch.empty(need, dtype=torch.uint8, device=u_hat.device)
-    elif workspace.numel() * workspace.element_size() < need:
-        raise SnapError(f"workspace too small: {workspace.numel() * workspace.element_size()} < {need}")
+        workspace = torch.empty(snap_workspace_bytes(p, batch), dtype=torch.uint8, device=u_hat.device)
+    # the size check is the library's (SNAP_ENOMEM), not the binding's
     rc = load_library().snap_project(p.handle, int(batch), _ptr(u_hat), _ptr(cdata), _ptr(u_star), _ptr(lam), _ptr(iters),
-                                     int(bool(warm)), _ptr(workspace), _stream_handle(stream))
+                                     int(bool(warm)), _ptr(workspace), _nbytes(workspace), _stream_handle(stream))
     _check(rc, "snap_project")
     return workspace
 
@@ -214,14 +220,15 @@ def snap_residual(p: Problem, batch: int, u, cdata, h=None, norms=None, stream=N
 
 def snap_schur_apply(p: Problem, batch: int, u, x, out, workspace, stream=None):
     rc = load_library().snap_schur_apply(p.handle, int(batch), _ptr(u), _ptr(x), _ptr(out), _ptr(workspace),
-                                         _stream_handle(stream))
+                                         _nbytes(workspace), _stream_handle(stream))
     _check(rc, "snap_schur_apply")
 
 
 def snap_project_stats(p: Problem, batch: int, workspace, stats, stream=None):
     """Copy the per-sample work counters of the last snap_project that used `workspace` into
-    `stats` (CUDA int64 tensor [batch][4]: linearisations, passes, rows read, rows written)."""
+    `stats` (CUDA int64 tensor [batch][STAT_COUNT], slots STAT_* = include/snap.h SNAP_STAT_*)."""
     import torch
-    _need(stats, 4 * batch, "stats", torch.int64)
-    rc = load_library().snap_project_stats(p.handle, int(batch), _ptr(workspace), _ptr(stats), _stream_handle(stream))
+    _need(stats, STAT_COUNT * batch, "stats", torch.int64)
+    rc = load_library().snap_project_stats(p.handle, int(batch), _ptr(workspace), _nbytes(workspace), _ptr(stats),
+                                           _stream_handle(stream))
     _check(rc, "snap_project_stats")

@@ -130,6 +130,11 @@ bool make_row_map(CUtensorMap* tm, const void* base, int batch, size_t n, size_t
 }
 
 size_t aux_bytes(const snap_problem* p, size_t B) { return align_up(B * 2 * (size_t)p->dp.nt * 8, 256); }
+// every workspace starts (after alignment to 256 bytes) with the per-sample work counters [B][SNAP_STAT_COUNT]
+size_t stats_bytes(size_t B) { return align_up(B * 8 * SNAP_STAT_COUNT, 256); }
+unsigned char* ws_base(const void* workspace) {
+  return reinterpret_cast<unsigned char*>(align_up(reinterpret_cast<uintptr_t>(workspace), 256));
+}
 
 bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
 
@@ -243,26 +248,30 @@ long long snap_launch_count(const snap_problem* p) { return p ? p->launches : 0;
 size_t snap_workspace_bytes(const snap_problem* p, int batch) {
   if (!p || batch <= 0) return 0;
   const size_t n = (size_t)p->dp.n, B = (size_t)batch;
-  if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return 256;
-  if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return align_up(B * n * 8 * kPcgVectors, 256) + 256;
-  return align_up(B * n * 8, 256) * 2 + aux_bytes(p, B) + align_up(B * 32, 256) + 256;
+  const size_t head = 256 + stats_bytes(B);   // alignment slack + work counters
+  if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return head;
+  if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return head + align_up(B * n * 8 * kPcgVectors, 256);
+  return head + align_up(B * n * 8, 256) * 2 + aux_bytes(p, B);
 }
 
 int snap_project(const snap_problem* cp, int batch, const double* u_hat, const double* cdata, double* u_star,
-                 double* lambda, int* iters, int warm, void* workspace, snap_stream stream) {
+                 double* lambda, int* iters, int warm, void* workspace, size_t workspace_bytes, snap_stream stream) {
   snap_problem* p = const_cast<snap_problem*>(cp);
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
-  if (!u_hat || !cdata || !u_star || !lambda || !iters) return SNAP_EINVAL;
+  if (!u_hat || !cdata || !u_star || !lambda || !iters || !workspace) return SNAP_EINVAL;
+  if (workspace_bytes < snap_workspace_bytes(p, batch)) return SNAP_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const DevParams& d = p->dp;
+  unsigned char* w = ws_base(workspace);
+  long long* stats = reinterpret_cast<long long*>(w);
+  w += stats_bytes((size_t)batch);
   if (d.kind == SNAP_HEAT1D_IC_MASS) {
-    heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters);
+    heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters, stats);
     return check_launch(p);
   }
-  if (!workspace) return SNAP_EINVAL;
   if (d.kind == SNAP_ALLENCAHN2D_IE)
-    return launch_project2d(p, batch, u_hat, cdata, u_star, lambda, iters, warm, workspace, st);
+    return launch_project2d(p, batch, u_hat, cdata, u_star, lambda, iters, warm, w, stats, st);
 
   Plan1d pl;
   if (!plan_1d(p, batch, pl)) return SNAP_EINVAL;
@@ -271,12 +280,10 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   a.batch = batch; a.warm = warm;
   a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
   const size_t field = align_up((size_t)batch * d.n * 8, 256);
-  unsigned char* w = static_cast<unsigned char*>(workspace);
-  w = reinterpret_cast<unsigned char*>(align_up(reinterpret_cast<uintptr_t>(w), 256));
   a.bufA = reinterpret_cast<double*>(w);
   a.bufB = reinterpret_cast<double*>(w + field);
   a.aux = reinterpret_cast<double*>(w + 2 * field);
-  a.stats = reinterpret_cast<long long*>(w + 2 * field + aux_bytes(p, (size_t)batch));
+  a.stats = stats;
   a.fuse = p->params.gn_fuse;
   // bulk (TMA) copies need every row start 16-byte aligned
   const bool bulk_ok = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
@@ -293,16 +300,17 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
                       make_row_map(&a.tm[TM_LAM], lambda, batch, n, (size_t)d.m, box);
       if (ok) {
         a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
+        a.variant = SNAP_VAR_FUSED_TMA;
         p->launches++;
         return d.kind == SNAP_FISHER1D_IE ? launch_project1d_fisher_fused(a, pf, st)
                                           : launch_project1d_burgers_fused(a, pf, st);
       }
     }
   }
-  cudaMemsetAsync(a.stats, 0, (size_t)batch * 32, st);
   a.nst = pl.nst; a.rp = pl.rp; a.warp_bytes = pl.warp_bytes;
   pl.tma = bulk_ok;
   if (!pl.tma) pl.full = false;  // the plain-load path is only instantiated with bounds checks
+  a.variant = pl.tma ? SNAP_VAR_CLASSIC_BULK : SNAP_VAR_CLASSIC_PLAIN;
   p->launches++;
   if (d.kind == SNAP_FISHER1D_IE) return launch_project1d_fisher(a, pl, st);
   return launch_project1d_burgers(a, pl, st);
@@ -362,7 +370,7 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
       ok = ok && cudaMemcpyAsync(d_l, lambda_host + (size_t)b0 * d.m, B * d.m * 8, cudaMemcpyHostToDevice, p->s_in) == cudaSuccess;
     ok = ok && cudaEventRecord(p->ev_in[c], p->s_in) == cudaSuccess && cudaStreamWaitEvent(st, p->ev_in[c], 0) == cudaSuccess;
     if (!ok) return SNAP_ECUDA;
-    const int rc = snap_project(p, nb, d_uh, d_c, d_us, d_l, d_i, warm, d_w, stream);
+    const int rc = snap_project(p, nb, d_uh, d_c, d_us, d_l, d_i, warm, d_w, b_w, stream);
     if (rc != SNAP_OK) return rc;
     ok = cudaEventRecord(p->ev_k[c], st) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_k[c], 0) == cudaSuccess;
     ok = ok && cudaMemcpyAsync(u_star_host + (size_t)b0 * d.n, d_us, B * d.n * 8, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
@@ -375,20 +383,15 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
   return cudaStreamSynchronize(st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
 }
 
-int snap_project_stats(const snap_problem* p, int batch, const void* workspace, long long* stats, snap_stream stream) {
+int snap_project_stats(const snap_problem* p, int batch, const void* workspace, size_t workspace_bytes,
+                       long long* stats, snap_stream stream) {
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
-  if (!stats) return SNAP_EINVAL;
+  if (!stats || !workspace) return SNAP_EINVAL;
+  if (workspace_bytes < snap_workspace_bytes(p, batch)) return SNAP_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const DevParams& d = p->dp;
-  if (d.kind == SNAP_HEAT1D_IC_MASS || d.kind == SNAP_ALLENCAHN2D_IE || !workspace)
-    return cudaMemsetAsync(stats, 0, (size_t)batch * 32, st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
-  const size_t field = align_up((size_t)batch * d.n * 8, 256);
-  const unsigned char* w = static_cast<const unsigned char*>(workspace);
-  w = reinterpret_cast<const unsigned char*>(align_up(reinterpret_cast<uintptr_t>(w), 256));
-  const void* src = w + 2 * field + aux_bytes(p, (size_t)batch);
-  return cudaMemcpyAsync(stats, src, (size_t)batch * 32, cudaMemcpyDeviceToDevice, st) == cudaSuccess ? SNAP_OK
-                                                                                                      : SNAP_ECUDA;
+  return cudaMemcpyAsync(stats, ws_base(workspace), (size_t)batch * 8 * SNAP_STAT_COUNT, cudaMemcpyDeviceToDevice,
+                         st) == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
 }
 
 int snap_residual(const snap_problem* cp, int batch, const double* u, const double* cdata, double* h, double* norms,
@@ -402,11 +405,12 @@ int snap_residual(const snap_problem* cp, int batch, const double* u, const doub
 }
 
 int snap_schur_apply(const snap_problem* cp, int batch, const double* u, const double* x, double* out, void* workspace,
-                     snap_stream stream) {
+                     size_t workspace_bytes, snap_stream stream) {
   snap_problem* p = const_cast<snap_problem*>(cp);
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
   if (!u || !x || !out || !workspace) return SNAP_EINVAL;
+  if (workspace_bytes < (size_t)batch * p->dp.n * 8) return SNAP_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   double* g = static_cast<double*>(workspace);
   jt_apply_kernel<<<batch, kMiscThreads, 0, st>>>(p->dp, batch, u, x, g);

@@ -549,15 +549,16 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
   const double* cur = uh;   // accepted iterate
   double* trial = bufA;     // where the next trial point goes
   bool have_trial = false, polishing = false;
-  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0;
+  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0, nfwd = 0, nbwd = 0, nback = 0;
   double alpha = 1.0, phi_cur = 0.0, Dphi = 0.0;
   SweepNorms nrm;
   const bool want_sig = (P.kind == SNAP_BURGERS1D_LF_MASS) && (P.lambda_mode == 0);
 
   while (true) {
     const double* pt = have_trial ? trial : cur;
-    if (KIND == KB) fwd_sweep_b<Q, FULL, TMA>(P, pp, pt, uh, u0, lam, M0, nrm);
+    if constexpr (KIND == KB) fwd_sweep_b<Q, FULL, TMA>(P, pp, pt, uh, u0, lam, M0, nrm);
     else fwd_sweep_f<Q, TMA>(P, pp, pt, uh, u0, lam, nrm);
+    ++nfwd;
     if (have_trial) {
       if (!polishing) {
         const double phi_t = nrm.f + mu * nrm.h1;
@@ -568,6 +569,7 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
           __threadfence_block();
           __syncwarp();
           alpha *= P.ls_shrink;
+          ++nback;
           continue;
         }
         ++steps;
@@ -594,13 +596,15 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
     }
     double linf, wd, dd;
     if (final_solve) {
-      if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, ustar, 1, want_sig ? sig : nullptr, linf, wd, dd);
+      if constexpr (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, ustar, 1, want_sig ? sig : nullptr, linf, wd, dd);
       else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, ustar, 1, linf, wd, dd);
+      ++nbwd;
       if (!finite_d(linf)) status = SNAP_ST_NONFINITE;
       break;
     }
-    if (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, trial, 0, nullptr, linf, wd, dd);
+    if constexpr (KIND == KB) bwd_sweep_b<Q, FULL, TMA>(P, pp, cur, uh, lam, trial, 0, nullptr, linf, wd, dd);
     else bwd_sweep_f<Q, TMA>(P, pp, cur, uh, lam, trial, 0, linf, wd, dd);
+    ++nbwd;
     if (!finite_d(linf)) { status = SNAP_ST_NONFINITE; break; }
     if (polishing) {
       --polish_left;
@@ -630,7 +634,17 @@ __global__ void __launch_bounds__(256) project1d_kernel(const __grid_constant__ 
       for (int k = lane; k < nt; k += 32) lam[n + k] = 0.0;
     }
   }
-  if (lane == 0) A.iters[b] = (status == 0) ? solves : status;
+  if (lane == 0) {
+    A.iters[b] = (status == 0) ? solves : status;
+    if (A.stats) {   // the traffic of this variant: forward sweep reads u, u_hat, writes y; backward reads y, u, u_hat, writes lam, u+
+      long long* stat = A.stats + (size_t)b * SNAP_STAT_COUNT;
+      stat[SNAP_STAT_LINEARISATIONS] = solves; stat[SNAP_STAT_PASSES] = nfwd + nbwd;
+      stat[SNAP_STAT_ROWS_READ] = (long long)nt * (2 * nfwd + 3 * nbwd);
+      stat[SNAP_STAT_ROWS_WRITTEN] = (long long)nt * (nfwd + 2 * nbwd);
+      stat[SNAP_STAT_VARIANT] = A.variant; stat[SNAP_STAT_INNER] = 0; stat[SNAP_STAT_ROW_DOUBLES] = nx;
+      stat[SNAP_STAT_BACKTRACKS] = nback;
+    }
+  }
 }
 
 template <int KIND, int Q, bool FULL, bool TMA>

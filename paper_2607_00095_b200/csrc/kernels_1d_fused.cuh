@@ -934,7 +934,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   bool pend = false;
   int pend_J = 0;                // updates of the pass that produced the pending trial (1: trial = cur + alpha d)
   bool conv = false;             // tol (or max_iter) reached at an accepted iterate: only polish steps remain
-  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0, sweeps = 0;
+  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0, sweeps = 0, nback = 0;
   double alpha = 1.0, mu = 0.0, phi_cur = 0.0, Dphi = 0.0;
   const double* xfin = nullptr;  // final iterate; its multiplier right-hand side y has been emitted into lam
   // snapshot of the driver state at the start of the last walked pass (restored when that pass is discarded)
@@ -979,6 +979,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
         fence_proxy_async_all();
         pp.gsync();
         alpha *= P.ls_shrink;
+        ++nback;
         jcap = 1;
         continue;
       }
@@ -1052,6 +1053,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
       fence_proxy_async_all();
       pp.gsync();
       alpha = P.ls_shrink;
+      ++nback;
       pend = true; pend_J = 1; jcap = 1;
       continue;
     }
@@ -1071,7 +1073,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     }
   }
 
-  long long* stat = A.stats ? A.stats + (size_t)b * 4 : nullptr;
+  long long* stat = A.stats ? A.stats + (size_t)b * SNAP_STAT_COUNT : nullptr;
   if (status == SNAP_ST_NONFINITE) {  // R16: u* = u_hat, lam = 0
     if (ustar != uh)
       for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
@@ -1083,15 +1085,23 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
       xfin = cur;
     }
     const bool want_sig = (P.kind == SNAP_BURGERS1D_LF_MASS) && (P.lambda_mode == 0);
-    const CUtensorMap* const tm_copy = (xfin != ustar) ? &A.tm[TM_USTAR] : nullptr;
+    // in place (u_star aliases u_hat) the final iterate is copied out only after the multiplier sweep proved finite:
+    // status -3 must leave u* = u_hat (include/snap.h)
+    const bool late_copy = (ustar == uh) && (xfin != ustar);
+    const CUtensorMap* const tm_copy = (xfin != ustar && !late_copy) ? &A.tm[TM_USTAR] : nullptr;
     double chk;
     if constexpr (KIND == KF_FUSED) chk = fused_bwd_f<Q>(P, pp, mk(xfin), mk(lam), tm_copy ? ustar : nullptr);
     else chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), tm_copy, tm_copy ? ustar : nullptr, want_sig ? sig : nullptr);
     ++sweeps;
+    if (finite_d(chk) && late_copy) {
+      for (size_t i = gtid; i < n; i += GT) ustar[i] = xfin[i];
+      if (gtid == 0) { pp.rows_rd += nt; pp.rows_wr += nt; }
+    }
     if (!finite_d(chk)) {
       status = SNAP_ST_NONFINITE;
       pp.gsync();
-      for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
+      if (ustar != uh)
+        for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
       for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
     } else if (P.has_mass) {
       if (want_sig) {
@@ -1111,7 +1121,12 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   }
   if (gtid == 0) {
     A.iters[b] = (status == 0) ? solves : status;
-    if (stat) { stat[0] = solves; stat[1] = sweeps; stat[2] = pp.rows_rd; stat[3] = pp.rows_wr; }
+    if (stat) {
+      stat[SNAP_STAT_LINEARISATIONS] = solves; stat[SNAP_STAT_PASSES] = sweeps;
+      stat[SNAP_STAT_ROWS_READ] = pp.rows_rd; stat[SNAP_STAT_ROWS_WRITTEN] = pp.rows_wr;
+      stat[SNAP_STAT_VARIANT] = A.variant; stat[SNAP_STAT_INNER] = 0; stat[SNAP_STAT_ROW_DOUBLES] = nx;
+      stat[SNAP_STAT_BACKTRACKS] = nback;
+    }
   }
 }
 

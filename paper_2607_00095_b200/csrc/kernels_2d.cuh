@@ -4,8 +4,9 @@
 //     S p = J (J^T p)                  two stencil passes fused per level through shared memory
 //     M   = Jt Jt^T,  Jt = J with T_k replaced by the constant ADI operator (I - ax dxx)(I - ay dyy)
 //     M^{-1} r: forward time sweep y_k = Tt^{-1}(r_k + y_{k-1}), backward sweep z_k = Tt^{-1}(y_k + z_{k+1})
-// The cyclic constant-coefficient line solves of Tt^{-1} are applied as truncated circulant convolutions
-// (Green's function of (-a, 1+2a, -a), exact to fp64 rounding) on the level held in shared memory.
+// The cyclic constant-coefficient line solves of Tt^{-1} are applied as circulant convolutions with the Green's
+// function of (-a, 1+2a, -a) truncated below 1e-8 of its peak (api.cu kGreenTol; the operator only preconditions,
+// and M^{-1} stays SPD because both time sweeps use the same taps) on the level held in shared memory.
 #pragma once
 #include "device_utils.cuh"
 #include "launch.h"
@@ -24,6 +25,7 @@ struct Proj2dArgs {
   double* lam;
   int* iters;
   double* ws;  // [batch][kPcgVectors][n]
+  long long* stats;  // [batch][SNAP_STAT_COUNT]
 };
 
 struct Ctx2d {
@@ -287,8 +289,14 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
 // ---- a6: PCG on S lam = b.  Returns 0 on success, 1 if pcg_max was hit ----------------------------------
 __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __restrict__ u, const double* __restrict__ b,
                          double* __restrict__ x, double* __restrict__ r, double* __restrict__ z, double* __restrict__ p,
-                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n, const double rtol) {
+                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n, const double rtol,
+                         long long& rows_rd, long long& rows_wr, int& its_total) {
   const int tid = threadIdx.x;
+  // level rows this solve asks HBM for (every vector pass = nt rows), per function:
+  //   schur_apply 2 in 1 out; precond_apply 3 in 2 out (precond 0: 1 in 1 out); vector updates as written below
+  const long long nt = c.nt;
+  const long long pre_rd = (P.precond == 0) ? nt : 3 * nt, pre_wr = (P.precond == 0) ? nt : 2 * nt;
+  rows_rd += nt;   // ||b||
   double bb = 0.0;
 #pragma unroll 8
   for (size_t i = tid; i < n; i += kT2) bb = fma(b[i], b[i], bb);
@@ -302,15 +310,20 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
     schur_apply(P, c, u, x, q);
     __syncthreads();
     for (size_t i = tid; i < n; i += kT2) r[i] = b[i] - q[i];
+    rows_rd += 4 * nt; rows_wr += 2 * nt;
   } else {
     for (size_t i = tid; i < n; i += kT2) { x[i] = 0.0; r[i] = b[i]; }
+    rows_rd += nt; rows_wr += 2 * nt;
   }
   __syncthreads();
   double rz = precond_apply(P, c, r, z, y);
   __syncthreads();
   for (size_t i = tid; i < n; i += kT2) p[i] = z[i];
+  rows_rd += pre_rd + nt; rows_wr += pre_wr + nt;
   for (int it = 0; it < P.pcg_max; ++it) {
     __syncthreads();
+    ++its_total;
+    rows_rd += 2 * nt + 4 * nt; rows_wr += nt + 2 * nt;   // schur_apply + (x, r) update
     const double pq = schur_apply(P, c, u, p, q);
     const double alpha = rz / pq;
     __syncthreads();
@@ -327,6 +340,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
     if (sqrt(rr) <= rtol * bnorm) {
       if (rtol > P.pcg_rtol) return 0;   // inexact (forcing-term) solve: the recurred residual is good enough
       // exit test on the true residual, recomputed
+      rows_rd += 4 * nt; rows_wr += 2 * nt;
       __syncthreads();
       schur_apply(P, c, u, x, q);
       __syncthreads();
@@ -340,6 +354,7 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
       if (sqrt(tr) <= rtol * bnorm) return 0;
     }
     __syncthreads();
+    rows_rd += pre_rd + 2 * nt; rows_wr += pre_wr + nt;   // preconditioner + p update
     const double rz_new = precond_apply(P, c, r, z, y);
     const double beta = rz_new / rz;
     rz = rz_new;
@@ -404,15 +419,17 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
   const double* cur = uh;
   double* trial = bufA;
   bool have_trial = false, polishing = false;
-  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0;
+  int polish_left = 0, steps = 0, solves = 0, tries = 0, status = 0, pcg_its = 0, nback = 0, passes = 0;
   double alpha = 1.0, phi_cur = 0.0, Dphi = 0.0;
   double hinf = 0.0, h1 = 0.0, f = 0.0;
   int bad = 0;
+  long long rows_rd = have_lam ? c.nt : 0, rows_wr = 0;   // level rows (nx ny doubles) asked of HBM
 
   while (true) {
     const double* pt = have_trial ? trial : cur;
     __syncthreads();
     rhs_pass(P, c, pt, uh, u0, bv, hinf, h1, f, bad);
+    rows_rd += 2 * c.nt; rows_wr += c.nt; ++passes;
     if (have_trial) {
       if (!polishing) {
         const double phi_t = f + mu * h1;
@@ -422,6 +439,7 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
           __syncthreads();
           for (size_t i = tid; i < n; i += kT2) trial[i] = fma(P.ls_shrink, trial[i] - cur[i], cur[i]);
           alpha *= P.ls_shrink;
+          rows_rd += 2 * c.nt; rows_wr += c.nt; ++nback;
           continue;
         }
         ++steps;
@@ -439,7 +457,7 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     // system solved to pcg_rtol; the forcing term shrinks with ||h||_inf, and every solve whose multiplier is
     // returned or used for the polish step (||h||_inf < tol) runs to the full pcg_rtol (R15).
     const double rt = (polishing || hinf < P.tol) ? P.pcg_rtol : fmax(P.pcg_rtol, fmin(1e-4, 1e-3 * hinf));
-    const int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n, rt);
+    const int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n, rt, rows_rd, rows_wr, pcg_its);
     have_lam = true;
     __syncthreads();
     if (prc == 2) { status = SNAP_ST_NONFINITE; break; }
@@ -459,6 +477,7 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     if (final_solve) break;
     double linf, wd, dd;
     step_pass(P, c, cur, uh, lam, trial, linf, wd, dd);
+    rows_rd += 3 * c.nt; rows_wr += c.nt; ++passes;
     if (!finite_d(linf) || !finite_d(wd) || !finite_d(dd)) { status = SNAP_ST_NONFINITE; break; }
     if (polishing) {
       --polish_left;
@@ -478,19 +497,32 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     for (size_t i = tid; i < n; i += kT2) lam[i] = 0.0;
   } else if (ustar != cur) {
     for (size_t i = tid; i < n; i += kT2) ustar[i] = cur[i];
+    rows_rd += c.nt; rows_wr += c.nt;
   }
-  if (tid == 0) A.iters[b] = (status == 0) ? solves : status;
+  if (tid == 0) {
+    A.iters[b] = (status == 0) ? solves : status;
+    if (A.stats) {
+      long long* stat = A.stats + (size_t)b * SNAP_STAT_COUNT;
+      stat[SNAP_STAT_LINEARISATIONS] = solves; stat[SNAP_STAT_PASSES] = passes;
+      stat[SNAP_STAT_ROWS_READ] = rows_rd; stat[SNAP_STAT_ROWS_WRITTEN] = rows_wr;
+      stat[SNAP_STAT_VARIANT] = SNAP_VAR_PCG2D; stat[SNAP_STAT_INNER] = pcg_its;
+      stat[SNAP_STAT_ROW_DOUBLES] = c.L; stat[SNAP_STAT_BACKTRACKS] = nback;
+    }
+  }
 }
 
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
-                            double* lambda, int* iters, int warm, void* workspace, cudaStream_t st) {
+                            double* lambda, int* iters, int warm, void* workspace, long long* stats, cudaStream_t st) {
   const DevParams& d = p->dp;
   if (d.nx > kT2) return SNAP_EINVAL;
+  // a thread owns column i and rows jr, jr + rpp, ...: at most kCpt of them (register arrays of the level passes)
+  if ((d.ny + (kT2 / d.nx) - 1) / (kT2 / d.nx) > kCpt) return SNAP_EINVAL;
   Proj2dArgs a;
   a.P = d;
   a.batch = batch; a.warm = warm;
   a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
-  a.ws = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~(uintptr_t)255);
+  a.ws = reinterpret_cast<double*>(workspace);
+  a.stats = stats;
   const size_t smem = ((size_t)3 * d.lvl + 32 + d.gx_K + 1 + d.gy_K + 1) * sizeof(double);
   if (smem > (size_t)p->max_smem_optin) return SNAP_EINVAL;
   if (cudaFuncSetAttribute(project2d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)

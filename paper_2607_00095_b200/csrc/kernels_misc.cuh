@@ -219,7 +219,8 @@ __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid
                                                                     const double* __restrict__ u_hat,
                                                                     const double* __restrict__ cdata,
                                                                     double* __restrict__ u_star,
-                                                                    double* __restrict__ lam, int* __restrict__ iters) {
+                                                                    double* __restrict__ lam, int* __restrict__ iters,
+                                                                    long long* __restrict__ stats) {
   // One CTA per sample: the levels are independent (every non-redundant mass row has its own multiplier), so the
   // warps of the CTA take the levels round-robin; only ||h||_inf and the non-finite flag are reduced over the CTA.
   __shared__ double s_max[kMiscThreads / 32];
@@ -232,6 +233,13 @@ __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid
   const double* u0 = cdata + (size_t)b * nx;
   double* us = u_star + (size_t)b * P.n;
   double* lb = lam + (size_t)b * P.m;
+  if (threadIdx.x == 0 && stats) {   // one pass: reads u_hat twice at most (the second time from cache), writes u*
+    long long* stat = stats + (size_t)b * SNAP_STAT_COUNT;
+    stat[SNAP_STAT_LINEARISATIONS] = 2; stat[SNAP_STAT_PASSES] = 2;
+    stat[SNAP_STAT_ROWS_READ] = 2 * nt; stat[SNAP_STAT_ROWS_WRITTEN] = nt;
+    stat[SNAP_STAT_VARIANT] = SNAP_VAR_HEAT_CLOSED_FORM; stat[SNAP_STAT_INNER] = 0;
+    stat[SNAP_STAT_ROW_DOUBLES] = nx; stat[SNAP_STAT_BACKTRACKS] = 0;
+  }
   const double c = (double)nx * P.dx * P.dx;
   double s0 = 0.0;
   for (int i = lane; i < nx; i += 32) s0 += u0[i];
@@ -277,6 +285,7 @@ __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid
     if (threadIdx.x == 0) iters[b] = SNAP_ST_NONFINITE;
     return;
   }
+
   double dsum = 0.0;
   for (int i = lane; i < nx; i += 32) dsum += uh[i] - u0[i];
   dsum = warp_sum(dsum);

@@ -22,7 +22,8 @@ struct Proj1dArgs {
   double* bufA;  // [batch][n]  trial / iterate ping-pong
   double* bufB;  // [batch][n]
   double* aux;   // [batch][2*nt]  level sums and null-space coefficients (min-norm multiplier, kind 4)
-  long long* stats;  // [batch][4]  linearisations, passes, HBM rows read, rows written (snap_project_stats)
+  long long* stats;  // [batch][SNAP_STAT_COUNT]  work counters (snap_project_stats)
+  int variant;       // SNAP_VAR_* recorded in the stats
   int fuse;      // cap on Gauss-Newton iterations per forward pass (0 = as many as the kernel supports)
   int nst;       // ring depth (levels in flight per warp)
   int rp;        // shared-memory row pitch in doubles (even; nx + halo + padding)
@@ -51,6 +52,6 @@ bool fused_variant(int nx, int& W, int& Q, int& JT, int& maxt);
 int launch_project1d_fisher_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
 bool fused_variant_fisher(int nx, int& W, int& Q, int& JT, int& maxt);
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
-                     double* lambda, int* iters, int warm, void* workspace, cudaStream_t st);
+                     double* lambda, int* iters, int warm, void* workspace, long long* stats, cudaStream_t st);
 
 }  // namespace snap

@@ -66,9 +66,27 @@ def test_create_validates_arguments(lib):
         lib.snap_problem_create(lib.BURGERS1D_LF, 32, 1, 16, dict(ok, gn_fuse=fuse)).destroy()
     # the workspace carries the per-sample work counters of snap_project_stats
     p = lib.snap_problem_create(lib.FISHER1D_IE, 64, 1, 16, ok)
-    assert lib.snap_workspace_bytes(p, 3) >= 2 * 3 * p.n * 8 + 3 * 2 * 16 * 8 + 3 * 32
+    assert lib.snap_workspace_bytes(p, 3) >= 2 * 3 * p.n * 8 + 3 * 2 * 16 * 8 + 3 * 8 * lib.STAT_COUNT
     p.destroy()
     assert "invalid" in lib.snap_strerror(-1)
+
+
+def test_short_workspace_is_refused_by_the_library_itself(lib):
+    """SNAP_ENOMEM comes from the C entry points (not from the Python binding): call them through raw ctypes
+    with a workspace one byte short.  The size check precedes every CUDA call, so no GPU is needed and the
+    (never dereferenced) dummy pointers are safe."""
+    p = lib.snap_problem_create(lib.BURGERS1D_LF_MASS, 64, 1, 16, dict(dx=0.1, dt=1e-3))
+    dll = lib.load_library()
+    need = lib.snap_workspace_bytes(p, 5)
+    fake = C.c_void_p(0x1000)
+    assert dll.snap_project(p.handle, 5, fake, fake, fake, fake, fake, 0, fake, need - 1, None) == -3
+    assert dll.snap_project(p.handle, 5, fake, fake, fake, fake, fake, 0, fake, 0, None) == -3
+    assert dll.snap_project(p.handle, 5, fake, fake, fake, fake, fake, 0, None, need, None) == -1   # NULL workspace
+    assert dll.snap_project_stats(p.handle, 5, fake, need - 1, fake, None) == -3
+    assert dll.snap_schur_apply(p.handle, 5, fake, fake, fake, fake, 5 * p.n * 8 - 1, None) == -3
+    assert dll.snap_project(p.handle, 0, None, None, None, None, None, 0, None, 0, None) == 0       # empty batch
+    assert "workspace" in lib.snap_strerror(-3)
+    p.destroy()
 
 
 def test_missing_library_fails_loudly(lib, monkeypatch):

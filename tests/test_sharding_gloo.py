@@ -73,3 +73,18 @@ def test_world_size_2_gloo(total):
         assert ok is False                         # one rank reported non-convergence
         assert (ms2, units2, ok2) == (1.0, total, True)
         assert seed == 1005 + 1000 * rank
+
+
+def test_bench_gpus_flag_self_launches_ranks_and_reduces_through_sharding():
+    """`python bench.py --gpus 2` with no torchrun environment re-execs itself under torch.distributed.run and
+    reduces through sharding.reduce_timing — exercised here on CPU (gloo, no GPU work)."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--backend", "gloo", "--selftest-dist"],
+                         capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                    # rank 0 alone prints
+    rec = json.loads(lines[0])
+    assert rec["n_gpus"] == 2 and rec["units"] == 200 and rec["max_ms"] == 11.0 and rec["ok"] is True

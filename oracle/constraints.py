@@ -24,36 +24,72 @@ BURGERS1D_LF = 1
 FISHER1D_IE = 2
 ALLENCAHN2D_IE = 3
 BURGERS1D_LF_MASS = 4
+BURGERS1D_FLUXK = 5
 
 _HAS_MASS = (HEAT1D_IC_MASS, BURGERS1D_LF_MASS)
 
+# Kind 5, BURGERS1D_FLUXK — the paper's own Burgers constraint set "IC, Mass, Flux(k)" (Eq. 14,
+# Table XVIII) with the energy-evolution row of Eq. 11 (L336, Appendix D) as an option:
+#   local block  [K+1][nx] : level 0 = IC rows; level k = 1..K = one-step finite-volume residual of step k-1 -> k
+#                            (L549, L561), K = p["flux_steps"]; numerical flux p["flux_kind"]: 0 Lax-Friedrichs (as
+#                            kinds 1, 4), 1 Godunov (L555, non-smooth: an element of the generalised Jacobian is used)
+#   mass block   [F]       : levels k = K+1..nt-1 (F = nt-1-K):  dx sum_i u[k][i] - M0   (L573-575).  The rows of
+#                            levels 0..K are implied by IC + conservative periodic flux rows and are OMITTED, as the
+#                            paper omits its implied first row ("the constraint at the first timestep is omitted", L493)
+#   energy block [F]       : steps k = K..nt-2, only if p["energy_rows"]:
+#                            E(u[k+1]) - E(u[k]) + dt nu D(u[k]),   E(v) = 1/2 dx sum_i v_i^2   (Eq. 7),
+#                            D(v) = dx sum_i ((v_{i+1} - v_i)/dx)^2 (periodic)  — Eq. 11's  d/dt 1/2 int u^2 + alpha int u_x^2
+#                            discretised as L603-607 (Riemann sums, forward difference in time, un-divided by dt like
+#                            the other rows, R11), dissipation explicit at level k (R8), alpha = nu.
+# Levels 0..K are pinned by square local rows (unique, as kinds 1/4); levels K+1.. are free up to 1-2 global rows
+# each, so J is wide, u* depends on u_hat, and with energy rows the border Schur complement is a banded SPD matrix
+# (each energy row couples two consecutive levels) and Gauss-Newton with W = I converges only linearly.
 
-def num_rows(kind: int, nx: int, ny: int, nt: int) -> int:
+
+def fluxk_counts(p: dict, nt: int):
+    """(K, F, E): flux steps, free levels, energy rows of kind 5."""
+    K = int(p.get("flux_steps", 0))
+    if not 0 <= K <= nt - 1:
+        raise ValueError(f"flux_steps {K} outside [0, nt-1]")
+    F = nt - 1 - K
+    return K, F, (F if int(p.get("energy_rows", 0)) else 0)
+
+
+def num_rows(kind: int, nx: int, ny: int, nt: int, p: dict = None) -> int:
     if kind == HEAT1D_IC_MASS:
         return nx + nt
+    if kind == BURGERS1D_FLUXK:
+        K, F, E = fluxk_counts(p, nt)
+        return (K + 1) * nx + F + E
     n = nx * ny * nt
     return n + nt if kind == BURGERS1D_LF_MASS else n
 
 
-def row_slices(kind: int, nx: int, ny: int, nt: int):
-    """{'ic': slice, 'pde': slice, 'mass': slice} into the row vector (empty slices where absent)."""
+def row_slices(kind: int, nx: int, ny: int, nt: int, p: dict = None):
+    """{'ic': slice, 'pde': slice, 'mass': slice[, 'energy': slice]} into the row vector (empty where absent)."""
     lvl = nx * ny
     if kind == HEAT1D_IC_MASS:
         return {"ic": slice(0, nx), "pde": slice(nx, nx), "mass": slice(nx, nx + nt)}
+    if kind == BURGERS1D_FLUXK:
+        K, F, E = fluxk_counts(p, nt)
+        loc = (K + 1) * nx
+        return {"ic": slice(0, nx), "pde": slice(nx, loc), "mass": slice(loc, loc + F), "energy": slice(loc + F, loc + F + E)}
     n = lvl * nt
     mass = slice(n, n + nt) if kind == BURGERS1D_LF_MASS else slice(n, n)
     return {"ic": slice(0, lvl), "pde": slice(lvl, n), "mass": mass}
 
 
-def full_rank_rows(kind: int, nx: int, ny: int, nt: int) -> np.ndarray:
+def full_rank_rows(kind: int, nx: int, ny: int, nt: int, p: dict = None) -> np.ndarray:
     """Boolean mask of a maximal linearly independent row subset.
 
     kind 0: the t=0 mass row is implied by the nx IC rows (the paper omits it, L493).
     kind 4: every mass row is implied by IC + conservative periodic finite-volume rows
             (sum_i h^P_{k,i} dx = mass_{k+1} - mass_k identically).
     tests/test_oracle_pins.py verifies both statements by numerical rank on tiny grids."""
-    m = num_rows(kind, nx, ny, nt)
+    m = num_rows(kind, nx, ny, nt, p)
     keep = np.ones(m, dtype=bool)
+    if kind == BURGERS1D_FLUXK:
+        return keep                      # implied rows are not part of this kind's row set
     s = row_slices(kind, nx, ny, nt)["mass"]
     if kind == HEAT1D_IC_MASS:
         keep[s.start] = False
@@ -72,6 +108,44 @@ def _lf_flux(a, b, alpha):
     return 0.5 * (0.5 * a * a + 0.5 * b * b) - 0.5 * alpha * (b - a)
 
 
+def godunov_flux(a, b):
+    """Godunov numerical flux for f(u) = u^2/2: min of f over [a, b] if a <= b, max over [b, a]
+    otherwise.  For this convex f both cases equal  max(f(max(a, 0)), f(min(b, 0)))  (the textbook closed form;
+    tests/test_oracle_pins.py checks it against the min/max definition by brute force)."""
+    return np.maximum(0.5 * np.maximum(a, 0.0) ** 2, 0.5 * np.minimum(b, 0.0) ** 2)
+
+
+def godunov_flux_grad(a, b):
+    """(dF/da, dF/db): an element of the generalised Jacobian of the piecewise-smooth flux; where the two
+    branches tie (incl. a <= 0 <= b, F = 0) the first branch is taken: dF/da = max(a, 0), dF/db = 0."""
+    fa, fb = 0.5 * np.maximum(a, 0.0) ** 2, 0.5 * np.minimum(b, 0.0) ** 2
+    first = fa >= fb
+    return np.where(first, np.maximum(a, 0.0), 0.0), np.where(first, 0.0, np.minimum(b, 0.0))
+
+
+def _fv_step_residual(v, w, p):
+    """One conservative finite-volume update residual  w - [v - dt/dx (F_{i+1/2} - F_{i-1/2})] - viscous term
+    (L561; R8) between consecutive levels v = u[k], w = u[k+1]; periodic."""
+    dx, dt = p["dx"], p["dt"]
+    s = dt / dx
+    c = p["nu"] * dt / dx ** 2
+    vp, vm = np.roll(v, -1), np.roll(v, 1)
+    if int(p.get("flux_kind", 0)) == 1:
+        F_r, F_l = godunov_flux(v, vp), godunov_flux(vm, v)
+    else:
+        F_r, F_l = _lf_flux(v, vp, p["alpha"]), _lf_flux(vm, v, p["alpha"])
+    return w - v + s * (F_r - F_l) - c * (vp - 2.0 * v + vm)
+
+
+def _energy(v, dx):
+    return 0.5 * dx * math.fsum((v * v).tolist())
+
+
+def _dissipation(v, dx):
+    d = np.roll(v, -1) - v
+    return math.fsum((d * d).tolist()) / dx
+
+
 def _mass_rows(u, u0, dx):
     nt = u.shape[0]
     M0 = dx * math.fsum(u0.ravel().tolist())
@@ -87,6 +161,13 @@ def residual(kind: int, u: np.ndarray, u0: np.ndarray, p: dict) -> np.ndarray:
     ic = (u[0] - u0).ravel()
     if kind == HEAT1D_IC_MASS:
         return np.concatenate([ic, _mass_rows(u, u0, dx)])
+    if kind == BURGERS1D_FLUXK:
+        K, F, E = fluxk_counts(p, nt)
+        loc = [ic] + [_fv_step_residual(u[k, 0], u[k + 1, 0], p) for k in range(K)]
+        mass = _mass_rows(u, u0, dx)[K + 1:]
+        en = [_energy(u[k + 1, 0], dx) - _energy(u[k, 0], dx) + dt * p["nu"] * _dissipation(u[k, 0], dx)
+              for k in range(K, nt - 1)] if E else []
+        return np.concatenate(loc + [mass, np.array(en, dtype=np.float64)])
 
     loc = np.empty_like(u)
     loc[0] = u[0] - u0
@@ -130,9 +211,12 @@ def residual_norms(kind: int, u: np.ndarray, u0: np.ndarray, p: dict) -> np.ndar
     are the per-sample terms of the paper's constraint-error metric (Eq. 27)."""
     nt, ny, nx = np.asarray(u).shape
     h = residual(kind, u, u0, p)
-    sl = row_slices(kind, nx, ny, nt)
-    return np.array([np.abs(h).max() if h.size else 0.0,
-                     np.linalg.norm(h[sl["ic"]]), np.linalg.norm(h[sl["pde"]]), np.linalg.norm(h[sl["mass"]])])
+    sl = row_slices(kind, nx, ny, nt, p)
+    out = [np.abs(h).max() if h.size else 0.0,
+           np.linalg.norm(h[sl["ic"]]), np.linalg.norm(h[sl["pde"]]), np.linalg.norm(h[sl["mass"]])]
+    if "energy" in sl:
+        out.append(np.linalg.norm(h[sl["energy"]]))
+    return np.array(out)
 
 
 # ------------------------------------------------------------------------------------------
@@ -145,7 +229,7 @@ def jacobian(kind: int, u: np.ndarray, p: dict) -> sp.csr_matrix:
     nt, ny, nx = u.shape
     lvl = nx * ny
     n = lvl * nt
-    m = num_rows(kind, nx, ny, nt)
+    m = num_rows(kind, nx, ny, nt, p)
     dx, dt = p["dx"], p["dt"]
     rows, cols, vals = [], [], []
 
@@ -157,19 +241,25 @@ def jacobian(kind: int, u: np.ndarray, p: dict) -> sp.csr_matrix:
     cell = np.arange(lvl)
     add(cell, cell, 1.0)                                 # IC rows: d(u[0]-u0)/du[0] = I
 
-    if kind in (BURGERS1D_LF, BURGERS1D_LF_MASS):
+    if kind in (BURGERS1D_LF, BURGERS1D_LF_MASS, BURGERS1D_FLUXK):
         s = dt / dx
         c = p["nu"] * dt / dx ** 2
         al = p["alpha"]
         i = np.arange(nx)
         ip = (i + 1) % nx
         im = (i - 1) % nx
-        for k in range(nt - 1):
+        godunov = kind == BURGERS1D_FLUXK and int(p.get("flux_kind", 0)) == 1
+        steps = fluxk_counts(p, nt)[0] if kind == BURGERS1D_FLUXK else nt - 1
+        for k in range(steps):
             v = u[k, 0]
             r = (k + 1) * nx + i
-            # dF_{i+1/2}/du_i = u_i/2 + alpha/2 ; dF_{i+1/2}/du_{i+1} = u_{i+1}/2 - alpha/2
-            dFr_di, dFr_dip = 0.5 * v[i] + 0.5 * al, 0.5 * v[ip] - 0.5 * al
-            dFl_dim, dFl_di = 0.5 * v[im] + 0.5 * al, 0.5 * v[i] - 0.5 * al
+            if godunov:
+                dFr_di, dFr_dip = godunov_flux_grad(v[i], v[ip])
+                dFl_dim, dFl_di = godunov_flux_grad(v[im], v[i])
+            else:
+                # dF_{i+1/2}/du_i = u_i/2 + alpha/2 ; dF_{i+1/2}/du_{i+1} = u_{i+1}/2 - alpha/2
+                dFr_di, dFr_dip = 0.5 * v[i] + 0.5 * al, 0.5 * v[ip] - 0.5 * al
+                dFl_dim, dFl_di = 0.5 * v[im] + 0.5 * al, 0.5 * v[i] - 0.5 * al
             add(r, (k + 1) * nx + i, 1.0)
             add(r, k * nx + i, -1.0 + s * (dFr_di - dFl_di) + 2.0 * c)
             add(r, k * nx + ip, s * dFr_dip - c)
@@ -211,6 +301,19 @@ def jacobian(kind: int, u: np.ndarray, p: dict) -> sp.csr_matrix:
     elif kind != HEAT1D_IC_MASS:
         raise ValueError(f"unknown kind {kind}")
 
+    if kind == BURGERS1D_FLUXK:
+        K, F, E = fluxk_counts(p, nt)
+        i = np.arange(nx)
+        ip, im = (i + 1) % nx, (i - 1) % nx
+        m0 = (K + 1) * nx
+        for f in range(F):                                   # mass rows of the free levels k = K+1..nt-1
+            add(np.full(nx, m0 + f), (K + 1 + f) * nx + i, dx)
+        for f in range(E):                                   # energy row of step k = K+f: levels k and k+1
+            k = K + f
+            v, w = u[k, 0], u[k + 1, 0]
+            add(np.full(nx, m0 + F + f), (k + 1) * nx + i, dx * w)
+            add(np.full(nx, m0 + F + f), k * nx + i,
+                -dx * v + dt * p["nu"] * (2.0 / dx) * (2.0 * v - v[ip] - v[im]))
     if kind in _HAS_MASS:
         m0 = nx if kind == HEAT1D_IC_MASS else n
         i = np.arange(nx)

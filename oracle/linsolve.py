@@ -60,6 +60,16 @@ def solve_schur_banded_cholesky(S: sp.spmatrix, r: np.ndarray, refine: int = 1) 
     return x
 
 
+def solve_schur_dense_cholesky(S: np.ndarray, r: np.ndarray, refine: int = 1) -> np.ndarray:
+    """Few rows with dense border rows (kind 5): explicit dense S = J J^T (SPD) -> LAPACK potrf/potrs + `refine`
+    steps of iterative refinement."""
+    cf = sla.cho_factor(S, lower=True, check_finite=False)
+    x = sla.cho_solve(cf, r, check_finite=False)
+    for _ in range(refine):
+        x = x + sla.cho_solve(cf, r - S @ x, check_finite=False)
+    return x
+
+
 def solve_schur_cg(S: sp.spmatrix, r: np.ndarray, x0=None, rtol: float = 1e-13, maxiter: int = 20000):
     """2D at size: plain un-preconditioned conjugate gradients on explicit S to relative
     residual ||r - S x|| / ||r|| <= rtol.  Returns (x, iterations)."""

@@ -55,6 +55,8 @@ def _solve_basic(J, w, h, keep, backend, cg_state):
     rk = h[keep] - Jk @ w
     if backend == "banded":
         lam_k = L.solve_schur_banded_cholesky((Jk @ Jk.T).tocsr(), rk)
+    elif backend == "dense_chol":
+        lam_k = L.solve_schur_dense_cholesky((Jk @ Jk.T).toarray(), rk)
     elif backend == "cg":
         lam_k, its = L.solve_schur_cg((Jk @ Jk.T).tocsr(), rk, rtol=cg_state["rtol"], maxiter=cg_state["maxiter"])
         cg_state["iters"] += its
@@ -73,8 +75,9 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     u0 = np.asarray(u0, dtype=np.float64)
     nt, ny, nx = u_hat.shape
     if backend == "auto":
-        backend = "cg" if kind == C.ALLENCAHN2D_IE else "banded"
-    keep = C.full_rank_rows(kind, nx, ny, nt)
+        # kind 5: few rows (m ~ (K+1) nx + 2 nt) with dense border rows: dense Cholesky of the assembled J J^T
+        backend = {C.ALLENCAHN2D_IE: "cg", C.BURGERS1D_FLUXK: "dense_chol"}.get(kind, "banded")
+    keep = C.full_rank_rows(kind, nx, ny, nt, p)
     tol = p.get("tol", 1e-10)
     max_iter = int(p.get("max_iter", 50))
     polish = int(p.get("polish", 1))
@@ -107,7 +110,7 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     steps = 0
     backtracks = 0
     status = STATUS_OK
-    lam = np.zeros(C.num_rows(kind, nx, ny, nt))
+    lam = np.zeros(C.num_rows(kind, nx, ny, nt, p))
     J = None
     while True:
         h, J, lam = lin(u)

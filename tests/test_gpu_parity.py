@@ -18,6 +18,10 @@ pytestmark = pytest.mark.gpu
 
 TOL_U, TOL_L = 1e-9, 1e-8
 ABS_L_FEASIBLE = 1e-12      # |lam| where lam* = 0 exactly (SURVEY.md §8(c) "Parity metric")
+# The one case that needs more: cfg 5 at 256 x 256, tau = 1, maximum over all 1024 samples.  There
+# lam = J^-T J^-1 h(u_true) with h(u_true) pure rounding (|h| <= 1.5 ulp(1.46) = 3.3e-16) and ||J^-1||_2 = 177
+# (SURVEY.md P-5): |lam| <= 177^2 * 3.3e-16 = 1.0e-11.  Observed on the B200: 1.6e-12 (oracle, one sample: 1.1e-13).
+ABS_L_FEASIBLE_CFG5_FULL = 1e-11
 TOL_KKT = 1e-11
 
 
@@ -226,7 +230,7 @@ def test_project_parity_cfg5_full_size_tau_sequence(S):
             assert torch.equal(us.view_as(uh), uh)
             amax = float(lam.abs().max())
             print(f"cfg5 tau=1 sample {b}: rel_u {ru:.1e} max|lam| over the batch {amax:.1e} (oracle {np.abs(o['lam']).max():.1e})")
-            assert ru <= TOL_U and amax <= ABS_L_FEASIBLE and np.abs(o["lam"]).max() <= ABS_L_FEASIBLE
+            assert ru <= TOL_U and amax <= ABS_L_FEASIBLE_CFG5_FULL and np.abs(o["lam"]).max() <= ABS_L_FEASIBLE_CFG5_FULL
         else:
             rl = rel_lam(gl, o["lam"])
             print(f"cfg5 tau={j}/50 sample {b}: rel_u {ru:.1e} rel_lam {rl:.1e} iters {np.bincount(it.cpu().numpy())}")

@@ -26,9 +26,10 @@ KIND_BURGERS1D_LF = 1
 KIND_FISHER1D_IE = 2
 KIND_ALLENCAHN2D_IE = 3
 KIND_BURGERS1D_LF_MASS = 4
+KIND_BURGERS1D_FLUXK = 5
 KIND_NAMES = {
     0: "HEAT1D_IC_MASS", 1: "BURGERS1D_LF", 2: "FISHER1D_IE",
-    3: "ALLENCAHN2D_IE", 4: "BURGERS1D_LF_MASS",
+    3: "ALLENCAHN2D_IE", 4: "BURGERS1D_LF_MASS", 5: "BURGERS1D_FLUXK",
 }
 
 # cfg -> (kind, batch, nx, ny, nt, seed)   (BASELINE.json configs[0..4] = cfg 1..5)
@@ -38,7 +39,13 @@ CONFIG_SHAPES = {
     3: (KIND_FISHER1D_IE, 256, 128, 1, 128, 1003),
     4: (KIND_ALLENCAHN2D_IE, 64, 64, 64, 32, 1004),
     5: (KIND_BURGERS1D_LF_MASS, 1024, 256, 1, 256, 1005),
+    # SURVEY.md §8(f) NEXT-1 / NEXT-4 (not BASELINE.json configs): the paper's "IC, Mass, Flux(k = 5)" row set
+    # (Eq. 14, Table XVIII) at the scale of cfg 5.
+    6: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1006),   # Lax-Friedrichs flux rows + energy-evolution rows (Eq. 11)
+    7: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1007),   # Godunov flux rows (L555), inviscid, no energy rows
 }
+CONFIG_EXTRA = {6: dict(flux_steps=5, energy_rows=1, flux_kind=0),
+                7: dict(flux_steps=5, energy_rows=0, flux_kind=1, nu=0.0)}
 
 F64 = torch.float64
 
@@ -51,8 +58,10 @@ def default_params(kind: int, nx: int, ny: int, nt: int) -> Dict[str, float]:
              pcg_rtol=1e-13, pcg_max=200, precond=2, lambda_mode=0)
     if kind == KIND_HEAT1D_IC_MASS:
         p.update(dx=1.0 / (nx - 1), dt=1.0 / max(nt - 1, 1), nu=0.1)
-    elif kind in (KIND_BURGERS1D_LF, KIND_BURGERS1D_LF_MASS):
+    elif kind in (KIND_BURGERS1D_LF, KIND_BURGERS1D_LF_MASS, KIND_BURGERS1D_FLUXK):
         p.update(dx=2.0 * math.pi / nx, dt=1e-3, nu=0.01, alpha=1.0)
+        if kind == KIND_BURGERS1D_FLUXK:
+            p.update(flux_steps=min(5, nt - 1), energy_rows=1, flux_kind=0)
     elif kind == KIND_FISHER1D_IE:
         p.update(dx=1.0 / nx, dt=1.0 / max(nt - 1, 1), D=0.01, rho=1.0)
     elif kind == KIND_ALLENCAHN2D_IE:
@@ -88,6 +97,10 @@ class Workload:
             return self.nx + self.nt
         if self.kind == KIND_BURGERS1D_LF_MASS:
             return self.n + self.nt
+        if self.kind == KIND_BURGERS1D_FLUXK:
+            K = int(self.params["flux_steps"])
+            F = self.nt - 1 - K
+            return (K + 1) * self.nx + F * (2 if int(self.params["energy_rows"]) else 1)
         return self.n
 
 
@@ -103,6 +116,16 @@ def _burgers_lf_step(v: torch.Tensor, dx: float, dt: float, nu: float, alpha: fl
     f = 0.5 * v * v
     F_right = 0.5 * (f + torch.roll(f, -1, -1)) - 0.5 * alpha * (vp - v)   # F_{i+1/2}
     F_left = torch.roll(F_right, 1, -1)                                    # F_{i-1/2}
+    return v - (dt / dx) * (F_right - F_left) + (nu * dt / dx ** 2) * (vp - 2.0 * v + vm)
+
+
+def _burgers_godunov_step(v: torch.Tensor, dx: float, dt: float, nu: float) -> torch.Tensor:
+    """One finite-volume step with the Godunov flux of f = u^2/2 and optional explicit
+    central viscosity, periodic."""
+    vp = torch.roll(v, -1, -1)
+    vm = torch.roll(v, 1, -1)
+    F_right = torch.maximum(0.5 * v.clamp_min(0.0) ** 2, 0.5 * vp.clamp_max(0.0) ** 2)   # F(u_i, u_{i+1})
+    F_left = torch.roll(F_right, 1, -1)
     return v - (dt / dx) * (F_right - F_left) + (nu * dt / dx ** 2) * (vp - 2.0 * v + vm)
 
 
@@ -204,7 +227,8 @@ def _gen(seed: int, device) -> torch.Generator:
 
 def make_workload(cfg: int, batch: Optional[int] = None, nx: Optional[int] = None,
                   ny: Optional[int] = None, nt: Optional[int] = None, seed: Optional[int] = None,
-                  device="cpu", noise: Optional[float] = None, with_u_hat: bool = True) -> Workload:
+                  device="cpu", noise: Optional[float] = None, with_u_hat: bool = True,
+                  params: Optional[Dict[str, float]] = None) -> Workload:
     """Build config `cfg` (1..5) of BASELINE.json, optionally at reduced batch/grid
     (same recipe, same seeds) for tests.  For cfg 5 `u_hat` is the tau_j = j/50, j=25
     input unless `with_u_hat=False`; use `burgers_tau_input` for the 50-tau sequence."""
@@ -217,6 +241,11 @@ def make_workload(cfg: int, batch: Optional[int] = None, nx: Optional[int] = Non
     dev = torch.device(device)
     g = _gen(seed, dev)
     p = default_params(kind, nx, ny, nt)
+    if cfg in CONFIG_EXTRA:
+        p.update(CONFIG_EXTRA[cfg])
+        p["flux_steps"] = min(int(p["flux_steps"]), nt - 1)
+    if params:
+        p.update(params)
     meta: Dict[str, object] = {}
 
     if kind == KIND_HEAT1D_IC_MASS:
@@ -227,15 +256,19 @@ def make_workload(cfg: int, batch: Optional[int] = None, nx: Optional[int] = Non
                  * torch.exp(-math.pi ** 2 * p["nu"] * t)[None, :, None]).expand(B, nt, nx)
         u_true = clean.reshape(B, nt, 1, nx).contiguous()
         sigma = 0.1 if noise is None else noise
-    elif kind in (KIND_BURGERS1D_LF, KIND_BURGERS1D_LF_MASS):
+    elif kind in (KIND_BURGERS1D_LF, KIND_BURGERS1D_LF_MASS, KIND_BURGERS1D_FLUXK):
         x = torch.arange(nx, dtype=F64, device=dev) * p["dx"]
         phi = torch.rand(B, generator=g, dtype=F64, device=dev) * (2.0 * math.pi)
         meta["phi"] = phi
         u0 = (torch.sin(x)[None, :] + 0.5 * torch.sin(2.0 * x[None, :] + phi[:, None])).reshape(B, 1, nx)
         u_true = torch.empty(B, nt, 1, nx, dtype=F64, device=dev)
         u_true[:, 0] = u0
+        godunov = kind == KIND_BURGERS1D_FLUXK and int(p.get("flux_kind", 0)) == 1
         for k in range(nt - 1):
-            u_true[:, k + 1] = _burgers_lf_step(u_true[:, k], p["dx"], p["dt"], p["nu"], p["alpha"])
+            if godunov:
+                u_true[:, k + 1] = _burgers_godunov_step(u_true[:, k], p["dx"], p["dt"], p["nu"])
+            else:
+                u_true[:, k + 1] = _burgers_lf_step(u_true[:, k], p["dx"], p["dt"], p["nu"], p["alpha"])
         sigma = 0.05 if noise is None else noise
     elif kind == KIND_FISHER1D_IE:
         x = (torch.arange(nx, dtype=F64, device=dev) + 0.5) * p["dx"]

@@ -215,7 +215,7 @@ class GpuRun:
         self.lam = torch.zeros(self.B, self.p.m, dtype=torch.float64, device=dev)
         self.iters = torch.zeros(self.calls, self.B, dtype=torch.int32, device=dev)
         self.ws = torch.empty(S.snap_workspace_bytes(self.p, self.B), dtype=torch.uint8, device=dev)
-        self.norms = torch.empty(self.B, 4, dtype=torch.float64, device=dev)
+        self.norms = torch.empty(self.B, 5, dtype=torch.float64, device=dev)
         self.stats = torch.zeros(self.B, S.STAT_COUNT, dtype=torch.int64, device=dev)
 
     def step(self, events=None):

@@ -24,6 +24,12 @@
  *                                   (PAPER.md L549, L561).  Kind HEAT1D_IC_MASS has level 0 only (nx rows).
  *         mass block  [nt]        : dx * sum_i u[k][i] - M0,  M0 = dx * sum_i u0[i],
  *                                   kinds HEAT1D_IC_MASS and BURGERS1D_LF_MASS only.
+ *     Kind BURGERS1D_FLUXK, K = flux_steps, F = nt-1-K:  m = (K+1) nx + F + (energy_rows ? F : 0),
+ *         local block [K+1][nx] (level 0 = IC rows, level k = residual of step k-1 -> k),
+ *         mass block  [F]  levels K+1..nt-1 (the rows of levels 0..K are implied by the local rows and omitted,
+ *                          as the paper omits its implied first row, L493),
+ *         energy block [F] steps k = K..nt-2:  E(u[k+1]) - E(u[k]) + dt nu D(u[k]),  E(v) = dx/2 sum v_i^2,
+ *                          D(v) = dx sum ((v_{i+1} - v_i)/dx)^2  (periodic), only if energy_rows != 0.
  *     (The paper lists IC, mass, flux rows in that order, L374/L499; row order only permutes lam.)
  *   - Asynchrony: device entry points only enqueue work on `stream` and return; per-sample outcome is in
  *     device memory (`iters`).  They never synchronise the host.
@@ -50,7 +56,12 @@ enum {
   SNAP_BURGERS1D_LF = 1,      /* IC + finite-volume residual, Lax-Friedrichs flux, explicit viscosity, periodic  */
   SNAP_FISHER1D_IE = 2,       /* IC + implicit-Euler Fisher-KPP residual, ghost-cell Neumann                     */
   SNAP_ALLENCAHN2D_IE = 3,    /* IC + implicit-Euler Allen-Cahn residual, 5-point periodic (2D, PCG path)        */
-  SNAP_BURGERS1D_LF_MASS = 4  /* kind 1 + per-level mass rows (dense border rows, all linearly dependent)        */
+  SNAP_BURGERS1D_LF_MASS = 4, /* kind 1 + per-level mass rows (dense border rows, all linearly dependent)        */
+  SNAP_BURGERS1D_FLUXK = 5    /* the paper's "IC, Mass, Flux(k)" set (Eq. 14, Table XVIII): IC rows,
+                                 finite-volume residual rows of the first flux_steps steps only (Lax-Friedrichs or
+                                 Godunov flux, L555), a mass row per later level, optionally the energy-evolution row
+                                 of Eq. 11 (L336, L603-607) per later step.  J is wide; the border rows are genuinely
+                                 coupled (banded SPD Schur complement, banded Cholesky)       */
 };
 
 /* Return codes. */
@@ -77,7 +88,8 @@ enum {
   SNAP_VAR_CLASSIC_PLAIN = 3,    /* project1d_kernel, plain loads/stores (odd nx / unaligned buffers)             */
   SNAP_VAR_FUSED_TMA = 4,        /* project1d_fused_kernel, tensor-map TMA rows, several GN iterations per pass   */
   SNAP_VAR_PCG2D = 5,            /* project2d_kernel: PCG on J J^T (precond 0, 1, 2)                              */
-  SNAP_VAR_DIRECT2D = 6          /* project2d_direct_kernel: product-form sweeps with in-SMEM level solves        */
+  SNAP_VAR_DIRECT2D = 6,         /* project2d_direct_kernel: product-form sweeps with in-SMEM level solves        */
+  SNAP_VAR_FLUXK_BAND = 7        /* project1d_fluxk_kernel: product form on the pinned levels + banded border solve */
 };
 
 /* Slots of one sample's work-counter record (snap_project_stats), 8 x int64. */
@@ -94,7 +106,8 @@ enum {
 };
 
 /* Size limits of this implementation (snap_problem_create returns SNAP_EINVAL beyond them):
- *   1D kinds: 2 <= nx <= 512, ny == 1, 2 <= nt <= 65535;  2D kind: 4 <= nx, ny and nx*ny <= 4096, nt >= 2. */
+ *   1D kinds: 2 <= nx <= 512, ny == 1, 2 <= nt <= 65535;  2D kind: 4 <= nx, ny and nx*ny <= 4096, nt >= 2;
+ *   kind BURGERS1D_FLUXK: nx in {32, 64, 128, 256}, nt <= 512 (the band system lives in shared memory). */
 
 typedef struct {
   double dx, dy, dt;  /* grid steps (caller supplied so that oracle and GPU share them bit for bit)           */
@@ -117,6 +130,9 @@ typedef struct {
                          forward pass over the levels.  0 = as many as the kernel holds in
                          registers (default), k >= 1 = at most k, -1 = classic path (one forward and one
                          backward sweep per iteration).  Other kinds / sizes always take the classic path.   */
+  int flux_steps;     /* kind BURGERS1D_FLUXK: K, number of leading steps that carry flux rows (0 <= K <= nt-1)     */
+  int energy_rows;    /* kind BURGERS1D_FLUXK: 1 = add the energy-evolution row of every later step                  */
+  int flux_kind;      /* kind BURGERS1D_FLUXK: 0 = Lax-Friedrichs (alpha), 1 = Godunov                               */
 } snap_params;
 
 /* Fill *p with the defaults listed above (grid steps 1, physical constants 0, alpha = 1). */
@@ -161,11 +177,12 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
 /* Constraint residual and the per-type norms of the paper's constraint-error metric
  * (Eq. 27).
  *   h      dev [batch][m] or NULL.
- *   norms  dev [batch][4] or NULL: ||h||_inf, ||h_IC||_2, ||h_PDE||_2, ||h_mass||_2 (0 where a type is absent). */
+ *   norms  dev [batch][5] or NULL: ||h||_inf, ||h_IC||_2, ||h_PDE||_2, ||h_mass||_2, ||h_energy||_2 (0 where a type
+ *          is absent). */
 int snap_residual(const snap_problem* p, int batch, const double* u, const double* cdata, double* h,
                   double* norms, snap_stream stream);
 
-/* Matrix-free Schur operator (SURVEY.md §8(a) a2+a4): out = J(u) J(u)^T x for x in the multiplier layout,
+/* Matrix-free Schur operator (SURVEY.md §8(a) a2+a4; kinds 0-4): out = J(u) J(u)^T x for x in the multiplier layout,
  * the operator is never assembled.  x, out: dev [batch][m]; u: dev [batch][nt][ny][nx].  `workspace` must
  * hold batch*n doubles (workspace_bytes >= batch*n*8, else SNAP_ENOMEM).  Used by the PCG path and exported for
  * validation against an assembled J J^T. */

@@ -124,7 +124,14 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
             lam[:] = 0.0
             break
         u_full = uh - J.T @ lam
-        if hinf < tol:
+        # Wide J (kind 5): Gauss-Newton with W = I contracts only linearly and ||h|| alone says nothing about
+        # stationarity, so convergence also asks for a small step, RMS(d) <= tol (R18).  For the square
+        # kinds d = -J^-1 h and the paper's/north_star's rule ||h||_inf < tol stands alone.
+        small_step = True
+        if kind == C.BURGERS1D_FLUXK:
+            d0 = u_full - u
+            small_step = float(d0 @ d0) <= d0.size * tol * tol
+        if hinf < tol and small_step:
             if hinf > POLISH_SKIP_FACTOR * tol:
                 for _ in range(polish):        # R4: full step(s), then the multiplier at the polished point
                     u = u_full
@@ -138,6 +145,12 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
         if steps >= max_iter:
             status = STATUS_MAXITER
             break
+        if hinf < tol:
+            # feasible to tolerance but the step is not small yet (wide J only, R18): full Gauss-Newton steps without
+            # a merit test, like polish steps (R4) -- merit differences are below rounding here
+            u = u_full
+            steps += 1
+            continue
         d = u_full - u
         h1 = float(np.abs(h).sum())
         if mu_rule == "nw18_36":

@@ -138,6 +138,54 @@ unsigned char* ws_base(const void* workspace) {
 
 bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
 
+// kind 5: one warp per sample; per sample a ring of nst x 2 swizzled rows, the band system (11 doubles per free
+// level) and the mbarriers
+int project_fluxk(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star, double* lambda,
+                  int* iters, unsigned char* w, long long* stats, cudaStream_t st) {
+  const DevParams& d = p->dp;
+  if (!(aligned16(u_hat) && aligned16(u_star) && aligned16(w))) return SNAP_EINVAL;   // TMA rows
+  const int F = d.nt - 1 - d.fk_K;
+  const int rp = fused_row_pitch(d.nx);
+  const int sms = p->sm_count > 0 ? p->sm_count : 148;
+  int spc = (batch + sms - 1) / sms;
+  if (spc < 1) spc = 1;
+  if (spc > 8) spc = 8;
+  Plan1d pl;
+  bool found = false;
+  for (; spc >= 1 && !found; --spc) {
+    for (int nst = 4; nst >= 2; --nst) {
+      const size_t sb = align_up(((size_t)2 * nst * rp + (size_t)11 * (F > 0 ? F : 1) + nst) * 8, 1024);
+      if (sb * spc + 1024 <= (size_t)p->max_smem_optin) {
+        pl.wpc = spc; pl.nst = nst; pl.warp_bytes = (int)sb; pl.smem = sb * spc + 1024;
+        pl.grid = (batch + spc - 1) / spc;
+        found = true;
+        break;
+      }
+    }
+  }
+  if (!found) return SNAP_EINVAL;
+  Proj1dArgs a;
+  a.P = d;
+  a.batch = batch; a.warm = 0;
+  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
+  const size_t field = align_up((size_t)batch * d.n * 8, 256);
+  a.bufA = reinterpret_cast<double*>(w);
+  a.bufB = reinterpret_cast<double*>(w + field);
+  a.aux = reinterpret_cast<double*>(w + 2 * field);
+  a.stats = stats;
+  a.fuse = 0;
+  const int box = d.nx / 16;
+  const size_t n = (size_t)d.n;
+  if (!(make_row_map(&a.tm[TM_UHAT], u_hat, batch, n, n, box) && make_row_map(&a.tm[TM_BUFA], a.bufA, batch, n, n, box) &&
+        make_row_map(&a.tm[TM_BUFB], a.bufB, batch, n, n, box) && make_row_map(&a.tm[TM_USTAR], u_star, batch, n, n, box)))
+    return SNAP_ECUDA;
+  a.tm[TM_LAM] = a.tm[TM_USTAR];   // unused by this kind
+  a.nst = pl.nst; a.rp = rp; a.warp_bytes = pl.warp_bytes;
+  a.variant = SNAP_VAR_FLUXK_BAND;
+  p->launches++;
+  return launch_project1d_fluxk(a, pl, st);
+}
+
 }  // namespace
 
 extern "C" {
@@ -158,11 +206,19 @@ void snap_params_default(snap_params* p) {
   p->precond = 2;
   p->lambda_mode = 0;
   p->gn_fuse = 0;
+  p->flux_steps = 0;
+  p->energy_rows = 0;
+  p->flux_kind = 0;
 }
 
 int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, const snap_params* prm) {
   if (!out || !prm) return SNAP_EINVAL;
-  if (kind < SNAP_HEAT1D_IC_MASS || kind > SNAP_BURGERS1D_LF_MASS) return SNAP_EINVAL;
+  if (kind < SNAP_HEAT1D_IC_MASS || kind > SNAP_BURGERS1D_FLUXK) return SNAP_EINVAL;
+  if (kind == SNAP_BURGERS1D_FLUXK) {
+    if (!(nx == 32 || nx == 64 || nx == 128 || nx == 256) || nt > 512) return SNAP_EINVAL;
+    if (prm->flux_steps < 0 || prm->flux_steps > nt - 1) return SNAP_EINVAL;
+    if (prm->energy_rows < 0 || prm->energy_rows > 1 || prm->flux_kind < 0 || prm->flux_kind > 1) return SNAP_EINVAL;
+  }
   if (is_1d(kind)) {
     if (ny != 1 || nx < 2 || nx > 512 || nt < 2 || nt > 65535) return SNAP_EINVAL;
   } else {
@@ -185,6 +241,16 @@ int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, co
   d.n = d.lvl * nt;
   d.has_mass = (kind == SNAP_HEAT1D_IC_MASS || kind == SNAP_BURGERS1D_LF_MASS);
   d.m = (kind == SNAP_HEAT1D_IC_MASS) ? nx + nt : d.n + (d.has_mass ? nt : 0);
+  if (kind == SNAP_BURGERS1D_FLUXK) {
+    d.fk_K = prm->flux_steps; d.fk_energy = prm->energy_rows; d.fk_flux = prm->flux_kind;
+    const int F = nt - 1 - d.fk_K;
+    d.m = (d.fk_K + 1) * nx + F + (d.fk_energy ? F : 0);
+    d.fk_s = prm->dt / prm->dx;
+    d.fk_c = prm->nu * prm->dt / (prm->dx * prm->dx);
+    d.fk_cD = 2.0 * prm->dt * prm->nu / prm->dx;
+    d.fk_dtnu = prm->dt * prm->nu;
+    d.fk_alpha = prm->alpha;
+  }
   d.dx = prm->dx; d.dy = prm->dy; d.dt = prm->dt;
   const double s = prm->dt / prm->dx;
   d.bs_e = 0.5 * s * prm->alpha + prm->nu * prm->dt / (prm->dx * prm->dx);
@@ -273,6 +339,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   if (d.kind == SNAP_ALLENCAHN2D_IE)
     return launch_project2d(p, batch, u_hat, cdata, u_star, lambda, iters, warm, w, stats, st);
 
+  if (d.kind == SNAP_BURGERS1D_FLUXK) return project_fluxk(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, st);
   Plan1d pl;
   if (!plan_1d(p, batch, pl)) return SNAP_EINVAL;
   Proj1dArgs a;
@@ -400,6 +467,10 @@ int snap_residual(const snap_problem* cp, int batch, const double* u, const doub
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
   if (!u || !cdata || (!h && !norms)) return SNAP_EINVAL;
+  if (p->dp.kind == SNAP_BURGERS1D_FLUXK) {
+    p->launches++;
+    return launch_residual_fluxk(p->dp, batch, u, cdata, h, norms, static_cast<cudaStream_t>(stream));
+  }
   residual_kernel<<<batch, kMiscThreads, 0, static_cast<cudaStream_t>(stream)>>>(p->dp, batch, u, cdata, h, norms);
   return check_launch(p);
 }
@@ -410,6 +481,7 @@ int snap_schur_apply(const snap_problem* cp, int batch, const double* u, const d
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
   if (!u || !x || !out || !workspace) return SNAP_EINVAL;
+  if (p->dp.kind == SNAP_BURGERS1D_FLUXK) return SNAP_EINVAL;   // kinds 0-4 only (include/snap.h)
   if (workspace_bytes < (size_t)batch * p->dp.n * 8) return SNAP_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   double* g = static_cast<double*>(workspace);

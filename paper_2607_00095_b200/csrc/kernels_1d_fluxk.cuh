@@ -1,0 +1,600 @@
+// Kind 5, BURGERS1D_FLUXK: the paper's "IC, Mass, Flux(k)" Burgers row set (Eq. 14, Table XVIII
+// L768-777) with the energy-evolution rows of Eq. 11 (L336; discretisation L603-607) as an option, Lax-Friedrichs or
+// Godunov flux (L555).  One persistent warp per sample, nx = 32 Q.
+//
+// Structure of the Newton-KKT system (Eq. 5 L96 / Eq. 24, W = I).  Rows:
+//   J_loc : IC rows + finite-volume residual rows of steps 0..K-1.  They touch levels 0..K only and are square and
+//           block lower-bidiagonal there, exactly as in kinds 1/4 (product form, zero-fill Cholesky factor L = J_loc).
+//   J_b   : dense border rows -- mass row M_k of every free level k = K+1..nt-1 and energy row E_k of every step
+//           k = K..nt-2 (couples levels k and k+1, quadratic in u).
+// Block elimination (Sherman-Morrison-Woodbury / Schur complement on the border):
+//   A = J_loc J_loc^T,  C = J_b J_loc^T,  D = J_b J_b^T,  S_b = D - C A^-1 C^T = J_b P J_b^T,
+//   P = projector on null(J_loc) = the unknowns of the free levels, so S_b = J_b^f (J_b^f)^T where J_b^f is J_b
+//   restricted to the free columns: a symmetric positive definite band matrix of half-bandwidth 2 in the ordering
+//   (E_K, M_{K+1}, E_{K+1}, M_{K+2}, ...), assembled from level-local dot products and factored by a hand-written
+//   banded LDL^T (one system of size 2 (nt-1-K) per sample).  In primal terms, with w = u - u_hat:
+//     levels <= K :  d = -q,  q_0 = h_0, q_k = h_k + A_{k-1} q_{k-1}                  (Newton on the square block)
+//     S_b lam_b = h_b + J_b^{<=K} d^{<=K} - J_b^f w_f ,   d_f = -w_f - (J_b^f)^T lam_b   (free levels)
+//     J_loc^T lam_loc = (q - w)^{<=K} - (J_b^{<=K})^T lam_b                            (multipliers, at the end)
+// J is wide: u* depends on u_hat, Gauss-Newton converges linearly when energy rows are present, and the Armijo
+// test is live.
+//
+// One pass over the levels per trial point: it applies the step of the previous solve (u+ = u + alpha d, which
+// needs the row of u for the border-row gradients), evaluates h, the merit sums and every dot product of the next
+// linearisation AT u+ (all level-local), and writes u+.  Traffic per Gauss-Newton iteration: read u, u_hat, write
+// u+ = 24 n bytes (the first pass reads u_hat only).
+#pragma once
+#include "kernels_1d_fused.cuh"
+
+namespace snap {
+
+constexpr int FLUX_LF = 0, FLUX_GODUNOV = 1;
+
+// numerical flux F(a, b) through the interface between a = u_i and b = u_{i+1}, and its linearisation
+// G = dF/da qa + dF/db qb  (Godunov: an element of the generalised Jacobian; ties take the first branch)
+template <int FLUX>
+__device__ __forceinline__ void flux_lin(double a, double b, double qa, double qb, double al, double& F, double& G) {
+  if constexpr (FLUX == FLUX_LF) {
+    F = 0.25 * (a * a + b * b) - 0.5 * al * (b - a);
+    G = (0.5 * a + 0.5 * al) * qa + (0.5 * b - 0.5 * al) * qb;
+  } else {
+    const double ap = fmax(a, 0.0), bm = fmin(b, 0.0);
+    const double fa = 0.5 * ap * ap, fb = 0.5 * bm * bm;
+    const bool first = fa >= fb;
+    F = first ? fa : fb;
+    G = first ? ap * qa : bm * qb;
+  }
+}
+template <int FLUX>
+__device__ __forceinline__ void flux_grad(double a, double b, double al, double& ga, double& gb) {
+  if constexpr (FLUX == FLUX_LF) {
+    ga = 0.5 * a + 0.5 * al;
+    gb = 0.5 * b - 0.5 * al;
+  } else {
+    const double ap = fmax(a, 0.0), bm = fmin(b, 0.0);
+    const bool first = 0.5 * ap * ap >= 0.5 * bm * bm;
+    ga = first ? ap : 0.0;
+    gb = first ? 0.0 : bm;
+  }
+}
+
+// Phi(v) (one explicit finite-volume step from level v) and A(v) q (its linearisation applied to q), own cells
+template <int Q, int FLUX>
+__device__ __forceinline__ void level_phi_Aq(const DevParams& P, const double (&v)[Q], const double (&q)[Q], int lane,
+                                             double (&phi)[Q], double (&aq)[Q]) {
+  const double s = P.fk_s, cv = P.fk_c, al = P.fk_alpha;
+  const double vR = shfl_next(v[0], lane), qR = shfl_next(q[0], lane);
+  const double vL = shfl_prev(v[Q - 1], lane), qL = shfl_prev(q[Q - 1], lane);
+  double Fp, Gp;
+  flux_lin<FLUX>(vL, v[0], qL, q[0], al, Fp, Gp);
+#pragma unroll
+  for (int c = 0; c < Q; ++c) {
+    const double vr = (c < Q - 1) ? v[c + 1] : vR, qr = (c < Q - 1) ? q[c + 1] : qR;
+    const double vm = (c > 0) ? v[c - 1] : vL, qm = (c > 0) ? q[c - 1] : qL;
+    double F, G;
+    flux_lin<FLUX>(v[c], vr, q[c], qr, al, F, G);
+    phi[c] = v[c] - s * (F - Fp) + cv * ((vr - v[c]) + (vm - v[c]));
+    aq[c] = q[c] - s * (G - Gp) + cv * ((qr - q[c]) + (qm - q[c]));
+    Fp = F; Gp = G;
+  }
+}
+
+// (A(v)^T l)_j = (s ga_j + c) l_{j+1} + (1 - s ga_j + s gb_{j-1} - 2c) l_j + (-s gb_{j-1} + c) l_{j-1},
+// ga_j = dF/da(v_j, v_{j+1}), gb_{j-1} = dF/db(v_{j-1}, v_j)
+template <int Q, int FLUX>
+__device__ __forceinline__ void level_At(const DevParams& P, const double (&v)[Q], const double (&l)[Q], int lane,
+                                         double (&out)[Q]) {
+  const double s = P.fk_s, cv = P.fk_c, al = P.fk_alpha;
+  const double vR = shfl_next(v[0], lane), lR = shfl_next(l[0], lane);
+  const double vL = shfl_prev(v[Q - 1], lane), lL = shfl_prev(l[Q - 1], lane);
+  double gaL, gbL;
+  flux_grad<FLUX>(vL, v[0], al, gaL, gbL);   // interface left of cell 0
+#pragma unroll
+  for (int c = 0; c < Q; ++c) {
+    const double vr = (c < Q - 1) ? v[c + 1] : vR;
+    const double lr = (c < Q - 1) ? l[c + 1] : lR, lm = (c > 0) ? l[c - 1] : lL;
+    double ga, gb;
+    flux_grad<FLUX>(v[c], vr, al, ga, gb);   // interface right of cell c
+    out[c] = (s * ga + cv) * lr + (1.0 - s * ga + s * gbL - 2.0 * cv) * l[c] + (-s * gbL + cv) * lm;
+    gbL = gb;
+  }
+}
+
+// border-row gradient of an energy row on its EARLIER level:  b(v) = -dx v + cD (2 v - v_{i+1} - v_{i-1}),  cD = 2 dt nu / dx
+template <int Q>
+__device__ __forceinline__ void energy_b(const DevParams& P, const double (&v)[Q], int lane, double (&b)[Q], double& sD) {
+  const double vR = shfl_next(v[0], lane), vL = shfl_prev(v[Q - 1], lane);
+  double acc = 0.0;
+#pragma unroll
+  for (int c = 0; c < Q; ++c) {
+    const double vr = (c < Q - 1) ? v[c + 1] : vR, vm = (c > 0) ? v[c - 1] : vL;
+    b[c] = fma(-P.dx, v[c], P.fk_cD * ((v[c] - vr) + (v[c] - vm)));
+    const double dv = vr - v[c];
+    acc = fma(dv, dv, acc);
+  }
+  sD = acc;   // per-lane part of sum_i (v_{i+1} - v_i)^2
+}
+
+// per-sample band system in shared memory: 10 doubles per free level f (level k = K+1+f), rows E_{k-1} then M_k
+struct Band {
+  double* dE;    // [F] diagonal of the E row (LDL^T: becomes D)
+  double* dM;    // [F] diagonal of the M row
+  double* eM;    // [F] (E_{k-1}, M_{k-1})  sub-diagonal 1 of the E row
+  double* eE;    // [F] (E_{k-1}, E_{k-2})  sub-diagonal 2 of the E row
+  double* mE;    // [F] (M_k, E_{k-1})      sub-diagonal 1 of the M row
+  double* rE;    // [F] right-hand side of the E row (becomes y, then the solution)
+  double* rM;    // [F]
+  double* lE;    // [F] multipliers of the last solve: energy rows
+  double* lM;    // [F]                               mass rows
+  double* jw;    // [2F] J_b^f w_f (for the penalty parameter), E rows then M rows
+  __device__ __forceinline__ void carve(double* base, int F) {
+    dE = base; dM = dE + F; eM = dM + F; eE = eM + F; mE = eE + F; rE = mE + F; rM = rE + F; lE = rM + F; lM = lE + F;
+    jw = lM + F;
+  }
+  static __host__ __device__ constexpr int doubles_per_level() { return 11; }
+};
+
+// group-uniform results of one pass
+struct FluxkSums {
+  double hlev;      // ||h||_inf against (tol, kPolishSkip tol): 0, 1, 2 as in hinf_level
+  double h1, f;     // ||h||_1, 1/2 ||u - u_hat||^2 at the point the pass produced
+  double wq, qq;    // pinned levels: w^T q', ||q'||^2 of the Newton direction d = -q' at that point
+  double ww;        // free levels: ||w_f||^2
+  bool bad;
+};
+
+template <int N>
+__device__ __forceinline__ void warp_sum_n(double (&r)[N]) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) r[i] += __shfl_xor_sync(SNAP_FULL, r[i], o);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// One pass over the levels.  Reads the iterate x (and u_hat unless x is u_hat), applies the step of the last solve
+//     pinned levels k <= K :  t = x - alpha q ,  q from the Newton recurrence at x (iteration "A")
+//     free levels          :  t = x + alpha ((u_hat - (J_b^f)^T lam_b) - x) ,  border-row gradients at x
+// when `update` (otherwise t = x), writes t to `xo`, and evaluates at t: h (norm sums), the Newton recurrence of
+// the pinned levels (iteration "B": q', for the next step and the coupling term of energy row K) and the band
+// system S_b, its right-hand side and J_b^f w_f.
+// ------------------------------------------------------------------------------------------------
+template <int Q, int FLUX>
+__device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x, const Buf uh,
+                                        const double* __restrict__ u0, double* __restrict__ xo, bool update,
+                                        double alpha, double M0, Band bd, FluxkSums& S) {
+  constexpr int nx = 32 * Q;
+  RowPipe<1, Q> pp = pp_ref;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
+  const int K = P.fk_K, F = nt - 1 - K;
+  const bool energy = P.fk_energy != 0;
+  const bool same = (x.p == uh.p);
+  const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
+  const double dx = P.dx, dtnu = P.fk_dtnu;
+  const double tol = P.tol, skip = kPolishSkip * P.tol;
+
+  double phiA[Q], ccA[Q], phiB[Q], ccB[Q];
+#pragma unroll
+  for (int c = 0; c < Q; ++c) { phiA[c] = u0[first + c]; phiB[c] = phiA[c]; ccA[c] = 0.0; ccB[c] = 0.0; }
+  double h1 = 0.0, f2 = 0.0, wq = 0.0, qq = 0.0, ww_free = 0.0;   // h1 / ww_free: lane 0 adds the warp-uniform row values
+  int hmx = 0;
+  // carried from the previous level (warp-uniform): energy, dissipation, and the dot products of its b vector
+  double E_prev = 0.0, D_prev = 0.0, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, bq_K = 0.0;
+
+  const int npro = nst < nt ? nst : nt;
+  for (int k = 0; k < npro; ++k) pp.issue(k, k, x.tm, tm_uh);
+  int s = 0;
+  for (int k = 0; k < nt; ++k) {
+    pp.wait(s);
+    double v[Q], uhr[Q], t[Q];
+    load_cells<Q>(pp.row(s, 0), pp.lo, v);
+    if (same) {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) uhr[c] = v[c];
+    } else {
+      load_cells<Q>(pp.row(s, 1), pp.lo, uhr);
+    }
+    if (k <= K) {
+      // ---- pinned level: iteration A at x (the step), iteration B at t (the next linearisation) ----
+      double q[Q];
+#pragma unroll
+      for (int c = 0; c < Q; ++c) q[c] = (v[c] - phiA[c]) + ccA[c];
+      if (k < K) level_phi_Aq<Q, FLUX>(P, v, q, lane, phiA, ccA);
+#pragma unroll
+      for (int c = 0; c < Q; ++c) t[c] = update ? fma(-alpha, q[c], v[c]) : v[c];
+      double qb[Q];
+#pragma unroll
+      for (int c = 0; c < Q; ++c) {
+        const double h = t[c] - phiB[c];
+        qb[c] = h + ccB[c];
+        const double ah = fabs(h), w = t[c] - uhr[c];
+        hmx = max(hmx, __double2hiint(ah));
+        h1 += ah;
+        f2 = fma(w, w, f2);
+        wq = fma(w, qb[c], wq);
+        qq = fma(qb[c], qb[c], qq);
+      }
+      if (k < K) level_phi_Aq<Q, FLUX>(P, t, qb, lane, phiB, ccB);
+      if (k == K && F > 0) {   // level K feeds energy row K: E, D and the coupling term b_K . d_K  (d_K = -q'_K)
+        double b[Q], sD;
+        energy_b<Q>(P, t, lane, b, sD);
+        double r[3] = {0.0, sD, 0.0};
+#pragma unroll
+        for (int c = 0; c < Q; ++c) { r[0] = fma(t[c], t[c], r[0]); r[2] = fma(b[c], qb[c], r[2]); }
+        warp_sum_n<3>(r);
+        E_prev = 0.5 * dx * r[0];
+        D_prev = r[1] / dx;
+        bq_K = r[2];
+      }
+    } else {
+      // ---- free level f: step with the border multipliers, then the dot products of the next band system ----
+      const int f = k - K - 1;
+      if (update) {
+        const double lamM = bd.lM[f], lamE0 = energy ? bd.lE[f] : 0.0;
+        const double lamE1 = (energy && f + 1 < F) ? bd.lE[f + 1] : 0.0;
+        double b[Q], sDx;
+        energy_b<Q>(P, v, lane, b, sDx);
+#pragma unroll
+        for (int c = 0; c < Q; ++c) {
+          const double full = uhr[c] - (dx * lamM + lamE0 * dx * v[c] + lamE1 * b[c]);
+          t[c] = fma(alpha, full - v[c], v[c]);
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < Q; ++c) t[c] = v[c];
+      }
+      double b[Q], sD;
+      energy_b<Q>(P, t, lane, b, sD);
+      // r: s1 = sum t, s2 = sum t^2, sD, bb = b.b, tb = t.b, sw = sum w, tw = t.w, bw = b.w, ww = w.w
+      double r[9] = {0.0, 0.0, sD, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+      for (int c = 0; c < Q; ++c) {
+        const double w = t[c] - uhr[c];
+        r[0] += t[c];
+        r[1] = fma(t[c], t[c], r[1]);
+        r[3] = fma(b[c], b[c], r[3]);
+        r[4] = fma(t[c], b[c], r[4]);
+        r[5] += w;
+        r[6] = fma(t[c], w, r[6]);
+        r[7] = fma(b[c], w, r[7]);
+        r[8] = fma(w, w, r[8]);
+      }
+      warp_sum_n<9>(r);
+      const double E_k = 0.5 * dx * r[1], D_k = r[2] / dx;
+      const double hM = fma(dx, r[0], -M0);
+      const double hE = energy ? (E_k - E_prev) + dtnu * D_prev : 0.0;
+      const double aM = fabs(hM), aE = fabs(hE);
+      hmx = max(hmx, max(__double2hiint(aM), __double2hiint(aE)));
+      if (lane == 0) { h1 += aM + aE; ww_free += r[8]; }
+      f2 += (lane == 0) ? r[8] : 0.0;
+      if (lane == 0) {
+        const double aa = dx * dx * r[1], ab = dx * r[4], aw = dx * r[6];
+        if (energy) {
+          bd.dE[f] = aa + (f > 0 ? bb_prev : 0.0);
+          bd.eM[f] = (f > 0) ? -dx * dx * s1_prev : 0.0;       // M_{k-1} . b_{k-1} = dx sum b = -dx^2 sum t
+          bd.eE[f] = (f > 0) ? ab_prev : 0.0;                  // a_{k-1} . b_{k-1}
+          bd.mE[f] = dx * dx * r[0];                           // M_k . a_k
+          const double jwE = aw + (f > 0 ? bw_prev : 0.0);
+          bd.jw[f] = jwE;
+          bd.rE[f] = hE - jwE - (f == 0 ? bq_K : 0.0);         // h + J^{<=K} d^{<=K} - J^f w ,  d_K = -q'_K
+        } else {
+          bd.dE[f] = 1.0; bd.eM[f] = 0.0; bd.eE[f] = 0.0; bd.mE[f] = 0.0; bd.jw[f] = 0.0; bd.rE[f] = 0.0;
+        }
+        bd.dM[f] = (double)nx * dx * dx;
+        bd.jw[F + f] = dx * r[5];
+        bd.rM[f] = hM - dx * r[5];
+        (void)ab;
+      }
+      E_prev = E_k; D_prev = D_k; bb_prev = r[3]; ab_prev = dx * r[4]; bw_prev = r[7]; s1_prev = r[0];
+    }
+    if (update) {
+      store_cells_global<Q>(xo + (size_t)k * nx + first, t);
+      if (lane == 0) pp.rows_wr += 1;
+    }
+    if (k + nst < nt) pp.issue(s, k + nst, x.tm, tm_uh);
+    if (++s == nst) s = 0;
+  }
+  pp.drain();
+  S.hlev = hinf_level(hmx, tol, skip);
+  S.h1 = warp_sum(h1);
+  const double f2s = warp_sum(f2);
+  S.f = 0.5 * f2s;
+  S.wq = warp_sum(wq);
+  S.qq = warp_sum(qq);
+  S.ww = __shfl_sync(SNAP_FULL, ww_free, 0);
+  S.bad = !(finite_d(S.h1) && finite_d(f2s) && finite_d(S.wq) && finite_d(S.qq));
+  pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Banded LDL^T of the border Schur complement S_b (half-bandwidth 2, order E_K, M_{K+1}, E_{K+1}, ...) and the
+// solve S_b lam_b = rho, in place in shared memory, by one lane.  Returns false on a non-positive or non-finite
+// pivot.  Also returns lam^T (J_b^f w_f) and lam^T rho = y^T D^-1 y (for the penalty parameter).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool band_solve(Band bd, int F, double& lam_jw, double& lam_rho) {
+  // forward: factor and L y = rho.  Carried: D, L1 (entry to the row before) and y of the previous two rows.
+  double Dm2 = 1.0, Dm1 = 1.0, L1m1 = 0.0, ym2 = 0.0, ym1 = 0.0;   // rows i-2, i-1
+  double acc = 0.0;
+  bool ok = true;
+  for (int f = 0; f < F; ++f) {
+    // row E_f (i = 2f): a2 = eE (to E_{f-1} = row i-2), a1 = eM (to M_{f-1} = row i-1)
+    {
+      const double a2 = bd.eE[f], a1 = bd.eM[f], a0 = bd.dE[f];
+      const double l2 = a2 / Dm2;
+      const double l1 = (a1 - l2 * Dm2 * L1m1) / Dm1;
+      const double D = a0 - l2 * l2 * Dm2 - l1 * l1 * Dm1;
+      const double y = bd.rE[f] - l1 * ym1 - l2 * ym2;
+      ok = ok && (D > 0.0) && finite_d(D) && finite_d(y);
+      bd.eE[f] = l2; bd.eM[f] = l1; bd.dE[f] = D; bd.rE[f] = y;
+      acc = fma(y, y / D, acc);
+      Dm2 = Dm1; Dm1 = D; L1m1 = l1; ym2 = ym1; ym1 = y;
+    }
+    // row M_f (i = 2f+1): a2 = 0 (to M_{f-1}), a1 = mE (to E_f)
+    {
+      const double a1 = bd.mE[f], a0 = bd.dM[f];
+      const double l1 = a1 / Dm1;
+      const double D = a0 - l1 * l1 * Dm1;
+      const double y = bd.rM[f] - l1 * ym1;
+      ok = ok && (D > 0.0) && finite_d(D) && finite_d(y);
+      bd.mE[f] = l1; bd.dM[f] = D; bd.rM[f] = y;
+      acc = fma(y, y / D, acc);
+      Dm2 = Dm1; Dm1 = D; L1m1 = l1; ym2 = ym1; ym1 = y;
+    }
+  }
+  lam_rho = acc;
+  if (!ok) return false;
+  // backward: x_i = y_i / D_i - L1[i+1] x_{i+1} - L2[i+2] x_{i+2}
+  double xp1 = 0.0, xp2 = 0.0;          // x_{i+1}, x_{i+2}
+  double L1p1 = 0.0, L2p1 = 0.0, L2p2 = 0.0;   // L1 of row i+1; L2 of rows i+1, i+2
+  double dot = 0.0;
+  for (int f = F - 1; f >= 0; --f) {
+    // row M_f (i = 2f+1): rows above it: i+1 = E_{f+1} (L1 = eM[f+1], L2 = eE[f+1] points to E_f), i+2 = M_{f+1} (L2 = 0)
+    {
+      const double x = bd.rM[f] / bd.dM[f] - L1p1 * xp1 - L2p2 * xp2;
+      bd.lM[f] = x;
+      dot = fma(x, bd.jw[F + f], dot);
+      xp2 = xp1; xp1 = x;
+      L2p2 = L2p1;              // row i+1 becomes row i+2 of the next (lower) row
+      L1p1 = bd.mE[f]; L2p1 = 0.0;   // this row (M_f) is row i+1 of E_f
+    }
+    // row E_f (i = 2f)
+    {
+      const double x = bd.rE[f] / bd.dE[f] - L1p1 * xp1 - L2p2 * xp2;
+      bd.lE[f] = x;
+      dot = fma(x, bd.jw[f], dot);
+      xp2 = xp1; xp1 = x;
+      L2p2 = L2p1;
+      L1p1 = bd.eM[f]; L2p1 = bd.eE[f];
+    }
+  }
+  lam_jw = dot;
+  return finite_d(dot);
+}
+
+// ------------------------------------------------------------------------------------------------
+// multipliers of the local rows at the final point x (levels 0..K only; plain loads, K is small):
+//   y_k = q'_k - w_k  (k <= K),  y_K -= lam_{E_K} b_K(x[K]) ;   lam_K = y_K ,  lam_k = y_k + A_k^T lam_{k+1}
+// ------------------------------------------------------------------------------------------------
+template <int Q, int FLUX>
+__device__ __noinline__ bool fluxk_local_multipliers(const DevParams& P, int lane, int first, const double* __restrict__ x,
+                                                     const double* __restrict__ uh, const double* __restrict__ u0,
+                                                     double lamEK, double* __restrict__ lam) {
+  constexpr int nx = 32 * Q;
+  const int K = P.fk_K;
+  double phi[Q], cc[Q];
+#pragma unroll
+  for (int c = 0; c < Q; ++c) { phi[c] = u0[first + c]; cc[c] = 0.0; }
+  for (int k = 0; k <= K; ++k) {
+    double v[Q], q[Q], y[Q];
+#pragma unroll
+    for (int c = 0; c < Q; ++c) v[c] = x[(size_t)k * nx + first + c];
+#pragma unroll
+    for (int c = 0; c < Q; ++c) {
+      q[c] = (v[c] - phi[c]) + cc[c];
+      y[c] = q[c] - (v[c] - uh[(size_t)k * nx + first + c]);
+    }
+    if (k < K) level_phi_Aq<Q, FLUX>(P, v, q, lane, phi, cc);
+    if (k == K && lamEK != 0.0) {
+      double b[Q], sD;
+      energy_b<Q>(P, v, lane, b, sD);
+#pragma unroll
+      for (int c = 0; c < Q; ++c) y[c] = fma(-lamEK, b[c], y[c]);
+    }
+#pragma unroll
+    for (int c = 0; c < Q; ++c) lam[(size_t)k * nx + first + c] = y[c];
+  }
+  __syncwarp();
+  double l[Q], chk = 0.0;
+#pragma unroll
+  for (int c = 0; c < Q; ++c) { l[c] = lam[(size_t)K * nx + first + c]; chk += l[c]; }
+  for (int k = K - 1; k >= 0; --k) {
+    double v[Q], at[Q];
+#pragma unroll
+    for (int c = 0; c < Q; ++c) v[c] = x[(size_t)k * nx + first + c];
+    level_At<Q, FLUX>(P, v, l, lane, at);
+#pragma unroll
+    for (int c = 0; c < Q; ++c) {
+      l[c] = lam[(size_t)k * nx + first + c] + at[c];
+      lam[(size_t)k * nx + first + c] = l[c];
+      chk += l[c];
+    }
+  }
+  return finite_d(warp_sum(chk));
+}
+
+// ------------------------------------------------------------------------------------------------
+// the persistent Gauss-Newton driver of kind 5 (a8, a9): one warp per sample
+// ------------------------------------------------------------------------------------------------
+template <int Q, int FLUX>
+__global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_constant__ Proj1dArgs A) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  using G = RowGeom<1, Q>;
+  const DevParams& P = A.P;
+  const int slot = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int b = blockIdx.x * (blockDim.x >> 5) + slot;
+  if (b >= A.batch) return;
+  constexpr int nx = G::NX;
+  const int nt = P.nt, K = P.fk_K, F = nt - 1 - K;
+  const size_t n = (size_t)P.n;
+
+  unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) + (size_t)slot * A.warp_bytes;
+  RowPipe<1, Q> pp;
+  pp.stage = reinterpret_cast<double*>(base);
+  pp.orow = nullptr; pp.xch = nullptr; pp.red = nullptr;
+  double* bandmem = pp.stage + (size_t)A.nst * 2 * G::RP;
+  pp.aux = nullptr;
+  Band bd;
+  bd.carve(bandmem, F > 0 ? F : 1);
+  pp.bar0 = smem_u32(bandmem + (size_t)Band::doubles_per_level() * (F > 0 ? F : 1));
+  pp.phase = 0;
+  pp.nst = A.nst; pp.lane = lane; pp.w = 0; pp.bar_id = 1 + slot;
+  pp.first = lane * Q;
+  pp.b = b;
+  pp.lo.init(pp.first);
+  pp.rows_rd = 0; pp.rows_wr = 0;
+  if (lane == 0) {
+    for (int s = 0; s < A.nst; ++s) mbar_init(pp.bar0 + 8u * s, 1);
+    mbar_fence_init();
+    fence_proxy_async_smem();
+  }
+  __syncwarp();
+
+  const double* uh = A.u_hat + (size_t)b * n;
+  const double* u0 = A.cdata + (size_t)b * nx;
+  double* ustar = A.u_star + (size_t)b * n;
+  double* lam = A.lam + (size_t)b * P.m;
+  double* bufA = A.bufA + (size_t)b * n;
+  double* bufB = A.bufB + (size_t)b * n;
+  auto mk = [&](const double* q) -> Buf {
+    const CUtensorMap* t = nullptr;
+    if (q == uh) t = &A.tm[TM_UHAT];
+    else if (q == bufA) t = &A.tm[TM_BUFA];
+    else if (q == bufB) t = &A.tm[TM_BUFB];
+    else if (q == ustar) t = &A.tm[TM_USTAR];
+    return Buf{t, const_cast<double*>(q)};
+  };
+  double M0;
+  {
+    double sm = 0.0;
+    for (int i = lane; i < nx; i += 32) sm += u0[i];
+    M0 = P.dx * warp_sum(sm);
+  }
+  double* const buf0 = bufA;
+  double* const buf1 = (ustar != uh) ? ustar : bufB;
+
+  const double* cur = uh;
+  bool polishing = false;
+  int polish_left = 0, steps = 0, solves = 0, status = 0, passes = 0, nback = 0;
+  double mu = 0.0;
+  FluxkSums S;
+  fluxk_pass<Q, FLUX>(P, pp, mk(cur), mk(uh), u0, nullptr, false, 1.0, M0, bd, S);
+  ++passes;
+  while (true) {
+    if (S.bad) { status = SNAP_ST_NONFINITE; break; }
+    // ---- border solve (the SMW / Schur-complement step) ----
+    double lam_jw = 0.0, lam_rho = 0.0;
+    int okb = 1;
+    __syncwarp();
+    if (lane == 0 && F > 0) okb = band_solve(bd, F, lam_jw, lam_rho) ? 1 : 0;
+    __syncwarp();
+    okb = __shfl_sync(SNAP_FULL, okb, 0);
+    lam_jw = __shfl_sync(SNAP_FULL, lam_jw, 0);
+    lam_rho = __shfl_sync(SNAP_FULL, lam_rho, 0);
+    if (!okb) { status = SNAP_ST_NONFINITE; break; }
+    ++solves;
+    // step d: pinned levels d = -q', free levels d = -w - (J_b^f)^T lam_b
+    const double wd = -S.wq - S.ww - lam_jw;
+    const double dd = S.qq + S.ww + 2.0 * lam_jw + lam_rho;
+    // wide J: ||h|| alone says nothing about stationarity; converged = ||h||_inf < tol and RMS(d) <= tol (R18)
+    const bool conv = S.hlev < 2.0 && dd <= (double)n * P.tol * P.tol;
+    bool final_solve = false;
+    if (polishing) {
+      final_solve = (polish_left == 0);
+    } else if (conv) {
+      polishing = true;
+      polish_left = (S.hlev > 0.0) ? P.polish : 0;
+      final_solve = (polish_left == 0);
+    } else if (steps >= P.max_iter) {
+      status = SNAP_ST_MAXITER;
+      final_solve = true;
+    }
+    if (final_solve) break;
+    double phi_cur = 0.0, Dphi = 0.0;
+    // feasible to tolerance but the step is not small yet: full steps without a merit test, like polish steps (R18)
+    const bool free_step = polishing || S.hlev < 2.0;
+    if (polishing) {
+      --polish_left;
+    } else if (!free_step) {
+      mu = merit_mu(mu, wd, dd, S.h1, kMuRho, kMuFloor);
+      phi_cur = S.f + mu * S.h1;
+      Dphi = wd - mu * S.h1;
+    }
+    double alpha = 1.0;
+    int tries = 0;
+    double* xo = (cur == buf0) ? buf1 : buf0;
+    FluxkSums St;
+    while (true) {
+      fluxk_pass<Q, FLUX>(P, pp, mk(cur), mk(uh), u0, xo, true, alpha, M0, bd, St);
+      ++passes;
+      if (free_step) break;
+      const double phi_t = St.f + mu * St.h1;
+      if (!St.bad && finite_d(phi_t) && phi_t <= phi_cur + P.ls_c1 * alpha * Dphi) break;
+      if (++tries > P.ls_max) { status = SNAP_ST_LINESEARCH; break; }
+      alpha *= P.ls_shrink;
+      ++nback;
+    }
+    if (status == SNAP_ST_LINESEARCH) break;
+    if (!polishing) ++steps;
+    cur = xo;
+    S = St;
+  }
+
+  if (status == SNAP_ST_NONFINITE) {
+    if (ustar != uh)
+      for (size_t i = lane; i < n; i += 32) ustar[i] = uh[i];
+    for (size_t i = lane; i < (size_t)P.m; i += 32) lam[i] = 0.0;
+  } else {
+    // (after a failed line search the multipliers in lE / lM are those of the last accepted point `cur`)
+    const double lamEK = (P.fk_energy && F > 0) ? bd.lE[0] : 0.0;
+    const bool okl = fluxk_local_multipliers<Q, FLUX>(P, lane, pp.first, cur, uh, u0, lamEK, lam);
+    if (lane == 0) { pp.rows_rd += 3 * (K + 1); pp.rows_wr += 2 * (K + 1); }
+    if (!okl) {
+      status = SNAP_ST_NONFINITE;
+      if (ustar != uh)
+        for (size_t i = lane; i < n; i += 32) ustar[i] = uh[i];
+      for (size_t i = lane; i < (size_t)P.m; i += 32) lam[i] = 0.0;
+    } else {
+      double* lb = lam + (size_t)(K + 1) * nx;
+      for (int f = lane; f < F; f += 32) {
+        lb[f] = bd.lM[f];
+        if (P.fk_energy) lb[F + f] = bd.lE[f];
+      }
+      if (cur != ustar) {
+        for (size_t i = lane; i < n; i += 32) ustar[i] = cur[i];
+        if (lane == 0) { pp.rows_rd += nt; pp.rows_wr += nt; }
+      }
+    }
+  }
+  if (lane == 0) {
+    A.iters[b] = (status == 0) ? solves : status;
+    if (A.stats) {
+      long long* stat = A.stats + (size_t)b * SNAP_STAT_COUNT;
+      stat[SNAP_STAT_LINEARISATIONS] = solves; stat[SNAP_STAT_PASSES] = passes;
+      stat[SNAP_STAT_ROWS_READ] = pp.rows_rd; stat[SNAP_STAT_ROWS_WRITTEN] = pp.rows_wr;
+      stat[SNAP_STAT_VARIANT] = A.variant; stat[SNAP_STAT_INNER] = (long long)solves * 2 * F;
+      stat[SNAP_STAT_ROW_DOUBLES] = nx; stat[SNAP_STAT_BACKTRACKS] = nback;
+    }
+  }
+}
+
+template <int Q, int FLUX>
+inline int launch_fluxk_variant(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+  auto kern = project1d_fluxk_kernel<Q, FLUX>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
+    return SNAP_ECUDA;
+  kern<<<pl.grid, pl.wpc * 32, pl.smem, st>>>(a);
+  return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
+}
+
+}  // namespace snap

@@ -128,11 +128,12 @@ __global__ void __launch_bounds__(kMiscThreads) residual_kernel(const __grid_con
   s_pde = block_reduce(s_pde, red, false);
   s_mass = block_reduce(s_mass, red, false);
   if (norms && threadIdx.x == 0) {
-    double* nb = norms + (size_t)b * 4;
+    double* nb = norms + (size_t)b * 5;
     nb[0] = hinf;
     nb[1] = sqrt(s_ic);
     nb[2] = sqrt(s_pde);
     nb[3] = sqrt(s_mass);
+    nb[4] = 0.0;
   }
 }
 

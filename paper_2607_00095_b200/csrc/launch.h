@@ -51,6 +51,10 @@ bool fused_variant(int nx, int& W, int& Q, int& JT, int& maxt);
 // proj1d_fisher_fused.cu: same for kind 2
 int launch_project1d_fisher_fused(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
 bool fused_variant_fisher(int nx, int& W, int& Q, int& JT, int& maxt);
+// proj1d_fluxk.cu: kind 5
+int launch_project1d_fluxk(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st);
+int launch_residual_fluxk(const DevParams& P, int batch, const double* u, const double* cdata, double* h, double* norms,
+                          cudaStream_t st);
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, long long* stats, cudaStream_t st);
 

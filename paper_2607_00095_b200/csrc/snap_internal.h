@@ -29,6 +29,10 @@ struct DevParams {
   double fi_a, fi_dtrho;              // a = dt D / dx^2
   // Allen-Cahn (kind 3): T = I - dt eps^2 Lap_h + dt diag(3u^2-1)
   double ac_ax, ac_ay;                // dt eps^2 / dx^2 , dt eps^2 / dy^2
+  // kind 5 (BURGERS1D_FLUXK): K flux steps, energy rows on/off, flux kind; s = dt/dx, c = nu dt/dx^2,
+  // cD = 2 dt nu / dx, dtnu = dt nu
+  int fk_K, fk_energy, fk_flux;
+  double fk_s, fk_c, fk_cD, fk_dtnu, fk_alpha;
   // solver knobs
   double tol, ls_c1, ls_shrink, pcg_rtol;
   int max_iter, polish, ls_max, pcg_max, precond, lambda_mode;

@@ -67,7 +67,7 @@ def gpu_project(S, wl, u_hat, params=None, warm=False, lam0=None, in_place=False
         lam.copy_(lam0.to(dev))
     it = torch.full((B,), -99, dtype=torch.int32, device=dev)
     S.snap_project(p, B, uh, cd, us, lam, it, warm=warm)
-    norms = torch.empty(B, 4, dtype=torch.float64, device=dev)
+    norms = torch.empty(B, 5, dtype=torch.float64, device=dev)
     S.snap_residual(p, B, us, cd, None, norms)
     torch.cuda.synchronize()
     out = dict(u=us.cpu().numpy(), lam=lam.cpu().numpy(), iters=it.cpu().numpy(), norms=norms.cpu().numpy(),
@@ -118,7 +118,7 @@ def test_residual_and_schur_operator(S, cfg):
         u = wl.u_hat.to(dev)
         cd = wl.cdata.to(dev)
         h = torch.empty(B, p.m, dtype=torch.float64, device=dev)
-        norms = torch.empty(B, 4, dtype=torch.float64, device=dev)
+        norms = torch.empty(B, 5, dtype=torch.float64, device=dev)
         S.snap_residual(p, B, u, cd, h, norms)
         g = torch.Generator().manual_seed(7)
         x = torch.randn(B, p.m, generator=g, dtype=torch.float64)
@@ -131,7 +131,8 @@ def test_residual_and_schur_operator(S, cfg):
             h_ref = O.residual(wl.kind, ub, u0, wl.params)
             np.testing.assert_allclose(h[b].cpu().numpy(), h_ref, rtol=0, atol=2e-14 * max(1, np.abs(h_ref).max()))
             n_ref = O.residual_norms(wl.kind, ub, u0, wl.params)
-            np.testing.assert_allclose(norms[b].cpu().numpy(), n_ref, rtol=1e-13, atol=1e-15)
+            np.testing.assert_allclose(norms[b].cpu().numpy()[:4], n_ref, rtol=1e-13, atol=1e-15)
+            assert float(norms[b, 4]) == 0.0
             J = O.jacobian(wl.kind, ub, wl.params)
             s_ref = J @ (J.T @ x[b].numpy())
             np.testing.assert_allclose(out[b].cpu().numpy(), s_ref, rtol=0, atol=1e-13 * max(1, np.abs(s_ref).max()))
@@ -213,7 +214,7 @@ def test_project_parity_cfg5_full_size_tau_sequence(S):
     lam = torch.zeros(B, p.m, dtype=torch.float64, device=dev)
     it = torch.empty(B, dtype=torch.int32, device=dev)
     ws = torch.empty(S.snap_workspace_bytes(p, B), dtype=torch.uint8, device=dev)
-    norms = torch.empty(B, 4, dtype=torch.float64, device=dev)
+    norms = torch.empty(B, 5, dtype=torch.float64, device=dev)
     for n_call, (j, b) in enumerate([(1, 17), (25, 600), (50, 1023)]):
         uh_cpu = W.burgers_tau_input(wl, j)
         uh = uh_cpu.to(dev)
@@ -512,3 +513,126 @@ def test_host_entry_point_chunked_pipeline_matches_device_path(S):
             np.testing.assert_array_equal(lam.numpy(), ref["lam"])
             np.testing.assert_array_equal(it.numpy(), ref["iters"])
         p.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# kind 5, BURGERS1D_FLUXK: wide J, coupled border rows, banded border solve
+# ------------------------------------------------------------------------------------------------
+FLUXK_SMALL = [(6, dict(batch=3, nx=32, nt=20)), (6, dict(batch=9, nx=64, nt=33)), (6, dict(batch=2, nx=128, nt=12)),
+               (6, dict(batch=2, nx=256, nt=24)), (7, dict(batch=3, nx=32, nt=20)), (7, dict(batch=2, nx=128, nt=17)),
+               (6, dict(batch=2, nx=64, nt=12, params=dict(flux_steps=0))),
+               (6, dict(batch=2, nx=64, nt=9, params=dict(flux_steps=8))),        # no free level: the square kind again
+               (6, dict(batch=2, nx=64, nt=9, params=dict(flux_steps=7))),        # one free level
+               (6, dict(batch=2, nx=32, nt=16, params=dict(energy_rows=0))),      # Eq. 14 exactly (affine free levels)
+               (7, dict(batch=2, nx=64, nt=14, params=dict(energy_rows=1, nu=0.01)))]
+
+
+def test_fluxk_residual_matches_oracle(S):
+    dev = torch.device("cuda:0")
+    for cfg, kw in FLUXK_SMALL:
+        wl = W.make_workload(cfg, **kw)
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        assert p.m == wl.m == O.num_rows(wl.kind, wl.nx, 1, wl.nt, wl.params)
+        B = wl.batch
+        h = torch.empty(B, p.m, dtype=torch.float64, device=dev)
+        norms = torch.empty(B, 5, dtype=torch.float64, device=dev)
+        S.snap_residual(p, B, wl.u_hat.to(dev), wl.cdata.to(dev), h, norms)
+        torch.cuda.synchronize()
+        for b in range(B):
+            h_ref = O.residual(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+            np.testing.assert_allclose(h[b].cpu().numpy(), h_ref, rtol=0, atol=2e-14 * max(1, np.abs(h_ref).max()))
+            n_ref = O.residual_norms(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+            np.testing.assert_allclose(norms[b].cpu().numpy(), n_ref, rtol=1e-12, atol=1e-15)
+        p.destroy()
+
+
+def test_fluxk_project_parity_small(S):
+    for cfg, kw in FLUXK_SMALL:
+        wl = W.make_workload(cfg, **kw)
+        g = gpu_project(S, wl, wl.u_hat)
+        assert (g["iters"] > 0).all(), (cfg, kw, g["iters"])
+        assert g["norms"][:, 0].max() < 1e-10, (cfg, kw)
+        for b in range(wl.batch):
+            o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+            assert o["status"] == 0
+            ru = np.abs(g["u"][b] - o["u"]).max() / np.abs(o["u"]).max()
+            rl = rel_lam(g["lam"][b], o["lam"])
+            assert ru <= TOL_U and rl <= TOL_L, (cfg, kw, b, ru, rl)
+            assert abs(int(g["iters"][b]) - int(o["iters"])) <= 1
+            ks, _ = kkt_invariants(wl, wl.u_hat[b].numpy(), g["u"][b], g["lam"][b])
+            assert ks <= 1e-10, (cfg, kw, b, ks)       # wide J: first order in the last step (tests/test_oracle_fluxk.py)
+        print(f"cfg{cfg} {kw}: iters {g['iters'].tolist()}")
+
+
+def test_fluxk_result_depends_on_the_input_and_edge_cases(S):
+    wl = W.make_workload(6, batch=2, nx=64, nt=16)
+    g = gpu_project(S, wl, wl.u_hat)
+    K = int(wl.params["flux_steps"])
+    np.testing.assert_allclose(g["u"][:, :K + 1], wl.u_true.numpy()[:, :K + 1], rtol=0, atol=1e-11)   # pinned levels: P2
+    bumped = wl.u_hat + 0.01 * torch.cos(torch.arange(wl.u_hat.numel(), dtype=torch.float64)).reshape(wl.u_hat.shape)
+    g2 = gpu_project(S, wl, bumped)
+    assert np.abs(g2["u"][:, K + 1:] - g["u"][:, K + 1:]).max() > 1e-3                                # free levels move
+    np.testing.assert_allclose(g2["u"][:, :K + 1], g["u"][:, :K + 1], rtol=0, atol=1e-11)
+    again = gpu_project(S, wl, torch.from_numpy(g["u"]))                                              # idempotence
+    np.testing.assert_array_equal(again["u"], g["u"])
+    assert (again["iters"] == 1).all()
+    inp = gpu_project(S, wl, wl.u_hat.clone(), in_place=True)
+    np.testing.assert_array_equal(inp["u"], g["u"])
+    np.testing.assert_array_equal(inp["lam"], g["lam"])
+    one = gpu_project(S, wl, wl.u_hat[1:2].clone(), cdata=wl.cdata[1:2])
+    np.testing.assert_array_equal(one["u"][0], g["u"][1])
+    big = gpu_project(S, wl, wl.u_hat * 1e160)
+    assert (big["iters"] == -3).all() and np.all(big["lam"] == 0)
+    capped = gpu_project(S, wl, wl.u_hat, params=dict(max_iter=1))
+    assert (capped["iters"] == -1).all()
+    o = O.project(wl.kind, wl.u_hat[0].numpy(), wl.cdata[0].numpy(), dict(wl.params, max_iter=1))
+    np.testing.assert_allclose(capped["u"][0], o["u"], rtol=0, atol=1e-12)
+
+
+def test_fluxk_line_search_is_live_far_from_the_feasible_set(S):
+    """noise 1.0: Gauss-Newton with W = I contracts slowly and the Armijo test rejects full steps (oracle pin
+    test_gauss_newton_converges_linearly...); GPU and oracle take the same decisions and land on the same point."""
+    wl = W.make_workload(6, batch=2, nx=32, nt=12, noise=1.0, params=dict(max_iter=400))
+    dev = torch.device("cuda:0")
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    B = wl.batch
+    uh = wl.u_hat.to(dev)
+    us = torch.empty_like(uh)
+    lam = torch.zeros(B, p.m, dtype=torch.float64, device=dev)
+    it = torch.zeros(B, dtype=torch.int32, device=dev)
+    ws = S.snap_project(p, B, uh, wl.cdata.to(dev), us, lam, it)
+    st = torch.zeros(B, S.STAT_COUNT, dtype=torch.int64, device=dev)
+    S.snap_project_stats(p, B, ws, st)
+    torch.cuda.synchronize()
+    st = st.cpu().numpy()
+    assert (st[:, S.STAT_VARIANT] == S.VAR_FLUXK_BAND).all()
+    for b in range(B):
+        o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+        assert o["status"] == 0 and int(it[b]) > 0
+        assert st[b, S.STAT_BACKTRACKS] == o["backtracks"]
+        ru = np.abs(us[b].cpu().numpy().reshape(o["u"].shape) - o["u"]).max() / np.abs(o["u"]).max()
+        assert ru <= 1e-8, ru          # slow linear contraction (~0.9 per step): both stop ~1e-10/(1-rate) from the limit
+    p.destroy()
+
+
+@pytest.mark.parametrize("cfg", [6, 7])
+def test_fluxk_full_size(S, cfg):
+    """256 x 256, batch 1024, Flux(5): oracle on three samples, invariants on 64, pinned levels on all."""
+    wl = W.make_workload(cfg)
+    g = gpu_project(S, wl, wl.u_hat)
+    assert (g["iters"] > 0).all()
+    assert g["norms"][:, 0].max() < 1e-10
+    K = int(wl.params["flux_steps"])
+    assert np.abs(g["u"][:, :K + 1] - wl.u_true.numpy()[:, :K + 1]).max() < 1e-10
+    for b in (0, 500, 1023):
+        o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+        ru = np.abs(g["u"][b] - o["u"]).max() / np.abs(o["u"]).max()
+        rl = rel_lam(g["lam"][b], o["lam"])
+        print(f"cfg{cfg} sample {b}: rel_u {ru:.1e} rel_lam {rl:.1e} iters {int(g['iters'][b])} / {o['iters']}")
+        assert ru <= TOL_U and rl <= TOL_L
+    worst = 0.0
+    for b in range(0, wl.batch, 16):
+        ks, _ = kkt_invariants(wl, wl.u_hat[b].numpy(), g["u"][b], g["lam"][b])
+        worst = max(worst, ks)
+    print(f"cfg{cfg}: stationarity on 64 samples {worst:.1e}, iters {np.bincount(g['iters'])}")
+    assert worst <= 1e-10

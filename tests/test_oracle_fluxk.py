@@ -213,10 +213,13 @@ def test_gauss_newton_converges_linearly_with_energy_rows_and_the_line_search_is
     wl = _wl(batch=1, nx=24, nt=12, noise=1.0)
     uh, u0 = wl.u_hat[0].numpy(), wl.cdata[0].numpy()
     hist = []
-    a = O.project(K5, uh, u0, wl.params, history=hist)
-    assert a["status"] == 0 and len(hist) >= 6
-    rates = [hist[i + 1] / hist[i] for i in range(2, len(hist) - 2) if hist[i] > 1e-9]
-    assert rates and min(rates) > 1e-4            # not quadratic: successive ratios do not collapse
+    a = O.project(K5, uh, u0, dict(wl.params, max_iter=400), history=hist)   # contraction ~0.93 per step this far out
+    assert a["status"] == 0 and len(hist) >= 50
+    # linear, not quadratic: feasibility arrives early (h -> rounding) but the tangential step shrinks by a constant
+    # factor per solve, so stationarity takes > 50 solves here where Newton would need a handful
+    J = O.jacobian(K5, a["u"], wl.params)
+    stat = (a["u"] - uh).ravel() + J.T @ a["lam"]
+    assert np.abs(stat).max() < 1e-9 * max(1.0, np.abs(a["lam"]).max())    # the step criterion (R18) bounds stationarity
     assert a["backtracks"] > 0                    # and the Armijo test rejects full steps on the way
     # (this far out the lam_inf rule takes > 50 un-damped steps at contraction ~0.93: the regime NEXT-2's exact W is for)
     wl = _wl(batch=1, nx=24, nt=12, noise=0.3)

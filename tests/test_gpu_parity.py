@@ -560,7 +560,10 @@ def test_fluxk_project_parity_small(S):
             assert ru <= TOL_U and rl <= TOL_L, (cfg, kw, b, ru, rl)
             assert abs(int(g["iters"][b]) - int(o["iters"])) <= 1
             ks, _ = kkt_invariants(wl, wl.u_hat[b].numpy(), g["u"][b], g["lam"][b])
-            assert ks <= 1e-10, (cfg, kw, b, ks)       # wide J: first order in the last step (tests/test_oracle_fluxk.py)
+            # wide J, W = I: stationarity is first order in the last step and the stop rule bounds RMS(d) <= tol, not
+            # ||d||_inf (R18): the oracle itself sits at 1.2e-10 .. 1.9e-10 on the 64 x 33 case, hence the
+            # bound of tests/test_oracle_fluxk.py (1e-9), not P4's 1e-11
+            assert ks <= 1e-9, (cfg, kw, b, ks)
         print(f"cfg{cfg} {kw}: iters {g['iters'].tolist()}")
 
 
@@ -635,4 +638,4 @@ def test_fluxk_full_size(S, cfg):
         ks, _ = kkt_invariants(wl, wl.u_hat[b].numpy(), g["u"][b], g["lam"][b])
         worst = max(worst, ks)
     print(f"cfg{cfg}: stationarity on 64 samples {worst:.1e}, iters {np.bincount(g['iters'])}")
-    assert worst <= 1e-10
+    assert worst <= 1e-9      # R18: RMS(d) <= tol bounds stationarity only to first order (see the small-shape test)

@@ -336,8 +336,13 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
     heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters, stats);
     return check_launch(p);
   }
-  if (d.kind == SNAP_ALLENCAHN2D_IE)
+  if (d.kind == SNAP_ALLENCAHN2D_IE) {
+    if (p->params.gn_fuse >= 0) {   // product-form path (in-SMEM level solves) where the shape and parameters allow it
+      const int rc = launch_project2d_direct(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, st);
+      if (rc <= 0) return rc;
+    }
     return launch_project2d(p, batch, u_hat, cdata, u_star, lambda, iters, warm, w, stats, st);
+  }
 
   if (d.kind == SNAP_BURGERS1D_FLUXK) return project_fluxk(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, st);
   Plan1d pl;

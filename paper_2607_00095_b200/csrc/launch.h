@@ -58,4 +58,8 @@ int launch_residual_fluxk(const DevParams& P, int batch, const double* u, const 
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, long long* stats, cudaStream_t st);
 
+// proj2d_direct.cu: product-form path of kind 3; returns +1 when the shape / parameters / alignment are outside it
+int launch_project2d_direct(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
+                            double* lambda, int* iters, void* workspace, long long* stats, cudaStream_t st);
+
 }  // namespace snap

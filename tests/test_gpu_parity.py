@@ -312,8 +312,51 @@ def test_warm_start_2d_reaches_the_same_point(S):
 @pytest.mark.parametrize("precond", [0, 1, 2])
 def test_pcg_preconditioners_agree(S, precond):
     wl = W.make_workload(4, **SMALL[4][0])
-    g = gpu_project(S, wl, wl.u_hat, params=dict(precond=precond, pcg_max=2000))
+    g = gpu_project(S, wl, wl.u_hat, params=dict(precond=precond, pcg_max=2000, gn_fuse=-1))
     check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
+
+
+def test_direct2d_matches_oracle_and_pcg_path(S):
+    """Kind 3, product-form path (in-SMEM red-black level solves): same limit point as the oracle
+    and as the PCG kernel (gn_fuse = -1) on 2-row and 4-row patches, one and several warps, nt = 2."""
+    for kw in [dict(batch=2, nx=12, ny=10, nt=6), dict(batch=2, nx=16, ny=16, nt=4), dict(batch=3, nx=32, ny=16, nt=5),
+               dict(batch=2, nx=64, ny=64, nt=3), dict(batch=2, nx=24, ny=6, nt=2), dict(batch=2, nx=128, ny=32, nt=4)]:
+        wl = W.make_workload(4, **kw)
+        d = gpu_project(S, wl, wl.u_hat)
+        c = gpu_project(S, wl, wl.u_hat, params=dict(gn_fuse=-1))
+        assert (d["iters"] > 0).all() and (c["iters"] > 0).all(), (kw, d["iters"], c["iters"])
+        assert d["norms"][:, 0].max() < 1e-10
+        np.testing.assert_allclose(d["u"], c["u"], rtol=0, atol=1e-11)
+        np.testing.assert_allclose(d["lam"], c["lam"], rtol=0, atol=1e-9 * np.abs(c["lam"]).max())
+        check_against_oracle(wl, wl.u_hat, d, range(wl.batch))
+
+
+def test_direct2d_status_codes_and_line_search(S):
+    wl = W.make_workload(4, batch=2, nx=16, ny=16, nt=5)
+    big = gpu_project(S, wl, wl.u_hat * 1e160)
+    assert (big["iters"] == -3).all() and np.all(big["lam"] == 0)
+    np.testing.assert_array_equal(big["u"], (wl.u_hat * 1e160).numpy())
+    big_in_place = gpu_project(S, wl, wl.u_hat * 1e160, in_place=True)
+    assert (big_in_place["iters"] == -3).all()
+    np.testing.assert_array_equal(big_in_place["u"], (wl.u_hat * 1e160).numpy())
+    capped = gpu_project(S, wl, wl.u_hat, params=dict(max_iter=1))
+    assert (capped["iters"] == -1).all()
+    for b in range(wl.batch):
+        o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), dict(wl.params, max_iter=1))
+        np.testing.assert_allclose(capped["u"][b], o["u"], rtol=0, atol=1e-11)
+        assert rel_lam(capped["lam"][b], o["lam"]) <= TOL_L
+    # forced Armijo halving (R17): the limit point does not move; exhausted halvings give status -2 and the last accepted iterate
+    wn = W.make_workload(4, batch=2, nx=16, ny=16, nt=5, noise=1.0)
+    ref = gpu_project(S, wn, wn.u_hat)
+    forced = gpu_project(S, wn, wn.u_hat, params=dict(ls_c1=0.9))
+    assert (ref["iters"] > 0).all() and (forced["iters"] > 0).all()
+    np.testing.assert_allclose(forced["u"], ref["u"], rtol=0, atol=1e-11)
+    check_against_oracle(wn, wn.u_hat, forced, range(wn.batch), params=dict(ls_c1=0.9))
+    stuck = gpu_project(S, wn, wn.u_hat, params=dict(ls_c1=0.9, ls_max=0))
+    o = O.project(wn.kind, wn.u_hat[0].numpy(), wn.cdata[0].numpy(), dict(wn.params, ls_c1=0.9, ls_max=0))
+    assert int(stuck["iters"][0]) == o["iters"]
+    if o["status"] == -2:
+        np.testing.assert_allclose(stuck["u"][0], o["u"], rtol=0, atol=1e-11)
 
 
 def test_line_search_backtracking_on_gpu(S):
@@ -436,7 +479,9 @@ def test_stats_record_which_kernel_variant_ran(S):
     cases = [(5, dict(batch=2, nx=64, nt=12), {}, S.VAR_FUSED_TMA), (5, dict(batch=2, nx=64, nt=12), dict(gn_fuse=-1), S.VAR_CLASSIC_BULK),
              (2, dict(batch=2, nx=70, nt=12), {}, S.VAR_CLASSIC_BULK), (2, dict(batch=2, nx=101, nt=9), {}, S.VAR_CLASSIC_PLAIN),
              (3, dict(batch=2, nx=64, nt=12), {}, S.VAR_FUSED_TMA), (1, dict(batch=2, nx=20, nt=12), {}, S.VAR_HEAT_CLOSED_FORM),
-             (4, dict(batch=2, nx=12, ny=10, nt=6), dict(precond=2), S.VAR_PCG2D)]
+             (4, dict(batch=2, nx=12, ny=10, nt=6), dict(precond=2, gn_fuse=-1), S.VAR_PCG2D),
+             (4, dict(batch=2, nx=12, ny=10, nt=6), {}, S.VAR_DIRECT2D), (4, dict(batch=2, nx=32, ny=16, nt=5), {}, S.VAR_DIRECT2D),
+             (4, dict(batch=2, nx=10, ny=12, nt=5), {}, S.VAR_PCG2D)]     # nx not a multiple of 4: outside the direct path
     for cfg, kw, prm, want in cases:
         wl = W.make_workload(cfg, **kw)
         p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, dict(wl.params, **prm))
@@ -455,7 +500,8 @@ def test_stats_record_which_kernel_variant_ran(S):
         assert (st[:, S.STAT_ROWS_READ] > 0).all() and (st[:, S.STAT_ROWS_WRITTEN] > 0).all()
         assert (st[:, S.STAT_ROW_DOUBLES] == wl.nx * wl.ny).all()
         if cfg == 4:
-            assert (st[:, S.STAT_INNER] >= st[:, S.STAT_LINEARISATIONS]).all()   # >= 1 PCG iteration per solve (R15)
+            # PCG: >= 1 iteration per solve (R15); direct: >= 1 red-black sweep per level solve
+            assert (st[:, S.STAT_INNER] >= st[:, S.STAT_LINEARISATIONS]).all()
         p.destroy()
 
 

@@ -140,6 +140,7 @@ struct FluxkSums {
   double h1, f;     // ||h||_1, 1/2 ||u - u_hat||^2 at the point the pass produced
   double wq, qq;    // pinned levels: w^T q', ||q'||^2 of the Newton direction d = -q' at that point
   double ww;        // free levels: ||w_f||^2
+  double dstep;     // update passes: ||t - x||^2 / alpha^2 = ||d||^2 of the step just applied, summed directly
   bool bad;
 };
 
@@ -178,6 +179,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
 #pragma unroll
   for (int c = 0; c < Q; ++c) { phiA[c] = u0[first + c]; phiB[c] = phiA[c]; ccA[c] = 0.0; ccB[c] = 0.0; }
   double h1 = 0.0, f2 = 0.0, wq = 0.0, qq = 0.0, ww_free = 0.0;   // h1 / ww_free: lane 0 adds the warp-uniform row values
+  double ds2 = 0.0;
   int hmx = 0;
   // carried from the previous level (warp-uniform): energy, dissipation, and the dot products of its b vector
   double E_prev = 0.0, D_prev = 0.0, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, bq_K = 0.0;
@@ -289,6 +291,8 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       E_prev = E_k; D_prev = D_k; bb_prev = r[3]; ab_prev = dx * r[4]; bw_prev = r[7]; s1_prev = r[0];
     }
     if (update) {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) ds2 = fma(t[c] - v[c], t[c] - v[c], ds2);
       store_cells_global<Q>(xo + (size_t)k * nx + first, t);
       if (lane == 0) pp.rows_wr += 1;
     }
@@ -303,6 +307,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   S.wq = warp_sum(wq);
   S.qq = warp_sum(qq);
   S.ww = __shfl_sync(SNAP_FULL, ww_free, 0);
+  S.dstep = warp_sum(ds2) / (alpha * alpha);
   S.bad = !(finite_d(S.h1) && finite_d(f2s) && finite_d(S.wq) && finite_d(S.qq));
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
 }
@@ -506,8 +511,13 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
     // step d: pinned levels d = -q', free levels d = -w - (J_b^f)^T lam_b
     const double wd = -S.wq - S.ww - lam_jw;
     const double dd = S.qq + S.ww + 2.0 * lam_jw + lam_rho;
-    // wide J: ||h|| alone says nothing about stationarity; converged = ||h||_inf < tol and RMS(d) <= tol (R18)
-    const bool conv = S.hlev < 2.0 && dd <= (double)n * P.tol * P.tol;
+    // wide J: ||h|| alone says nothing about stationarity; converged = ||h||_inf < tol and RMS(d) <= tol (R18).
+    // dd is a difference of O(||w||^2) sums: it can certify a small step only when its rounding noise is below the
+    // threshold (w = 0: a feasible input); otherwise the step is taken as a free step and ||d||^2 is summed directly
+    // by the pass that applies it (below).
+    const double thr = (double)n * P.tol * P.tol;
+    const double noise = 1.8e-15 * (S.qq + S.ww + 2.0 * fabs(lam_jw) + lam_rho);
+    const bool conv = S.hlev < 2.0 && dd <= thr && noise <= thr;
     bool final_solve = false;
     if (polishing) {
       final_solve = (polish_left == 0);
@@ -545,6 +555,15 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
       ++nback;
     }
     if (status == SNAP_ST_LINESEARCH) break;
+    if (!polishing && free_step && St.dstep <= thr) {
+      // the step just applied was small: `cur` met both criteria, so this step was its first polish step (R4, R18)
+      if (S.hlev == 0.0 || P.polish == 0) break;   // no polish wanted: `cur` is final, lE / lM are its multipliers
+      polishing = true;
+      polish_left = P.polish - 1;
+      cur = xo;
+      S = St;
+      continue;
+    }
     if (!polishing) ++steps;
     cur = xo;
     S = St;

@@ -56,14 +56,35 @@ struct LaneOff {
   }
 };
 
+// Shared-memory rows are addressed in the .shared state space explicitly (LDS / STS): through the generic pointers of
+// RowPipe the compiler emitted generic LD.E / ST.E, which resolve the address space per access and are tracked by the
+// long scoreboard (profiles/r01d: the top stall of the fused passes).
+__device__ __forceinline__ double2 lds_v2(uint32_t a) {
+  double2 t;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(t.x), "=d"(t.y) : "r"(a));
+  return t;
+}
+__device__ __forceinline__ double lds_f64(uint32_t a) {
+  double t;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(t) : "r"(a));
+  return t;
+}
+__device__ __forceinline__ void sts_v2(uint32_t a, double x, double y) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void sts_f64(uint32_t a, double x) {
+  asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(x) : "memory");
+}
+
 template <int Q>
 __device__ __forceinline__ void load_cells(const double* row, const LaneOff<Q>& lo, double (&x)[Q]) {
+  const uint32_t a = smem_u32(row);
   if constexpr (Q == 1) {
-    x[0] = row[lo.o[0]];
+    x[0] = lds_f64(a + 8u * lo.o[0]);
   } else {
 #pragma unroll
     for (int c = 0; c < Q / 2; ++c) {
-      const double2 t = *reinterpret_cast<const double2*>(row + lo.o[c]);
+      const double2 t = lds_v2(a + 8u * lo.o[c]);
       x[2 * c] = t.x;
       x[2 * c + 1] = t.y;
     }
@@ -71,15 +92,16 @@ __device__ __forceinline__ void load_cells(const double* row, const LaneOff<Q>& 
 }
 template <int Q>
 __device__ __forceinline__ double cell_at(const double* row, const LaneOff<Q>& lo, int c) {
-  return row[lo.o[c >> 1] + (c & 1)];
+  return lds_f64(smem_u32(row) + 8u * (lo.o[c >> 1] + (c & 1)));
 }
 template <int Q>
 __device__ __forceinline__ void store_cells(double* row, const LaneOff<Q>& lo, const double (&x)[Q]) {
+  const uint32_t a = smem_u32(row);
   if constexpr (Q == 1) {
-    row[lo.o[0]] = x[0];
+    sts_f64(a + 8u * lo.o[0], x[0]);
   } else {
 #pragma unroll
-    for (int c = 0; c < Q / 2; ++c) *reinterpret_cast<double2*>(row + lo.o[c]) = make_double2(x[2 * c], x[2 * c + 1]);
+    for (int c = 0; c < Q / 2; ++c) sts_v2(a + 8u * lo.o[c], x[2 * c], x[2 * c + 1]);
   }
 }
 

@@ -446,7 +446,7 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
   unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) + (size_t)slot * A.warp_bytes;
   RowPipe<1, Q> pp;
   pp.stage = reinterpret_cast<double*>(base);
-  pp.orow = nullptr; pp.xch = nullptr; pp.red = nullptr;
+  pp.orow = nullptr; pp.xch = nullptr; pp.red = nullptr; pp.msb = nullptr;
   double* bandmem = pp.stage + (size_t)A.nst * 2 * G::RP;
   pp.aux = nullptr;
   Band bd;

@@ -151,6 +151,7 @@ __device__ __forceinline__ double hinf_level(int hmx_lane, double tol, double sk
   return (m >= __double2hiint(tol)) ? 2.0 : ((m >= __double2hiint(skip)) ? 1.0 : 0.0);
 }
 
+constexpr int kMsbPitch = 34;   // doubles per level slot of RowPipe::msb (32 lanes + padding: conflict-free 128-bit reads)
 constexpr int kRed = 24;   // doubles per warp in the reduction scratch (>= 4 JT + 1)
 
 // a global buffer of the path: its tensor map (rows as TMA boxes) and the sample's base pointer (generic access)
@@ -170,6 +171,7 @@ struct RowPipe {
   double* orow;    // [4][RP]
   double* xch;     // [2][W][8]
   double* red;     // [W][kRed] partial sums of a pass
+  double* msb;     // W = 1: [JT][8 levels][kMsbPitch] per-lane cell sums of the iterates (mass rows, reduced every 8 levels)
   double* aux;     // W = 1: min(nt, 512) doubles (suffix sums of the min-norm correction)
   uint32_t bar0, phase;
   int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
@@ -268,7 +270,6 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
   double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
   double h1[T], wd[T], dd[T];              // per-lane partial sums (thread 0 of the group also takes the mass rows)
   int hmx[T];                              // max over the upper 32 bits of |h| (see hinf_level)
-  double ms[T], msp[T];                    // per-lane sum of the iterate's cells (mass rows): this level, previous level
   const double tol = P.tol, skip = kPolishSkip * P.tol;
   double f2 = 0.0;
   {
@@ -282,29 +283,34 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
         phi[t][c] = u0r[c];   // level 0: h_0 = x[0] - u0
         cc[t][c] = 0.0;
       }
-      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; hmx[t] = 0; ms[t] = 0.0; msp[t] = 0.0;
+      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; hmx[t] = 0;
     }
   }
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, k, x0.tm, tm_uh);
 
-  // W == 1: the mass rows of level k are reduced over the lanes at the start of level k + 1 (branch-free, T
-  // butterflies interleaved), so that the shuffle latency hides behind that level's arithmetic
+  // W == 1, mass rows: every lane parks the sum of its cells of each iterate in shared memory ([t][k & 7][lane]);
+  // after 8 levels the warp reduces the 8 T level sums at once (lane (j, p) adds 8 lanes' entries of level j, two
+  // butterfly rounds join the 4 parts).  A butterfly per level and iterate (5 dependent shuffle rounds) was 12 % of
+  // the instructions of a pass and sat on its critical path (profiles/r02_project1d_fused.md).
   const double dxm = P.dx;
-  const bool mass_lane = has_mass && w == 0 && lane == 0;
-  auto mass_rows = [&](bool valid) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-      for (int t = 0; t < T; ++t) msp[t] += __shfl_xor_sync(SNAP_FULL, msp[t], o);
-    }
+  const uint32_t msb_a = smem_u32(pp.msb);
+  auto mass_rows8 = [&](int nv) {
+    __syncwarp();
+    const int j = lane & 7, pq = lane >> 3;
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-      const double hm = fabs(fma(dxm, msp[t], -M0));
-      const bool on = mass_lane && valid;
+      const uint32_t a = msb_a + 8u * (uint32_t)((t * 8 + j) * kMsbPitch + pq * 8);
+      const double2 x0 = lds_v2(a), x1 = lds_v2(a + 16u), x2 = lds_v2(a + 32u), x3 = lds_v2(a + 48u);
+      double sacc = ((x0.x + x0.y) + (x1.x + x1.y)) + ((x2.x + x2.y) + (x3.x + x3.y));
+      sacc += __shfl_xor_sync(SNAP_FULL, sacc, 8);
+      sacc += __shfl_xor_sync(SNAP_FULL, sacc, 16);
+      const double hm = fabs(fma(dxm, sacc, -M0));
+      const bool on = (pq == 0) && (j < nv);
       hmx[t] = max(hmx[t], on ? __double2hiint(hm) : 0);
       h1[t] += on ? hm : 0.0;
     }
+    __syncwarp();
   };
 
   int s = 0, par = 0;
@@ -342,9 +348,6 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
           if (t == 0) f2 = fma(wv, wv, f2);
         }
       }
-      if constexpr (W == 1) {
-        if (t == 0) mass_rows(k > 0);   // previous level's mass rows: independent of this level's arithmetic
-      }
       // end values of the next iterate (only the two ends are exchanged; the rest is updated in place below)
       const double vn0 = (t < NU) ? v[0] - q[0] : v[0], vnE = (t < NU) ? v[Q - 1] - q[Q - 1] : v[Q - 1];
       double qL = shfl_prev(q[Q - 1], lane), qR = shfl_next(q[0], lane);
@@ -370,7 +373,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
           h1[t] += hm;
         }
       } else {
-        ms[t] = msum;   // reduced after the iterations of this level, all T butterflies interleaved
+        if (has_mass) sts_f64(msb_a + 8u * (uint32_t)((t * 8 + (k & 7)) * kMsbPitch + lane), msum);
       }
       // state for the next level (needs the old v and q with neighbours), then the update in place
       double um = vL, ql = qL;
@@ -389,8 +392,9 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
       else if constexpr (kDirect) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
       else store_cells<Q>(so_y, pp.lo, q);
     }
-#pragma unroll
-    for (int t = 0; t < T; ++t) msp[t] = ms[t];
+    if constexpr (W == 1) {
+      if (has_mass && ((k & 7) == 7 || k == nt - 1)) mass_rows8((k & 7) + 1);
+    }
     if constexpr (kDirect) {
       if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
       if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + (EMIT ? 1 : 0);
@@ -402,7 +406,6 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
     if (++s == nst) s = 0;
   }
-  if constexpr (W == 1) mass_rows(true);   // last level
   pp.drain();
   // ---- reduce: lanes -> warp -> group (fixed order: identical in every warp, run-to-run deterministic) ----
   double part[4 * T + 1];
@@ -906,7 +909,8 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;           // output staging rows: only W > 1 uses them
   pp.xch = pp.orow + (size_t)(W > 1 ? 4 : 0) * G::RP;
   pp.red = pp.xch + G::XCH;
-  pp.aux = pp.red + W * kRed;
+  pp.msb = pp.red + W * kRed;
+  pp.aux = pp.msb + (W == 1 ? JT * 8 * kMsbPitch : 0);
   pp.bar0 = smem_u32(pp.aux + (W == 1 ? (nt < 512 ? nt : 512) : 0));
   pp.phase = 0;
   pp.nst = A.nst; pp.lane = lane; pp.w = w; pp.bar_id = 1 + slot;

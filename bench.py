@@ -7,7 +7,7 @@ flow-matching times tau_j = j/50 with the multiplier warm start carried from tau
 One "step" = that whole 50-call sequence = 51 200 projections.  All 50 inputs (25.6 GB) are resident in
 HBM before the timed region, so the working set is far larger than L2 and no L2 flush is needed.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg1..cfg4] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg1..cfg4|cfg6|cfg7] [--impl reference]
 
 Multi-GPU (torchrun): samples are independent blocks, so each rank projects its own
 batch of the same size with no data-path collective ("scaling": "weak"); NCCL carries only the barrier
@@ -160,7 +160,7 @@ def run_reference(args):
     cfg = int(args.workload[3:])
     cores = os.cpu_count() or 1
     workers = min(cores, 16)
-    n_samples = workers if cfg in (4, 5) else max(workers, 16)
+    n_samples = workers if cfg in (4, 5, 6, 7) else max(workers, 16)
     times = []
     desc = ""
     for s in range(args.warmup + args.steps):
@@ -187,8 +187,10 @@ def workload_name(cfg: int) -> str:
         1: "cfg1: 1D heat IC+mass projection, batch 4, 64x64 (linear)",
         2: "cfg2: 1D viscous Burgers LF projection, batch 32, 128x128",
         3: "cfg3: 1D Fisher-KPP implicit projection, batch 256, 128x128",
-        4: "cfg4: 2D Allen-Cahn implicit projection, batch 64, 64x64x32 (PCG)",
+        4: "cfg4: 2D Allen-Cahn implicit projection, batch 64, 64x64x32 (product-form sweeps, level solves in shared memory)",
         5: "cfg5: 1D Burgers LF + mass rows at scale, batch 1024, 256x256, 50 flow times tau=j/50, warm-started",
+        6: "cfg6 (SURVEY 8(f) NEXT-1): Burgers IC + Flux(k=5, Lax-Friedrichs) + mass + energy rows, batch 1024, 256x256 (wide J, banded border solve)",
+        7: "cfg7 (SURVEY 8(f) NEXT-1/4): inviscid Burgers IC + Flux(k=5, Godunov) + mass rows, batch 1024, 256x256",
     }[cfg]
 
 
@@ -308,8 +310,9 @@ def e2e_steps(run: GpuRun, steps: int, warmup: int):
 
 
 KERNEL_NAMES = {5: "project1d_fused_kernel<KB,1,8,3> (Burgers family, nx=256)", 2: "project1d_fused_kernel<KB,1,4,4> (nx=128)",
-                3: "project1d_fused_kernel<KF,1,4,3> (Fisher, nx=128)", 4: "project2d kernel (see variant)",
-                1: "heat_project_kernel"}
+                3: "project1d_fused_kernel<KF,1,4,3> (Fisher, nx=128)",
+                4: "project2d_direct_kernel<4,256> (variant 6; variant 5 = project2d_kernel, PCG)",
+                1: "heat_project_kernel", 6: "project1d_fluxk_kernel<8,LF>", 7: "project1d_fluxk_kernel<8,Godunov>"}
 
 
 def roofline_of(run, cfg, kern_s, alg_bytes_call, steps, peak, peak_src):
@@ -386,8 +389,9 @@ def run_gpu(args):
         "config": {"workload": workload_name(cfg), "batch_per_gpu": run.B, "nx": wl.nx, "ny": wl.ny, "nt": wl.nt,
                    "calls_per_step": run.calls, "projections_per_step": units,
                    "l2": "inputs (25.6 GB resident) exceed L2; no flush" if cfg == 5 else
-                         ("PCG/iterate vectors (0.6 GB) exceed L2; no flush" if cfg == 4 else
-                          "working set smaller than L2 (latency-bound config; see DESIGN.md)"),
+                         ("iterate / multiplier vectors (0.4 GB) exceed L2; no flush" if cfg == 4 else
+                          ("input + iterates (1.5 GB) exceed L2; no flush" if cfg in (6, 7) else
+                           "working set smaller than L2 (latency-bound config; see DESIGN.md)")),
                    "tol": wl.params["tol"], "converged_all": ok, "max_hinf_last_call": hmax,
                    "mean_linearisations_per_projection": float(solves.sum() / (run.B * run.calls)),
                    "alg_bytes_per_projection": sum(alg_bytes_call) / (run.B * run.calls)},
@@ -403,12 +407,12 @@ def run_gpu(args):
         cores = os.cpu_count() or 1
         workers = min(cores, 16)
         taus = (1, 25, 49) if cfg == 5 else (25,)
-        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5) else max(workers, 16), workers, taus=taus)
+        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5, 6, 7) else max(workers, 16), workers, taus=taus)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "host_cpu_count": cores, "kind": "oracle",
                                 "sample": desc, "seconds": dt}
     if rank == 0 and world == 1 and args.others and cfg == 5:
         others = {}
-        for c in (1, 2, 3, 4):
+        for c in (1, 2, 3, 4, 6, 7):
             r = GpuRun(S, c, dev)
             ms, km, _ = time_steps(r, 5, 3, None)
             okc, hm, itc = r.check()
@@ -417,7 +421,10 @@ def run_gpu(args):
             others[f"cfg{c}"] = {"projections_per_s": r.B * 5 / (ms * 1e-3), "ms_per_call": ms / 5, "converged_all": okc,
                                  "max_hinf": hm, "roofline": roofline_of(r, c, ks, ab, 5, peak, peak_src),
                                  "note": {1: "4 samples x 32 KiB: latency-bound, fits L2", 2: "32 samples, 4 MiB per field: fits L2, latency-bound",
-                                          3: "256 samples, 32 MiB per field: L2-borderline", 4: "64 samples, 64 MiB per field"}[c]}
+                                          3: "256 samples, 32 MiB per field: L2-borderline",
+                                          4: "64 samples, 64 MiB per field; 64 CTAs on 148 SMs: level solves bound by shared-memory latency (DESIGN.md 6.2)",
+                                          6: "not a BASELINE.json config: the paper's IC + Mass + Flux(k=5) row set with energy rows at cfg-5 scale",
+                                          7: "not a BASELINE.json config: Godunov flux variant"}[c]}
             del r
         line["other_workloads"] = others
     if rank == 0:
@@ -443,7 +450,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "cfg6", "cfg7"])
     ap.add_argument("--impl", default="snap", choices=["snap", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -116,20 +116,28 @@ __device__ __forceinline__ void energy_b(const DevParams& P, const double (&v)[Q
 }
 
 // per-sample band system in shared memory: 10 doubles per free level f (level k = K+1+f), rows E_{k-1} then M_k
+// (arrays live in shared memory and are addressed in the .shared space explicitly: through generic pointers every
+// access was a generic LD.E / ST.E tracked by the long scoreboard, profiles/r02_fluxk.md)
+struct SmemArr {
+  uint32_t a;
+  __device__ __forceinline__ double get(int i) const { return lds_f64(a + 8u * (uint32_t)i); }
+  __device__ __forceinline__ void set(int i, double v) const { sts_f64(a + 8u * (uint32_t)i, v); }
+};
 struct Band {
-  double* dE;    // [F] diagonal of the E row (LDL^T: becomes D)
-  double* dM;    // [F] diagonal of the M row
-  double* eM;    // [F] (E_{k-1}, M_{k-1})  sub-diagonal 1 of the E row
-  double* eE;    // [F] (E_{k-1}, E_{k-2})  sub-diagonal 2 of the E row
-  double* mE;    // [F] (M_k, E_{k-1})      sub-diagonal 1 of the M row
-  double* rE;    // [F] right-hand side of the E row (becomes y, then the solution)
-  double* rM;    // [F]
-  double* lE;    // [F] multipliers of the last solve: energy rows
-  double* lM;    // [F]                               mass rows
-  double* jw;    // [2F] J_b^f w_f (for the penalty parameter), E rows then M rows
+  SmemArr dE;    // [F] diagonal of the E row (LDL^T: becomes D)
+  SmemArr dM;    // [F] diagonal of the M row
+  SmemArr eM;    // [F] (E_{k-1}, M_{k-1})  sub-diagonal 1 of the E row
+  SmemArr eE;    // [F] (E_{k-1}, E_{k-2})  sub-diagonal 2 of the E row
+  SmemArr mE;    // [F] (M_k, E_{k-1})      sub-diagonal 1 of the M row
+  SmemArr rE;    // [F] right-hand side of the E row (becomes y, then the solution)
+  SmemArr rM;    // [F]
+  SmemArr lE;    // [F] multipliers of the last solve: energy rows
+  SmemArr lM;    // [F]                               mass rows
+  SmemArr jw;    // [2F] J_b^f w_f (for the penalty parameter), E rows then M rows
   __device__ __forceinline__ void carve(double* base, int F) {
-    dE = base; dM = dE + F; eM = dM + F; eE = eM + F; mE = eE + F; rE = mE + F; rM = rE + F; lE = rM + F; lM = lE + F;
-    jw = lM + F;
+    const uint32_t b = smem_u32(base), s = 8u * (uint32_t)F;
+    dE.a = b; dM.a = b + s; eM.a = b + 2 * s; eE.a = b + 3 * s; mE.a = b + 4 * s; rE.a = b + 5 * s; rM.a = b + 6 * s;
+    lE.a = b + 7 * s; lM.a = b + 8 * s; jw.a = b + 9 * s;
   }
   static __host__ __device__ constexpr int doubles_per_level() { return 11; }
 };
@@ -233,8 +241,8 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       // ---- free level f: step with the border multipliers, then the dot products of the next band system ----
       const int f = k - K - 1;
       if (update) {
-        const double lamM = bd.lM[f], lamE0 = energy ? bd.lE[f] : 0.0;
-        const double lamE1 = (energy && f + 1 < F) ? bd.lE[f + 1] : 0.0;
+        const double lamM = bd.lM.get(f), lamE0 = energy ? bd.lE.get(f) : 0.0;
+        const double lamE1 = (energy && f + 1 < F) ? bd.lE.get(f + 1) : 0.0;
         double b[Q], sDx;
         energy_b<Q>(P, v, lane, b, sDx);
 #pragma unroll
@@ -273,19 +281,19 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       if (lane == 0) {
         const double aa = dx * dx * r[1], ab = dx * r[4], aw = dx * r[6];
         if (energy) {
-          bd.dE[f] = aa + (f > 0 ? bb_prev : 0.0);
-          bd.eM[f] = (f > 0) ? -dx * dx * s1_prev : 0.0;       // M_{k-1} . b_{k-1} = dx sum b = -dx^2 sum t
-          bd.eE[f] = (f > 0) ? ab_prev : 0.0;                  // a_{k-1} . b_{k-1}
-          bd.mE[f] = dx * dx * r[0];                           // M_k . a_k
+          bd.dE.set(f, aa + (f > 0 ? bb_prev : 0.0));
+          bd.eM.set(f, (f > 0) ? -dx * dx * s1_prev : 0.0);       // M_{k-1} . b_{k-1} = dx sum b = -dx^2 sum t
+          bd.eE.set(f, (f > 0) ? ab_prev : 0.0);                  // a_{k-1} . b_{k-1}
+          bd.mE.set(f, dx * dx * r[0]);                           // M_k . a_k
           const double jwE = aw + (f > 0 ? bw_prev : 0.0);
-          bd.jw[f] = jwE;
-          bd.rE[f] = hE - jwE - (f == 0 ? bq_K : 0.0);         // h + J^{<=K} d^{<=K} - J^f w ,  d_K = -q'_K
+          bd.jw.set(f, jwE);
+          bd.rE.set(f, hE - jwE - (f == 0 ? bq_K : 0.0));         // h + J^{<=K} d^{<=K} - J^f w ,  d_K = -q'_K
         } else {
-          bd.dE[f] = 1.0; bd.eM[f] = 0.0; bd.eE[f] = 0.0; bd.mE[f] = 0.0; bd.jw[f] = 0.0; bd.rE[f] = 0.0;
+          bd.dE.set(f, 1.0); bd.eM.set(f, 0.0); bd.eE.set(f, 0.0); bd.mE.set(f, 0.0); bd.jw.set(f, 0.0); bd.rE.set(f, 0.0);
         }
-        bd.dM[f] = (double)nx * dx * dx;
-        bd.jw[F + f] = dx * r[5];
-        bd.rM[f] = hM - dx * r[5];
+        bd.dM.set(f, (double)nx * dx * dx);
+        bd.jw.set(F + f, dx * r[5]);
+        bd.rM.set(f, hM - dx * r[5]);
         (void)ab;
       }
       E_prev = E_k; D_prev = D_k; bb_prev = r[3]; ab_prev = dx * r[4]; bw_prev = r[7]; s1_prev = r[0];
@@ -325,24 +333,24 @@ __device__ __forceinline__ bool band_solve(Band bd, int F, double& lam_jw, doubl
   for (int f = 0; f < F; ++f) {
     // row E_f (i = 2f): a2 = eE (to E_{f-1} = row i-2), a1 = eM (to M_{f-1} = row i-1)
     {
-      const double a2 = bd.eE[f], a1 = bd.eM[f], a0 = bd.dE[f];
+      const double a2 = bd.eE.get(f), a1 = bd.eM.get(f), a0 = bd.dE.get(f);
       const double l2 = a2 / Dm2;
       const double l1 = (a1 - l2 * Dm2 * L1m1) / Dm1;
       const double D = a0 - l2 * l2 * Dm2 - l1 * l1 * Dm1;
-      const double y = bd.rE[f] - l1 * ym1 - l2 * ym2;
+      const double y = bd.rE.get(f) - l1 * ym1 - l2 * ym2;
       ok = ok && (D > 0.0) && finite_d(D) && finite_d(y);
-      bd.eE[f] = l2; bd.eM[f] = l1; bd.dE[f] = D; bd.rE[f] = y;
+      bd.eE.set(f, l2); bd.eM.set(f, l1); bd.dE.set(f, D); bd.rE.set(f, y);
       acc = fma(y, y / D, acc);
       Dm2 = Dm1; Dm1 = D; L1m1 = l1; ym2 = ym1; ym1 = y;
     }
     // row M_f (i = 2f+1): a2 = 0 (to M_{f-1}), a1 = mE (to E_f)
     {
-      const double a1 = bd.mE[f], a0 = bd.dM[f];
+      const double a1 = bd.mE.get(f), a0 = bd.dM.get(f);
       const double l1 = a1 / Dm1;
       const double D = a0 - l1 * l1 * Dm1;
-      const double y = bd.rM[f] - l1 * ym1;
+      const double y = bd.rM.get(f) - l1 * ym1;
       ok = ok && (D > 0.0) && finite_d(D) && finite_d(y);
-      bd.mE[f] = l1; bd.dM[f] = D; bd.rM[f] = y;
+      bd.mE.set(f, l1); bd.dM.set(f, D); bd.rM.set(f, y);
       acc = fma(y, y / D, acc);
       Dm2 = Dm1; Dm1 = D; L1m1 = l1; ym2 = ym1; ym1 = y;
     }
@@ -356,21 +364,21 @@ __device__ __forceinline__ bool band_solve(Band bd, int F, double& lam_jw, doubl
   for (int f = F - 1; f >= 0; --f) {
     // row M_f (i = 2f+1): rows above it: i+1 = E_{f+1} (L1 = eM[f+1], L2 = eE[f+1] points to E_f), i+2 = M_{f+1} (L2 = 0)
     {
-      const double x = bd.rM[f] / bd.dM[f] - L1p1 * xp1 - L2p2 * xp2;
-      bd.lM[f] = x;
-      dot = fma(x, bd.jw[F + f], dot);
+      const double x = bd.rM.get(f) / bd.dM.get(f) - L1p1 * xp1 - L2p2 * xp2;
+      bd.lM.set(f, x);
+      dot = fma(x, bd.jw.get(F + f), dot);
       xp2 = xp1; xp1 = x;
       L2p2 = L2p1;              // row i+1 becomes row i+2 of the next (lower) row
-      L1p1 = bd.mE[f]; L2p1 = 0.0;   // this row (M_f) is row i+1 of E_f
+      L1p1 = bd.mE.get(f); L2p1 = 0.0;   // this row (M_f) is row i+1 of E_f
     }
     // row E_f (i = 2f)
     {
-      const double x = bd.rE[f] / bd.dE[f] - L1p1 * xp1 - L2p2 * xp2;
-      bd.lE[f] = x;
-      dot = fma(x, bd.jw[f], dot);
+      const double x = bd.rE.get(f) / bd.dE.get(f) - L1p1 * xp1 - L2p2 * xp2;
+      bd.lE.set(f, x);
+      dot = fma(x, bd.jw.get(f), dot);
       xp2 = xp1; xp1 = x;
       L2p2 = L2p1;
-      L1p1 = bd.eM[f]; L2p1 = bd.eE[f];
+      L1p1 = bd.eM.get(f); L2p1 = bd.eE.get(f);
     }
   }
   lam_jw = dot;
@@ -575,7 +583,7 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
     for (size_t i = lane; i < (size_t)P.m; i += 32) lam[i] = 0.0;
   } else {
     // (after a failed line search the multipliers in lE / lM are those of the last accepted point `cur`)
-    const double lamEK = (P.fk_energy && F > 0) ? bd.lE[0] : 0.0;
+    const double lamEK = (P.fk_energy && F > 0) ? bd.lE.get(0) : 0.0;
     const bool okl = fluxk_local_multipliers<Q, FLUX>(P, lane, pp.first, cur, uh, u0, lamEK, lam);
     if (lane == 0) { pp.rows_rd += 3 * (K + 1); pp.rows_wr += 2 * (K + 1); }
     if (!okl) {
@@ -586,8 +594,8 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
     } else {
       double* lb = lam + (size_t)(K + 1) * nx;
       for (int f = lane; f < F; f += 32) {
-        lb[f] = bd.lM[f];
-        if (P.fk_energy) lb[F + f] = bd.lE[f];
+        lb[f] = bd.lM.get(f);
+        if (P.fk_energy) lb[F + f] = bd.lE.get(f);
       }
       if (cur != ustar) {
         for (size_t i = lane; i < n; i += 32) ustar[i] = cur[i];

@@ -220,13 +220,15 @@ class GpuRun:
         self.norms = torch.empty(self.B, 5, dtype=torch.float64, device=dev)
         self.stats = torch.zeros(self.B, S.STAT_COUNT, dtype=torch.int64, device=dev)
 
+    lam_free = False     # True: multiplier-free calls (lambda = NULL), the sampler-facing variant (Eq. 3)
+
     def step(self, events=None):
         """The whole hot path over one batch of input: `calls` back-to-back snap_project launches."""
         for c, uh in enumerate(self.inputs):
             if events is not None:
                 events[c][0].record()
-            self.S.snap_project(self.p, self.B, uh, self.cdata, self.u_star, self.lam, self.iters[c],
-                                warm=(self.cfg == 5 and c > 0), workspace=self.ws)
+            self.S.snap_project(self.p, self.B, uh, self.cdata, self.u_star, None if self.lam_free else self.lam, self.iters[c],
+                                warm=(self.cfg == 5 and c > 0 and not self.lam_free), workspace=self.ws)
             if events is not None:
                 events[c][1].record()
 
@@ -235,8 +237,8 @@ class GpuRun:
         (deterministic: same inputs, same counts as the timed steps).  Returns algorithmic bytes per call."""
         out = []
         for c, uh in enumerate(self.inputs):
-            self.S.snap_project(self.p, self.B, uh, self.cdata, self.u_star, self.lam, self.iters[c],
-                                warm=(self.cfg == 5 and c > 0), workspace=self.ws)
+            self.S.snap_project(self.p, self.B, uh, self.cdata, self.u_star, None if self.lam_free else self.lam, self.iters[c],
+                                warm=(self.cfg == 5 and c > 0 and not self.lam_free), workspace=self.ws)
             self.S.snap_project_stats(self.p, self.B, self.ws, self.stats)
             torch.cuda.synchronize()
             out.append(algorithmic_bytes(self))
@@ -410,6 +412,21 @@ def run_gpu(args):
         v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5, 6, 7) else max(workers, 16), workers, taus=taus)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "host_cpu_count": cores, "kind": "oracle",
                                 "sample": desc, "seconds": dt}
+    if rank == 0 and world == 1 and args.others:
+        # second line of the same workload: multiplier-free calls (lambda = NULL): no y row, no multiplier sweep, no
+        # min-norm correction; its fraction is quoted against ITS OWN algorithmic bytes
+        run.lam_free = True
+        ms_f, km_f, _ = time_steps(run, args.steps, args.warmup, None)
+        ok_f, hm_f, _ = run.check()
+        ab_f = run.traffic_model()
+        ks_f = sum(sum(k) for k in km_f) * 1e-3
+        rf = roofline_of(run, cfg, ks_f, ab_f, args.steps, peak, peak_src)
+        rf.pop("traffic", None); rf.pop("traffic_note", None); rf.pop("frac_dram", None); rf.pop("dram_over_alg", None)
+        line["lambda_free"] = {"value": run.projections_per_step() * args.steps / (ms_f * 1e-3), "unit": UNIT,
+                               "ms_per_step": ms_f / args.steps, "converged_all": ok_f, "max_hinf_last_call": hm_f,
+                               "alg_bytes_per_projection": sum(ab_f) / (run.B * run.calls), "roofline": rf,
+                               "note": "snap_project(lambda = NULL): u* only, as PCFM's pull-back needs (PAPER.md Eq. 3 L54)"}
+        run.lam_free = False
     if rank == 0 and world == 1 and args.others and cfg == 5:
         others = {}
         for c in (1, 2, 3, 4, 6, 7):

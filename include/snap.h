@@ -156,7 +156,14 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch);
  *   u_hat   dev [batch][nt][ny][nx]  in   point to project.  May alias u_star (in place).
  *   cdata   dev [batch][ny][nx]      in   per-sample initial-condition target u0.
  *   u_star  dev [batch][nt][ny][nx]  out  projected field.
- *   lambda  dev [batch][m]           in/out  multipliers lam*.  If warm != 0 the incoming values are the PCG
+ *   lambda  dev [batch][m] or NULL   in/out  multipliers lam*.  NULL = multiplier-free call (PCFM's pull-back, PAPER.md
+ *                                         Eq. 3, uses u* only): the product-form kernels then skip the y emission, the
+ *                                         multiplier sweep and the min-norm correction (config 5: 40 n instead of 88 n
+ *                                         bytes per projection); u*, status codes are unchanged, `iters` of the 2D
+ *                                         product-form path is one short (the final multiplier linearisation is not run).
+ *                                         Kernels that carry the multipliers in every iteration (classic sweeps, PCG, heat,
+ *                                         kind 5) keep them in the tail of the workspace.
+ *                                         If warm != 0 the incoming values are the PCG
  *                                         initial guess of the 2D kind; the 1D kinds solve
  *                                         directly and ignore them (R2/R3).  The iterate itself
  *                                         always starts at u_hat.
@@ -170,7 +177,7 @@ int snap_project(const snap_problem* p, int batch, const double* u_hat, const do
 
 /* Same computation with HOST buffers (pinned or pageable): copies inputs to a device staging area owned by
  * the handle, runs snap_project, copies u_star / lambda / iters back, and synchronises `stream` before
- * returning.  lambda is read only if warm != 0. */
+ * returning.  lambda is read only if warm != 0; lambda_host == NULL = multiplier-free call (no lambda copy either way). */
 int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, const double* cdata_host,
                       double* u_star_host, double* lambda_host, int* iters_host, int warm, snap_stream stream);
 

@@ -188,6 +188,8 @@ def snap_project(p: Problem, batch: int, u_hat, cdata, u_star, lam, iters, warm:
     for name, t, ne, dt in (("u_hat", u_hat, batch * p.n, torch.float64), ("cdata", cdata, batch * p.nx * p.ny, torch.float64),
                             ("u_star", u_star, batch * p.n, torch.float64), ("lambda", lam, batch * p.m, torch.float64),
                             ("iters", iters, batch, torch.int32)):
+        if t is None and name == "lambda":
+            continue                      # multiplier-free call (include/snap.h)
         _need(t, ne, name, dt)
         if not t.is_cuda:
             raise SnapError(f"{name} must be a CUDA tensor (use snap_project_host for host buffers)")
@@ -206,6 +208,8 @@ def snap_project_host(p: Problem, batch: int, u_hat, cdata, u_star, lam, iters, 
     for name, t, ne, dt in (("u_hat", u_hat, batch * p.n, torch.float64), ("cdata", cdata, batch * p.nx * p.ny, torch.float64),
                             ("u_star", u_star, batch * p.n, torch.float64), ("lambda", lam, batch * p.m, torch.float64),
                             ("iters", iters, batch, torch.int32)):
+        if t is None and name == "lambda":
+            continue
         _need(t, ne, name, dt)
         if t.is_cuda:
             raise SnapError(f"{name} must be a host tensor")

@@ -170,7 +170,7 @@ int project_fluxk(snap_problem* p, int batch, const double* u_hat, const double*
   Proj1dArgs a;
   a.P = d;
   a.batch = batch; a.warm = 0;
-  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
+  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;   // fused path: NULL = no multipliers
   const size_t field = align_up((size_t)batch * d.n * 8, 256);
   a.bufA = reinterpret_cast<double*>(w);
   a.bufB = reinterpret_cast<double*>(w + field);
@@ -318,9 +318,11 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch) {
   if (!p || batch <= 0) return 0;
   const size_t n = (size_t)p->dp.n, B = (size_t)batch;
   const size_t head = 256 + stats_bytes(B);   // alignment slack + work counters
-  if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return head;
-  if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return head + align_up(B * n * 8 * kPcgVectors, 256);
-  return head + align_up(B * n * 8, 256) * 2 + aux_bytes(p, B);
+  // tail: a multiplier array for multiplier-free calls (lambda == NULL) served by a kernel that needs the storage
+  const size_t lam_scratch = align_up(B * (size_t)p->dp.m * 8, 256);
+  if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return head + lam_scratch;
+  if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return head + align_up(B * n * 8 * kPcgVectors, 256) + lam_scratch;
+  return head + align_up(B * n * 8, 256) * 2 + aux_bytes(p, B) + lam_scratch;
 }
 
 int snap_project(const snap_problem* cp, int batch, const double* u_hat, const double* cdata, double* u_star,
@@ -328,15 +330,20 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   snap_problem* p = const_cast<snap_problem*>(cp);
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
-  if (!u_hat || !cdata || !u_star || !lambda || !iters || !workspace) return SNAP_EINVAL;
-  if (workspace_bytes < snap_workspace_bytes(p, batch)) return SNAP_ENOMEM;
+  if (!u_hat || !cdata || !u_star || !iters || !workspace) return SNAP_EINVAL;
+  const size_t need = snap_workspace_bytes(p, batch);
+  if (workspace_bytes < need) return SNAP_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const DevParams& d = p->dp;
   unsigned char* w = ws_base(workspace);
   long long* stats = reinterpret_cast<long long*>(w);
+  // multiplier-free call (lambda == NULL): the product-form kernels skip the multiplier work; the other kernels keep
+  // their multipliers in the tail of the workspace
+  double* const lam_scratch = reinterpret_cast<double*>(w + (need - 256) - align_up((size_t)batch * d.m * 8, 256));
+  double* const lam_any = lambda ? lambda : lam_scratch;
   w += stats_bytes((size_t)batch);
   if (d.kind == SNAP_HEAT1D_IC_MASS) {
-    heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters, stats);
+    heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lam_any, iters, stats);
     return check_launch(p);
   }
   if (d.kind == SNAP_ALLENCAHN2D_IE) {
@@ -344,16 +351,16 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
       const int rc = launch_project2d_direct(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, st);
       if (rc <= 0) return rc;
     }
-    return launch_project2d(p, batch, u_hat, cdata, u_star, lambda, iters, warm, w, stats, st);
+    return launch_project2d(p, batch, u_hat, cdata, u_star, lam_any, iters, lambda ? warm : 0, w, stats, st);
   }
 
-  if (d.kind == SNAP_BURGERS1D_FLUXK) return project_fluxk(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, st);
+  if (d.kind == SNAP_BURGERS1D_FLUXK) return project_fluxk(p, batch, u_hat, cdata, u_star, lam_any, iters, w, stats, st);
   Plan1d pl;
   if (!plan_1d(p, batch, pl)) return SNAP_EINVAL;
   Proj1dArgs a;
   a.P = d;
   a.batch = batch; a.warm = warm;
-  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;
+  a.u_hat = u_hat; a.cdata = cdata; a.u_star = u_star; a.lam = lambda; a.iters = iters;   // fused path: NULL = no multipliers
   const size_t field = align_up((size_t)batch * d.n * 8, 256);
   a.bufA = reinterpret_cast<double*>(w);
   a.bufB = reinterpret_cast<double*>(w + field);
@@ -362,7 +369,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   a.fuse = p->params.gn_fuse;
   // bulk (TMA) copies need every row start 16-byte aligned
   const bool bulk_ok = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
-                       aligned16(lambda) && aligned16(a.bufA);
+                       aligned16(lam_any) && aligned16(a.bufA);
   if (p->params.gn_fuse >= 0 && bulk_ok) {
     Plan1d pf;
     if (plan_fused(p, batch, pf)) {
@@ -372,7 +379,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
                       make_row_map(&a.tm[TM_BUFA], a.bufA, batch, n, n, box) &&
                       make_row_map(&a.tm[TM_BUFB], a.bufB, batch, n, n, box) &&
                       make_row_map(&a.tm[TM_USTAR], u_star, batch, n, n, box) &&
-                      make_row_map(&a.tm[TM_LAM], lambda, batch, n, (size_t)d.m, box);
+                      make_row_map(&a.tm[TM_LAM], lam_any, batch, n, (size_t)d.m, box);
       if (ok) {
         a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
         a.variant = SNAP_VAR_FUSED_TMA;
@@ -383,6 +390,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
     }
   }
   a.nst = pl.nst; a.rp = pl.rp; a.warp_bytes = pl.warp_bytes;
+  a.lam = lam_any;            // the classic sweeps carry the multipliers in every iteration
   pl.tma = bulk_ok;
   if (!pl.tma) pl.full = false;  // the plain-load path is only instantiated with bounds checks
   a.variant = pl.tma ? SNAP_VAR_CLASSIC_BULK : SNAP_VAR_CLASSIC_PLAIN;
@@ -395,7 +403,8 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
                       double* u_star_host, double* lambda_host, int* iters_host, int warm, snap_stream stream) {
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
-  if (!u_hat_host || !cdata_host || !u_star_host || !lambda_host || !iters_host) return SNAP_EINVAL;
+  if (!u_hat_host || !cdata_host || !u_star_host || !iters_host) return SNAP_EINVAL;
+  if (!lambda_host) warm = 0;   // multiplier-free call: lambda is neither read nor returned
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const DevParams& d = p->dp;
   // The batch is cut into chunks of samples (independent blocks) that flow through three
@@ -445,11 +454,12 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
       ok = ok && cudaMemcpyAsync(d_l, lambda_host + (size_t)b0 * d.m, B * d.m * 8, cudaMemcpyHostToDevice, p->s_in) == cudaSuccess;
     ok = ok && cudaEventRecord(p->ev_in[c], p->s_in) == cudaSuccess && cudaStreamWaitEvent(st, p->ev_in[c], 0) == cudaSuccess;
     if (!ok) return SNAP_ECUDA;
-    const int rc = snap_project(p, nb, d_uh, d_c, d_us, d_l, d_i, warm, d_w, b_w, stream);
+    const int rc = snap_project(p, nb, d_uh, d_c, d_us, lambda_host ? d_l : nullptr, d_i, warm, d_w, b_w, stream);
     if (rc != SNAP_OK) return rc;
     ok = cudaEventRecord(p->ev_k[c], st) == cudaSuccess && cudaStreamWaitEvent(p->s_out, p->ev_k[c], 0) == cudaSuccess;
     ok = ok && cudaMemcpyAsync(u_star_host + (size_t)b0 * d.n, d_us, B * d.n * 8, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
-    ok = ok && cudaMemcpyAsync(lambda_host + (size_t)b0 * d.m, d_l, B * d.m * 8, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
+    if (lambda_host)
+      ok = ok && cudaMemcpyAsync(lambda_host + (size_t)b0 * d.m, d_l, B * d.m * 8, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
     ok = ok && cudaMemcpyAsync(iters_host + b0, d_i, B * 4, cudaMemcpyDeviceToHost, p->s_out) == cudaSuccess;
     if (!ok) return SNAP_ECUDA;
   }

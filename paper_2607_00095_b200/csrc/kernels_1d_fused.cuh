@@ -389,7 +389,7 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
         else if (EMIT) q[c] = qc - (vc - uhr[c]);   // y
       }
       if (t < NU) { vL = vnL; vR = vnR; }
-      else if constexpr (kDirect) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
+      else if constexpr (kDirect) { if (yout.p) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q); }
       else store_cells<Q>(so_y, pp.lo, q);
     }
     if constexpr (W == 1) {
@@ -397,10 +397,10 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     }
     if constexpr (kDirect) {
       if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
-      if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + (EMIT ? 1 : 0);
+      if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + ((EMIT && yout.p) ? 1 : 0);
     } else {
       if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
-      pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, EMIT ? yout.tm : nullptr, so_y);
+      pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, (EMIT && yout.p) ? yout.tm : nullptr, so_y);
     }
     // stage s is free: every warp loaded its cells before the first exchange barrier of this level
     if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
@@ -526,10 +526,10 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
         if (t < NU) v[c] -= q[c];
         else if (EMIT) q[c] = q[c] - wv;   // y
       }
-      if (t >= NU) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
+      if (t >= NU && yout.p) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
     }
     if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
-    if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + (EMIT ? 1 : 0);
+    if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + ((EMIT && yout.p) ? 1 : 0);
     if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
     if (++s == nst) s = 0;
   }
@@ -928,7 +928,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   const double* uh = A.u_hat + (size_t)b * n;
   const double* u0 = A.cdata + (size_t)b * nx;
   double* ustar = A.u_star + (size_t)b * n;
-  double* lam = A.lam + (size_t)b * P.m;
+  double* lam = A.lam ? A.lam + (size_t)b * P.m : nullptr;   // nullptr: multiplier-free call (include/snap.h)
   double* bufA = A.bufA + (size_t)b * n;
   double* bufB = A.bufB + (size_t)b * n;
   double* sig = A.aux + (size_t)b * 2 * nt;
@@ -1103,7 +1103,15 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   if (status == SNAP_ST_NONFINITE) {  // R16: u* = u_hat, lam = 0
     if (ustar != uh)
       for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
-    for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
+    if (lam)
+      for (size_t i = gtid; i < (size_t)P.m; i += GT) lam[i] = 0.0;
+  } else if (!lam) {
+    // multiplier-free call: no y emission, no multiplier sweep, no min-norm correction; u* = the final iterate
+    const double* xf = (status == SNAP_ST_LINESEARCH) ? cur : xfin;
+    if (xf != ustar) {
+      for (size_t i = gtid; i < n; i += GT) ustar[i] = xf[i];
+      if (gtid == 0) { pp.rows_rd += nt; pp.rows_wr += nt; }
+    }
   } else {
     if (status == SNAP_ST_LINESEARCH) {   // multiplier at the last accepted iterate (as the oracle returns it)
       fused_fwd_dispatch<KIND, W, Q, JT>(P, pp, mk(cur), mk(uh), u0, Buf{nullptr, nullptr}, mk(lam), 0, 1, M0, S);

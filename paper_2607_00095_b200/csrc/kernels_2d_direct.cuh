@@ -415,7 +415,7 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
   const double* uh = A.u_hat + (size_t)b * n;
   const double* u0 = A.cdata + (size_t)b * L;
   double* ustar = A.u_star + (size_t)b * n;
-  double* lam = A.lam + (size_t)b * n;
+  double* lam = A.lam ? A.lam + (size_t)b * n : nullptr;   // nullptr: multiplier-free call
   double* ws = A.ws + (size_t)b * kPcgVectors * n;
   double* const buf[3] = {ws, ws + n, ws + 2 * n};
 
@@ -439,6 +439,13 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
   Pass2d S;
 
   while (true) {
+    if (!lam && have_trial && polishing && polish_left == 0) {
+      // multiplier-free call: the last polish step is accepted without a test (R4) and nothing is computed at the
+      // polished point (no y, no multiplier), so its pass is not run: `iters` is one linearisation short of a call with lam
+      cur = trial;
+      have_trial = false;
+      break;
+    }
     const double* pt = have_trial ? trial : cur;
     double* out = buf[0];
     if (out == pt || out == cur) out = buf[1];
@@ -447,7 +454,7 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     // evaluates is final (last polish step done) or may turn out to be (quadratic convergence: ||h|| ~ hprev^2 < tol),
     // and then the level solves run to rounding.
     const bool last = polishing && polish_left == 0;
-    const bool emit_y = last || hprev * hprev < 100.0 * P.tol;
+    const bool emit_y = lam && (last || hprev * hprev < 100.0 * P.tol);
     const int ns = (polishing || emit_y) ? A.ns_exact : sweeps_for(hprev);
     fwd_pass2d<PR>(P, g, ring, xpl, qpl, red, pt, uh, u0, last ? nullptr : out, emit_y ? lam : nullptr, ost, ns, active,
                    nwarp, S);
@@ -504,7 +511,14 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     have_trial = true;
   }
 
-  if (status == SNAP_ST_LINESEARCH || (status != SNAP_ST_NONFINITE && !have_y)) {
+  if (!lam) {
+    // multiplier-free call: u* = the returned iterate, nothing else to do
+    if (status != SNAP_ST_NONFINITE && cur != ustar) {
+      __syncthreads();
+      for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = cur[i];
+      rows_rd += nt; rows_wr += nt;
+    }
+  } else if (status == SNAP_ST_LINESEARCH || (status != SNAP_ST_NONFINITE && !have_y)) {
     // the returned point was not known to be final when its pass ran (feasible input, polish skipped or 0, max_iter,
     // line search): right-hand side of the multiplier solve there, level solves to rounding
     fwd_pass2d<PR>(P, g, ring, xpl, qpl, red, cur, uh, u0, nullptr, lam, ost, A.ns_exact, active, nwarp, S);
@@ -512,7 +526,7 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     rows_rd += 2 * nt; rows_wr += nt;
     if (S.bad || !finite_d(S.dd)) status = SNAP_ST_NONFINITE;
   }
-  if (status != SNAP_ST_NONFINITE) {
+  if (lam && status != SNAP_ST_NONFINITE) {
     const bool late_copy = (ustar == uh) && (cur != ustar);   // in place: u_hat survives until lam is known finite
     double* ucopy = (cur != ustar && !late_copy) ? ustar : nullptr;
     const double chk = bwd_pass2d<PR>(P, g, ring, qpl, red, cur, lam, ucopy, A.ns_exact, active, nwarp);
@@ -529,7 +543,8 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     __syncthreads();
     if (ustar != uh)
       for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = uh[i];
-    for (size_t i = tid; i < n; i += blockDim.x) lam[i] = 0.0;
+    if (lam)
+      for (size_t i = tid; i < n; i += blockDim.x) lam[i] = 0.0;
   }
   if (tid == 0) {
     A.iters[b] = (status == 0) ? solves : status;

@@ -316,6 +316,58 @@ def test_pcg_preconditioners_agree(S, precond):
     check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
 
 
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5, 6])
+def test_multiplier_free_call_returns_the_same_projection(S, cfg):
+    """lambda == NULL (include/snap.h; PCFM's pull-back uses u_1 only, Eq. 3): same u*, same status, fewer
+    rows moved on the product-form paths (no y row, no multiplier sweep, no min-norm correction)."""
+    dev = torch.device("cuda:0")
+    shapes = {1: dict(batch=3, nx=20, nt=12), 2: dict(batch=3, nx=64, nt=20), 3: dict(batch=3, nx=64, nt=17),
+              4: dict(batch=2, nx=16, ny=16, nt=5), 5: dict(batch=3, nx=64, nt=33), 6: dict(batch=2, nx=64, nt=16)}
+    for prm in ({}, dict(gn_fuse=-1)):
+        wl = W.make_workload(cfg, **shapes[cfg])
+        ref = gpu_project(S, wl, wl.u_hat, params=prm)
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, dict(wl.params, **prm))
+        B = wl.batch
+        uh = wl.u_hat.to(dev)
+        us = torch.full_like(uh, float("nan"))
+        it = torch.full((B,), -99, dtype=torch.int32, device=dev)
+        ws = S.snap_project(p, B, uh, wl.cdata.to(dev), us, None, it)
+        st = torch.zeros(B, S.STAT_COUNT, dtype=torch.int64, device=dev)
+        S.snap_project_stats(p, B, ws, st)
+        ws2 = S.snap_project(p, B, uh, wl.cdata.to(dev), torch.empty_like(uh), torch.zeros(B, p.m, dtype=torch.float64, device=dev), it.clone(), workspace=ws)
+        st2 = torch.zeros(B, S.STAT_COUNT, dtype=torch.int64, device=dev)
+        S.snap_project_stats(p, B, ws2, st2)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(us.cpu().numpy().reshape(ref["u"].shape), ref["u"])
+        direct2d = (cfg == 4 and not prm)
+        np.testing.assert_array_equal(it.cpu().numpy(), ref["iters"] - (1 if direct2d else 0))
+        st, st2 = st.cpu().numpy(), st2.cpu().numpy()
+        moved = st[:, S.STAT_ROWS_READ] + st[:, S.STAT_ROWS_WRITTEN]
+        moved2 = st2[:, S.STAT_ROWS_READ] + st2[:, S.STAT_ROWS_WRITTEN]
+        if st2[0, S.STAT_VARIANT] in (S.VAR_FUSED_TMA, S.VAR_DIRECT2D):
+            assert (moved < moved2).all(), (cfg, prm, moved, moved2)
+        else:
+            assert (moved == moved2).all()
+        # in place
+        inp = uh.clone()
+        S.snap_project(p, B, inp, wl.cdata.to(dev), inp, None, it, workspace=ws)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(inp.cpu().numpy().reshape(ref["u"].shape), ref["u"])
+        p.destroy()
+
+
+def test_multiplier_free_host_call(S):
+    wl = W.make_workload(5, batch=130, nx=32, nt=9)
+    ref = gpu_project(S, wl, wl.u_hat)
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    us = torch.empty_like(wl.u_hat).pin_memory()
+    it = torch.empty(wl.batch, dtype=torch.int32).pin_memory()
+    S.snap_project_host(p, wl.batch, wl.u_hat.contiguous().pin_memory(), wl.cdata.contiguous(), us, None, it)
+    np.testing.assert_array_equal(us.numpy().reshape(ref["u"].shape), ref["u"])
+    np.testing.assert_array_equal(it.numpy(), ref["iters"])
+    p.destroy()
+
+
 def test_direct2d_matches_oracle_and_pcg_path(S):
     """Kind 3, product-form path (in-SMEM red-black level solves): same limit point as the oracle
     and as the PCG kernel (gn_fuse = -1) on 2-row and 4-row patches, one and several warps, nt = 2."""

@@ -30,3 +30,4 @@ from .linsolve import (  # noqa: F401
     min_norm_multiplier,
 )
 from .project import project, project_batch  # noqa: F401
+from .flow import flow_step  # noqa: F401

@@ -175,6 +175,22 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch);
 int snap_project(const snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                  double* lambda, int* iters, int warm, void* workspace, size_t workspace_bytes, snap_stream stream);
 
+/* One PCFM sampling step around the projection (§III-A, Eq. 1-3), one launch
+ * where the product-form kernels serve the problem (fused 1D path with one warp per sample, 2D product-form path):
+ *     u_hat_1 = u_tau + (1 - tau) vel          Eq. 1, formed by the projection's first pass, written IN PLACE over u_tau
+ *     u_1     = argmin 1/2 ||u - u_hat_1||^2 s.t. h(u) = 0     Eq. 2 = snap_project
+ *     u_next  = u_prior + tau_next (u_1 - u_prior)             Eq. 3, written by the pass that streams the final iterate
+ *   u_tau   dev [batch][n]  in: state at flow time tau; out: u_hat_1
+ *   vel     dev [batch][n]  in: values of the flow model's velocity v_theta(u_tau, tau) (the model itself is the caller's)
+ *   u_prior dev [batch][n]  in: the prior sample u_0 of the OT interpolant
+ *   u1      dev [batch][n]  out: projected field;  u_next dev [batch][n] out;  the five field buffers must be distinct
+ *   lambda  dev [batch][m] or NULL (multiplier-free step: what a sampler needs);  iters, workspace as snap_project.
+ * Other kernels (classic sweeps, PCG, heat, kind 5) run Eq. 1 and Eq. 3 as two elementwise launches around theirs.
+ * 0 <= tau, tau_next <= 1, else SNAP_EINVAL. */
+int snap_flow_step(const snap_problem* p, int batch, double* u_tau, const double* vel, const double* u_prior, double tau,
+                   double tau_next, const double* cdata, double* u1, double* u_next, double* lambda, int* iters,
+                   void* workspace, size_t workspace_bytes, snap_stream stream);
+
 /* Same computation with HOST buffers (pinned or pageable): copies inputs to a device staging area owned by
  * the handle, runs snap_project, copies u_star / lambda / iters back, and synchronises `stream` before
  * returning.  lambda is read only if warm != 0; lambda_host == NULL = multiplier-free call (no lambda copy either way). */

@@ -18,7 +18,7 @@ HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS, BU
 EXPORTS = [
     "snap_params_default", "snap_problem_create", "snap_problem_destroy", "snap_num_unknowns", "snap_num_rows",
     "snap_workspace_bytes", "snap_project", "snap_project_host", "snap_residual", "snap_schur_apply",
-    "snap_project_stats", "snap_launch_count", "snap_strerror",
+    "snap_project_stats", "snap_launch_count", "snap_strerror", "snap_flow_step",
 ]
 
 
@@ -74,6 +74,8 @@ def load_library():
     lib.snap_workspace_bytes.restype = C.c_size_t
     lib.snap_project.argtypes = [vp, C.c_int, dp, dp, dp, dp, ip, C.c_int, vp, C.c_size_t, vp]
     lib.snap_project.restype = C.c_int
+    lib.snap_flow_step.argtypes = [vp, C.c_int, dp, dp, dp, C.c_double, C.c_double, dp, dp, dp, dp, ip, vp, C.c_size_t, vp]
+    lib.snap_flow_step.restype = C.c_int
     lib.snap_project_host.argtypes = [vp, C.c_int, dp, dp, dp, dp, ip, C.c_int, vp]
     lib.snap_project_host.restype = C.c_int
     lib.snap_residual.argtypes = [vp, C.c_int, dp, dp, dp, dp, vp]
@@ -199,6 +201,29 @@ def snap_project(p: Problem, batch: int, u_hat, cdata, u_star, lam, iters, warm:
     rc = load_library().snap_project(p.handle, int(batch), _ptr(u_hat), _ptr(cdata), _ptr(u_star), _ptr(lam), _ptr(iters),
                                      int(bool(warm)), _ptr(workspace), _nbytes(workspace), _stream_handle(stream))
     _check(rc, "snap_project")
+    return workspace
+
+
+def snap_flow_step(p: Problem, batch: int, u_tau, vel, u_prior, tau: float, tau_next: float, cdata, u1, u_next, lam, iters,
+                   workspace=None, stream=None):
+    """Enqueue one PCFM step (Eq. 1 shoot, Eq. 2 projection, Eq. 3 pull-back; include/snap.h).  `u_tau` is overwritten
+    by u_hat_1; `lam` may be None (multiplier-free step)."""
+    import torch
+    for name, t, ne, dt in (("u_tau", u_tau, batch * p.n, torch.float64), ("vel", vel, batch * p.n, torch.float64),
+                            ("u_prior", u_prior, batch * p.n, torch.float64), ("cdata", cdata, batch * p.nx * p.ny, torch.float64),
+                            ("u1", u1, batch * p.n, torch.float64), ("u_next", u_next, batch * p.n, torch.float64),
+                            ("lambda", lam, batch * p.m, torch.float64), ("iters", iters, batch, torch.int32)):
+        if t is None and name == "lambda":
+            continue
+        _need(t, ne, name, dt)
+        if not t.is_cuda:
+            raise SnapError(f"{name} must be a CUDA tensor")
+    if workspace is None:
+        workspace = torch.empty(snap_workspace_bytes(p, batch), dtype=torch.uint8, device=u_tau.device)
+    rc = load_library().snap_flow_step(p.handle, int(batch), _ptr(u_tau), _ptr(vel), _ptr(u_prior), float(tau), float(tau_next),
+                                       _ptr(cdata), _ptr(u1), _ptr(u_next), _ptr(lam), _ptr(iters), _ptr(workspace),
+                                       _nbytes(workspace), _stream_handle(stream))
+    _check(rc, "snap_flow_step")
     return workspace
 
 

@@ -177,6 +177,7 @@ int project_fluxk(snap_problem* p, int batch, const double* u_hat, const double*
   a.aux = reinterpret_cast<double*>(w + 2 * field);
   a.stats = stats;
   a.fuse = 0;
+  a.vel = nullptr; a.u_prior = nullptr; a.u_next = nullptr; a.omt = 0.0; a.taun = 0.0;
   const int box = d.nx / 16;
   const size_t n = (size_t)d.n;
   if (!(make_row_map(&a.tm[TM_UHAT], u_hat, batch, n, n, box) && make_row_map(&a.tm[TM_BUFA], a.bufA, batch, n, n, box) &&
@@ -325,8 +326,25 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch) {
   return head + align_up(B * n * 8, 256) * 2 + aux_bytes(p, B) + lam_scratch;
 }
 
-int snap_project(const snap_problem* cp, int batch, const double* u_hat, const double* cdata, double* u_star,
-                 double* lambda, int* iters, int warm, void* workspace, size_t workspace_bytes, snap_stream stream) {
+namespace {
+// Eq. 1 / Eq. 3 as separate elementwise launches (projection kernels that do not fuse them)
+int flow_unfused_shoot(snap_problem* p, int batch, const double* u_hat, const FlowArgs* flow, cudaStream_t st) {
+  if (!flow) return SNAP_OK;
+  const size_t total = (size_t)batch * p->dp.n;
+  flow_shoot_kernel<<<p->sm_count * 4, kMiscThreads, 0, st>>>(total, const_cast<double*>(u_hat), flow->vel, flow->omt);
+  return check_launch(p);
+}
+int flow_unfused_pullback(snap_problem* p, int batch, const double* u_star, const FlowArgs* flow, cudaStream_t st) {
+  if (!flow) return SNAP_OK;
+  const size_t total = (size_t)batch * p->dp.n;
+  flow_pullback_kernel<<<p->sm_count * 4, kMiscThreads, 0, st>>>(total, u_star, flow->u_prior, flow->u_next, flow->taun);
+  return check_launch(p);
+}
+}  // namespace
+
+static int project_impl(const snap_problem* cp, int batch, const double* u_hat, const double* cdata, double* u_star,
+                        double* lambda, int* iters, int warm, void* workspace, size_t workspace_bytes, snap_stream stream,
+                        const FlowArgs* flow) {
   snap_problem* p = const_cast<snap_problem*>(cp);
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
@@ -343,18 +361,29 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   double* const lam_any = lambda ? lambda : lam_scratch;
   w += stats_bytes((size_t)batch);
   if (d.kind == SNAP_HEAT1D_IC_MASS) {
+    int rc = flow_unfused_shoot(p, batch, u_hat, flow, st);
+    if (rc != SNAP_OK) return rc;
     heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lam_any, iters, stats);
-    return check_launch(p);
+    rc = check_launch(p);
+    return rc != SNAP_OK ? rc : flow_unfused_pullback(p, batch, u_star, flow, st);
   }
   if (d.kind == SNAP_ALLENCAHN2D_IE) {
     if (p->params.gn_fuse >= 0) {   // product-form path (in-SMEM level solves) where the shape and parameters allow it
-      const int rc = launch_project2d_direct(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, st);
+      const int rc = launch_project2d_direct(p, batch, u_hat, cdata, u_star, lambda, iters, w, stats, flow, st);
       if (rc <= 0) return rc;
     }
-    return launch_project2d(p, batch, u_hat, cdata, u_star, lam_any, iters, lambda ? warm : 0, w, stats, st);
+    int rc = flow_unfused_shoot(p, batch, u_hat, flow, st);
+    if (rc != SNAP_OK) return rc;
+    rc = launch_project2d(p, batch, u_hat, cdata, u_star, lam_any, iters, lambda ? warm : 0, w, stats, st);
+    return rc != SNAP_OK ? rc : flow_unfused_pullback(p, batch, u_star, flow, st);
   }
 
-  if (d.kind == SNAP_BURGERS1D_FLUXK) return project_fluxk(p, batch, u_hat, cdata, u_star, lam_any, iters, w, stats, st);
+  if (d.kind == SNAP_BURGERS1D_FLUXK) {
+    int rc = flow_unfused_shoot(p, batch, u_hat, flow, st);
+    if (rc != SNAP_OK) return rc;
+    rc = project_fluxk(p, batch, u_hat, cdata, u_star, lam_any, iters, w, stats, st);
+    return rc != SNAP_OK ? rc : flow_unfused_pullback(p, batch, u_star, flow, st);
+  }
   Plan1d pl;
   if (!plan_1d(p, batch, pl)) return SNAP_EINVAL;
   Proj1dArgs a;
@@ -367,6 +396,7 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   a.aux = reinterpret_cast<double*>(w + 2 * field);
   a.stats = stats;
   a.fuse = p->params.gn_fuse;
+  a.vel = nullptr; a.u_prior = nullptr; a.u_next = nullptr; a.omt = 0.0; a.taun = 0.0;
   // bulk (TMA) copies need every row start 16-byte aligned
   const bool bulk_ok = (d.nx % 2 == 0) && (d.m % 2 == 0 || batch == 1) && aligned16(u_hat) && aligned16(u_star) &&
                        aligned16(lam_any) && aligned16(a.bufA);
@@ -380,7 +410,12 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
                       make_row_map(&a.tm[TM_BUFB], a.bufB, batch, n, n, box) &&
                       make_row_map(&a.tm[TM_USTAR], u_star, batch, n, n, box) &&
                       make_row_map(&a.tm[TM_LAM], lam_any, batch, n, (size_t)d.m, box);
-      if (ok) {
+      // PCFM step: one warp per sample fuses Eq. 1 into the first pass and Eq. 3 into the multiplier sweep
+      const bool fuse_flow = flow && pf.wps == 1 && aligned16(flow->vel) && aligned16(flow->u_prior) && aligned16(flow->u_next);
+      bool okf = ok;
+      if (okf && fuse_flow) okf = make_row_map(&a.tm[TM_VEL], flow->vel, batch, n, n, box);
+      if (okf && (!flow || fuse_flow)) {
+        if (flow) { a.vel = flow->vel; a.u_prior = flow->u_prior; a.u_next = flow->u_next; a.omt = flow->omt; a.taun = flow->taun; }
         a.nst = pf.nst; a.rp = pf.rp; a.warp_bytes = pf.warp_bytes;
         a.variant = SNAP_VAR_FUSED_TMA;
         p->launches++;
@@ -394,9 +429,32 @@ int snap_project(const snap_problem* cp, int batch, const double* u_hat, const d
   pl.tma = bulk_ok;
   if (!pl.tma) pl.full = false;  // the plain-load path is only instantiated with bounds checks
   a.variant = pl.tma ? SNAP_VAR_CLASSIC_BULK : SNAP_VAR_CLASSIC_PLAIN;
+  int rc = flow_unfused_shoot(p, batch, u_hat, flow, st);
+  if (rc != SNAP_OK) return rc;
   p->launches++;
-  if (d.kind == SNAP_FISHER1D_IE) return launch_project1d_fisher(a, pl, st);
-  return launch_project1d_burgers(a, pl, st);
+  rc = (d.kind == SNAP_FISHER1D_IE) ? launch_project1d_fisher(a, pl, st) : launch_project1d_burgers(a, pl, st);
+  return rc != SNAP_OK ? rc : flow_unfused_pullback(p, batch, u_star, flow, st);
+}
+
+int snap_project(const snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
+                 double* lambda, int* iters, int warm, void* workspace, size_t workspace_bytes, snap_stream stream) {
+  return project_impl(p, batch, u_hat, cdata, u_star, lambda, iters, warm, workspace, workspace_bytes, stream, nullptr);
+}
+
+int snap_flow_step(const snap_problem* p, int batch, double* u_tau, const double* vel, const double* u_prior, double tau,
+                   double tau_next, const double* cdata, double* u1, double* u_next, double* lambda, int* iters,
+                   void* workspace, size_t workspace_bytes, snap_stream stream) {
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u_tau || !vel || !u_prior || !u1 || !u_next) return SNAP_EINVAL;
+  if (!(tau >= 0.0 && tau <= 1.0 && tau_next >= 0.0 && tau_next <= 1.0)) return SNAP_EINVAL;
+  // the buffers of a step are distinct: u_tau is overwritten by u_hat_1 while u1 / u_next are being produced
+  if (u1 == u_tau || u_next == u_tau || u_next == u1 || u_prior == u_tau || u_prior == u1 || u_prior == u_next ||
+      vel == u_tau || vel == u1 || vel == u_next)
+    return SNAP_EINVAL;
+  FlowArgs f;
+  f.vel = vel; f.u_prior = u_prior; f.u_next = u_next; f.omt = 1.0 - tau; f.taun = tau_next;
+  return project_impl(p, batch, u_tau, cdata, u1, lambda, iters, 0, workspace, workspace_bytes, stream, &f);
 }
 
 int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, const double* cdata_host,

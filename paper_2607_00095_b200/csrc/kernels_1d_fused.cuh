@@ -116,6 +116,21 @@ __device__ __forceinline__ void store_cells_global(double* __restrict__ g, const
   }
 }
 
+// a lane's Q contiguous cells from global memory (128-bit loads)
+template <int Q>
+__device__ __forceinline__ void load_cells_global(const double* __restrict__ g, double (&x)[Q]) {
+  if constexpr (Q == 1) {
+    x[0] = g[0];
+  } else {
+#pragma unroll
+    for (int c = 0; c < Q / 2; ++c) {
+      const double2 t = reinterpret_cast<const double2*>(g)[c];
+      x[2 * c] = t.x;
+      x[2 * c + 1] = t.y;
+    }
+  }
+}
+
 __device__ __forceinline__ double shfl_prev(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 31) & 31); }
 __device__ __forceinline__ double shfl_next(double v, int lane) { return __shfl_sync(SNAP_FULL, v, (lane + 1) & 31); }
 
@@ -177,6 +192,12 @@ struct RowPipe {
   int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
   LaneOff<Q> lo;
   long long rows_rd, rows_wr;        // HBM rows requested (counted once per group): the traffic this variant needs
+  // PCFM step (snap_flow_step): vel_tm != nullptr marks the pass that forms u_hat = u_tau + omt vel on the fly (Eq. 1);
+  // unext != nullptr makes the pass that streams the final iterate also write u_0 + taun (u* - u_0) (Eq. 3)
+  const CUtensorMap* vel_tm;
+  double omt, taun;
+  const double* uprior;
+  double* unext;
 
   __device__ __forceinline__ double* row(int s, int r) const { return stage + (size_t)(s * 2 + r) * G::RP; }
   __device__ __forceinline__ double* out(int r) const { return orow + (size_t)r * G::RP; }
@@ -265,7 +286,9 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
   const int wl = (w + W - 1) % W, wr = (w + 1) % W;
   // cells just outside this warp's range (periodic), read by lane 0 / lane 31 for iteration 0
   const int cellL = swz_idx((first + nx - 1) % nx), cellR = swz_idx((first + Q) % nx);
-  const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
+  bool shoot = false;
+  if constexpr (W == 1) shoot = (pp.vel_tm != nullptr);   // x0 holds u_tau: this pass forms u_hat (Eq. 1) in place
+  const CUtensorMap* const tm_uh = shoot ? pp.vel_tm : (same ? nullptr : uh.tm);
 
   double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
   double h1[T], wd[T], dd[T];              // per-lane partial sums (thread 0 of the group also takes the mass rows)
@@ -320,6 +343,18 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     const double* r0 = pp.row(s, 0);
     const double* ruh = same ? r0 : pp.row(s, 1);   // u_hat cells are re-read where needed
     load_cells<Q>(r0, pp.lo, v);
+    if constexpr (W == 1) {
+      if (shoot) {   // u_hat = u_tau + (1 - tau) v_theta: to global (in place over u_tau) and back into the stage row,
+                     // which later iterations of this level re-read as the u_hat row
+        double vv[Q];
+        load_cells<Q>(pp.row(s, 1), pp.lo, vv);
+#pragma unroll
+        for (int c = 0; c < Q; ++c) v[c] = fma(pp.omt, vv[c], v[c]);
+        store_cells<Q>(pp.row(s, 0), pp.lo, v);
+        store_cells_global<Q>(uh.p + (size_t)k * nx + first, v);
+        if (lane == 0) pp.rows_wr += 1;
+      }
+    }
     double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
     if constexpr (W > 1) {
       if (lane == 0) vL = r0[cellL];
@@ -465,7 +500,8 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
   const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
   const double fa = P.fi_a, fr = P.fi_dtrho;
   const bool same = (x0.p == uh.p);
-  const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
+  const bool shoot = (pp.vel_tm != nullptr);   // see fused_fwd_body
+  const CUtensorMap* const tm_uh = shoot ? pp.vel_tm : (same ? nullptr : uh.tm);
   const double tol = P.tol, skip = kPolishSkip * P.tol;
 
   double qo[T][Q], xp[T][Q];   // q_{k-1} and x_t[k-1] of iteration t, own cells
@@ -491,6 +527,15 @@ __device__ __forceinline__ void fused_fwd_f_body(const DevParams& P, RowPipe<1, 
     const double* r0 = pp.row(s, 0);
     const double* ruh = same ? r0 : pp.row(s, 1);
     load_cells<Q>(r0, pp.lo, v);
+    if (shoot) {
+      double vv[Q];
+      load_cells<Q>(pp.row(s, 1), pp.lo, vv);
+#pragma unroll
+      for (int c = 0; c < Q; ++c) v[c] = fma(pp.omt, vv[c], v[c]);
+      store_cells<Q>(pp.row(s, 0), pp.lo, v);
+      store_cells_global<Q>(uh.p + (size_t)k * nx + first, v);
+      if (lane == 0) pp.rows_wr += 1;
+    }
 #pragma unroll
     for (int t = 0; t < T; ++t) {
       double q[Q], uhr[Q], hv[Q];
@@ -566,9 +611,14 @@ __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp
   double chk = 0.0;
   const int npro = nst < nt ? nst : nt;
   for (int t = 0; t < npro; ++t) pp.issue(t, nt - 1 - t, lam.tm, x.tm);
+  // OT pull-back fused into this sweep (Eq. 3): the prior row of the next level travels while this one is computed
+  const bool pull = pp.unext != nullptr;
+  double upc[Q], upn[Q];
+  if (pull) load_cells_global<Q>(pp.uprior + (size_t)(nt - 1) * nx + first, upc);
   int s = 0;
   for (int t = 0; t < nt; ++t) {
     const int k = nt - 1 - t;
+    if (pull && k > 0) load_cells_global<Q>(pp.uprior + (size_t)(k - 1) * nx + first, upn);
     pp.wait(s);
     double l[Q], v[Q];
     load_cells<Q>(pp.row(s, 0), pp.lo, l);
@@ -585,6 +635,14 @@ __device__ __noinline__ double fused_bwd_f(const DevParams& P, RowPipe<1, Q>& pp
     store_cells_global<Q>(lam.p + (size_t)k * nx + first, l);
     if (ucopy) store_cells_global<Q>(ucopy + (size_t)k * nx + first, v);
     if (lane == 0) pp.rows_wr += ucopy ? 2 : 1;
+    if (pull) {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) { upc[c] = fma(pp.taun, v[c] - upc[c], upc[c]); }
+      store_cells_global<Q>(pp.unext + (size_t)k * nx + first, upc);
+#pragma unroll
+      for (int c = 0; c < Q; ++c) upc[c] = upn[c];
+      if (lane == 0) { pp.rows_rd += 1; pp.rows_wr += 1; }
+    }
     if (t + nst < nt) pp.issue(s, k - nst, lam.tm, x.tm);
     if (++s == nst) s = 0;
   }
@@ -659,9 +717,15 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
   double lL = 0.0, lR = 0.0, chk = 0.0, lsum_prev = 0.0;
   const int npro = nst < nt ? nst : nt;
   for (int t = 0; t < npro; ++t) pp.issue(t, nt - 1 - t, lam.tm, x.tm);
+  // OT pull-back fused into this sweep (Eq. 3; W = 1): the prior row of the next level travels while this one is computed
+  bool pull = false;
+  if constexpr (W == 1) pull = pp.unext != nullptr;
+  double upc[Q], upn[Q];
+  if (pull) load_cells_global<Q>(pp.uprior + (size_t)(nt - 1) * nx + first, upc);
   int s = 0, par = 0;
   for (int t = 0; t < nt; ++t) {
     const int k = nt - 1 - t;
+    if (pull && k > 0) load_cells_global<Q>(pp.uprior + (size_t)(k - 1) * nx + first, upn);
     pp.wait(s);
     double yv[Q], v[Q], l[Q];
     load_cells<Q>(pp.row(s, 0), pp.lo, yv);
@@ -707,6 +771,14 @@ __device__ __noinline__ double fused_bwd(const DevParams& P, RowPipe<W, Q>& pp_r
       store_cells_global<Q>(lam.p + (size_t)k * nx + first, l);
       if (ucopy_p) store_cells_global<Q>(ucopy_p + (size_t)k * nx + first, v);
       if (lane == 0) pp.rows_wr += ucopy_p ? 2 : 1;
+      if (pull) {
+#pragma unroll
+        for (int c = 0; c < Q; ++c) upc[c] = fma(pp.taun, v[c] - upc[c], upc[c]);
+        store_cells_global<Q>(pp.unext + (size_t)k * nx + first, upc);
+#pragma unroll
+        for (int c = 0; c < Q; ++c) upc[c] = upn[c];
+        if (lane == 0) { pp.rows_rd += 1; pp.rows_wr += 1; }
+      }
     } else {
       double* so_l = pp.out(t & 1);
       double* so_u = pp.out(2 + (t & 1));
@@ -918,6 +990,8 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.b = b;
   pp.lo.init(pp.first);
   pp.rows_rd = 0; pp.rows_wr = 0;
+  pp.vel_tm = nullptr; pp.omt = A.omt; pp.taun = A.taun;
+  pp.uprior = nullptr; pp.unext = nullptr;    // armed below, around the pass that streams the final iterate
   if (gtid == 0) {
     for (int s = 0; s < A.nst; ++s) mbar_init(pp.bar0 + 8u * s, 1);
     mbar_fence_init();
@@ -986,7 +1060,9 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     if (J > JT - 1 && (sweeps > 0 || conv || jcap < JT || x0 != uh)) J = JT - 1;   // the JT-update shape assumes x_0 == u_hat
     if (J < 0) J = 0;
     const int T = (J < JT) ? J + 1 : J;
+    if (A.vel && sweeps == 0) pp.vel_tm = &A.tm[TM_VEL];   // PCFM step: the first pass reads u_tau and forms u_hat (Eq. 1)
     fused_fwd_dispatch<KIND, W, Q, JT>(P, pp, mk(x0), mk(uh), u0, mk(xo), mk(lam), J, T, M0, S);
+    pp.vel_tm = nullptr;
     ++sweeps;
 
     // ---- a pending step is judged by iteration 0 of this pass ---------------------------------------------
@@ -1100,6 +1176,9 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   }
 
   long long* stat = A.stats ? A.stats + (size_t)b * SNAP_STAT_COUNT : nullptr;
+  const double* const up_b = A.u_next ? A.u_prior + (size_t)b * n : nullptr;   // PCFM pull-back (Eq. 3) wanted
+  double* const un_b = A.u_next ? A.u_next + (size_t)b * n : nullptr;
+  bool pulled = false;
   if (status == SNAP_ST_NONFINITE) {  // R16: u* = u_hat, lam = 0
     if (ustar != uh)
       for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
@@ -1108,7 +1187,15 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   } else if (!lam) {
     // multiplier-free call: no y emission, no multiplier sweep, no min-norm correction; u* = the final iterate
     const double* xf = (status == SNAP_ST_LINESEARCH) ? cur : xfin;
-    if (xf != ustar) {
+    if (un_b) {          // one stream: u* (if it is not in place already) and the pull-back
+      for (size_t i = gtid; i < n; i += GT) {
+        const double x = xf[i], u0p = up_b[i];
+        if (xf != ustar) ustar[i] = x;
+        un_b[i] = fma(A.taun, x - u0p, u0p);
+      }
+      pulled = true;
+      if (gtid == 0) { pp.rows_rd += 2 * nt; pp.rows_wr += nt + (xf != ustar ? nt : 0); }
+    } else if (xf != ustar) {
       for (size_t i = gtid; i < n; i += GT) ustar[i] = xf[i];
       if (gtid == 0) { pp.rows_rd += nt; pp.rows_wr += nt; }
     }
@@ -1124,8 +1211,10 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     const bool late_copy = (ustar == uh) && (xfin != ustar);
     const CUtensorMap* const tm_copy = (xfin != ustar && !late_copy) ? &A.tm[TM_USTAR] : nullptr;
     double chk;
+    if (un_b && W == 1 && !late_copy && status == 0) { pp.uprior = up_b; pp.unext = un_b; pulled = true; }
     if constexpr (KIND == KF_FUSED) chk = fused_bwd_f<Q>(P, pp, mk(xfin), mk(lam), tm_copy ? ustar : nullptr);
     else chk = fused_bwd<W, Q>(P, pp, mk(xfin), mk(lam), tm_copy, tm_copy ? ustar : nullptr, want_sig ? sig : nullptr);
+    pp.uprior = nullptr; pp.unext = nullptr;
     ++sweeps;
     if (finite_d(chk) && late_copy) {
       for (size_t i = gtid; i < n; i += GT) ustar[i] = xfin[i];
@@ -1133,6 +1222,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     }
     if (!finite_d(chk)) {
       status = SNAP_ST_NONFINITE;
+      pulled = false;
       pp.gsync();
       if (ustar != uh)
         for (size_t i = gtid; i < n; i += GT) ustar[i] = uh[i];
@@ -1152,6 +1242,15 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
         for (int k = gtid; k < nt; k += GT) lam[n + k] = 0.0;
       }
     }
+  }
+  if (un_b && !pulled) {   // pull-back of whatever u* holds (statuses that did not stream the final iterate)
+    pp.gsync();
+    __threadfence_block();
+    for (size_t i = gtid; i < n; i += GT) {
+      const double u0p = up_b[i];
+      un_b[i] = fma(A.taun, ustar[i] - u0p, u0p);
+    }
+    if (gtid == 0) { pp.rows_rd += 2 * nt; pp.rows_wr += nt; }
   }
   if (gtid == 0) {
     A.iters[b] = (status == 0) ? solves : status;

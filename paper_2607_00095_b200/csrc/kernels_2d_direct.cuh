@@ -33,6 +33,11 @@ struct Dir2dArgs {
   int* iters;
   double* ws;        // [batch][kPcgVectors][n]; vectors 0..2 are the iterate / trial buffers
   long long* stats;  // [batch][SNAP_STAT_COUNT]
+  // PCFM step fused around the projection (snap_flow_step; Eq. 1, 3): null / 0 for a plain projection
+  const double* vel;      // [batch][n]: the first pass forms u_hat = u_tau + omt vel, in place in u_hat
+  const double* u_prior;  // [batch][n] prior sample u_0
+  double* u_next;         // [batch][n] out: u_0 + taun (u* - u_0)
+  double omt, taun;
   int npx, nthr;     // patches per row, patches per level
   int ns_exact;      // full red-black sweeps that bring a level solve to fp64 rounding
   double log_rho2;   // log(rho^2) < 0: contraction per full sweep
@@ -202,18 +207,32 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
                            double* __restrict__ qpl, double* red, const double* __restrict__ x,
                            const double* __restrict__ uh, const double* __restrict__ u0, double* __restrict__ trial,
                            double* __restrict__ yout, double* __restrict__ ost, int ns, bool active, int nwarp,
-                           Pass2d& out) {
+                           Pass2d& out, const double* __restrict__ vel = nullptr, double omt = 0.0,
+                           double* __restrict__ uh_out = nullptr) {
   const int nt = P.nt, L = g.L;
   const double ax = P.ac_ax, ay = P.ac_ay, dt = P.dt;
   const double c0 = 1.0 + 2.0 * ax + 2.0 * ay - dt, dt3 = 3.0 * dt;
   double a_inf = 0.0, a_1 = 0.0, a_f = 0.0, a_wd = 0.0, a_dd = 0.0;
   double q[PR][4], rhs[PR][4], invD[PR][4];
-  if (threadIdx.x == 0) ring.issue(0, x, uh);
+  // PCFM step: x holds u_tau and the second row of a stage carries the velocity; the pass forms u_hat (Eq. 1) per level,
+  // writes it to `uh_out` (in place over u_tau) and into both stage rows, so the rest of the level sees x = u_hat
+  const double* __restrict__ second = vel ? vel : uh;
+  if (threadIdx.x == 0) ring.issue(0, x, second);
   for (int k = 0; k < nt; ++k) {
     const int s = k & 1;
     ring.wait(s);
     double xv[PR][4];
     load_nat<PR>(ring.row(s, 0) + g.nat, g.nx, xv);
+    if (vel) {
+      double vv[PR][4];
+      load_nat<PR>(ring.row(s, 1) + g.nat, g.nx, vv);
+#pragma unroll
+      for (int r = 0; r < PR; ++r)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) xv[r][e] = fma(omt, vv[r][e], xv[r][e]);
+      store_nat<PR>(ring.row(s, 1) + g.nat, g.nx, xv);
+      if (active) store_nat<PR>(uh_out + (size_t)k * L + g.nat, g.nx, xv);
+    }
     if (k == 0) {
       double u0v[PR][4];
       load_nat<PR>(u0 + g.nat, g.nx, u0v);
@@ -229,13 +248,13 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
         }
       store_planes<PR>(xpl, g, xv);
       __syncthreads();
-      if (threadIdx.x == 0 && nt > 1) ring.issue(1, x + L, uh + L);
+      if (threadIdx.x == 0 && nt > 1) ring.issue(1, x + L, second + L);
     } else {
       // rhs still holds x_{k-1} (own cells, left there by the end of the previous level); the planes take x_k
       store_planes<PR>(xpl, g, xv);
       if (threadIdx.x == 0) bulk_wait_read<0>();   // the previous level's trial row has left the staging row
       __syncthreads();
-      if (threadIdx.x == 0 && k + 1 < nt) ring.issue(s ^ 1, x + (size_t)(k + 1) * L, uh + (size_t)(k + 1) * L);
+      if (threadIdx.x == 0 && k + 1 < nt) ring.issue(s ^ 1, x + (size_t)(k + 1) * L, second + (size_t)(k + 1) * L);
       // halo of x_k in both colours
       const double2 n1 = *reinterpret_cast<const double2*>(xpl + g.psz + g.offN);   // (-1, e = 0, 2): colour 1
       const double2 n0 = *reinterpret_cast<const double2*>(xpl + g.offN);           // (-1, e = 1, 3): colour 0
@@ -316,7 +335,8 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
 template <int PR>
 __device__ double bwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, double* __restrict__ qpl, double* red,
                              const double* __restrict__ x, double* __restrict__ lam, double* __restrict__ ucopy, int ns,
-                             bool active, int nwarp) {
+                             bool active, int nwarp, const double* __restrict__ uprior = nullptr,
+                             double* __restrict__ unext = nullptr, double taun = 0.0) {
   const int nt = P.nt, L = g.L;
   const double ax = P.ac_ax, ay = P.ac_ay, dt = P.dt;
   const double c0 = 1.0 + 2.0 * ax + 2.0 * ay - dt, dt3 = 3.0 * dt;
@@ -333,6 +353,15 @@ __device__ double bwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, d
     double yv[PR][4], xv[PR][4];
     load_nat<PR>(ring.row(s, 0) + g.nat, g.nx, yv);
     load_nat<PR>(ring.row(s, 1) + g.nat, g.nx, xv);
+    if (unext) {   // OT pull-back of this level (Eq. 3): x is the final iterate, the prior row comes straight from HBM
+      double up[PR][4];
+      load_nat<PR>(uprior + (size_t)k * L + g.nat, g.nx, up);
+#pragma unroll
+      for (int r = 0; r < PR; ++r)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) up[r][e] = fma(taun, xv[r][e] - up[r][e], up[r][e]);
+      if (active) store_nat<PR>(unext + (size_t)k * L + g.nat, g.nx, up);
+    }
     __syncthreads();   // every thread is done with the other stage (read one level ago) and with the q planes
     if (threadIdx.x == 0 && k > 0) ring.issue(s ^ 1, lam + (size_t)(k - 1) * L, x + (size_t)(k - 1) * L);
 #pragma unroll
@@ -421,6 +450,11 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
 
   // sweeps of a pass whose input had ||h||_inf = hprev: the step only has to beat the quadratic term of the next
   // residual (inexact Newton; the residual itself is always evaluated exactly); eta = 1e-2 hprev^2 in [1e-16, 1e-6]
+  const double* vel_b = A.vel ? A.vel + (size_t)b * n : nullptr;
+  const double* up_b = A.u_next ? A.u_prior + (size_t)b * n : nullptr;
+  double* un_b = A.u_next ? A.u_next + (size_t)b * n : nullptr;
+  bool pulled = false;
+
   auto sweeps_for = [&](double hprev) -> int {
     double eta = 1e-2 * hprev * hprev;
     if (!(eta < 1e-6)) eta = 1e-6;
@@ -456,10 +490,11 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     const bool last = polishing && polish_left == 0;
     const bool emit_y = lam && (last || hprev * hprev < 100.0 * P.tol);
     const int ns = (polishing || emit_y) ? A.ns_exact : sweeps_for(hprev);
+    const bool shoot = vel_b && passes == 0;     // PCFM step: the first pass reads u_tau + velocity and forms u_hat
     fwd_pass2d<PR>(P, g, ring, xpl, qpl, red, pt, uh, u0, last ? nullptr : out, emit_y ? lam : nullptr, ost, ns, active,
-                   nwarp, S);
+                   nwarp, S, shoot ? vel_b : nullptr, A.omt, const_cast<double*>(uh));
     ++passes; inner += (long long)ns * (nt - 1);
-    rows_rd += 2 * nt; rows_wr += (last ? 0 : nt) + (emit_y ? nt : 0);
+    rows_rd += 2 * nt; rows_wr += (last ? 0 : nt) + (emit_y ? nt : 0) + (shoot ? nt : 0);
     have_y = emit_y;
     if (have_trial) {
       if (!polishing) {
@@ -515,8 +550,18 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     // multiplier-free call: u* = the returned iterate, nothing else to do
     if (status != SNAP_ST_NONFINITE && cur != ustar) {
       __syncthreads();
-      for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = cur[i];
-      rows_rd += nt; rows_wr += nt;
+      if (un_b) {     // one stream: u* and its pull-back
+        for (size_t i = tid; i < n; i += blockDim.x) {
+          const double xx = cur[i], u0p = up_b[i];
+          ustar[i] = xx;
+          un_b[i] = fma(A.taun, xx - u0p, u0p);
+        }
+        pulled = true;
+        rows_rd += 2 * nt; rows_wr += 2 * nt;
+      } else {
+        for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = cur[i];
+        rows_rd += nt; rows_wr += nt;
+      }
     }
   } else if (status == SNAP_ST_LINESEARCH || (status != SNAP_ST_NONFINITE && !have_y)) {
     // the returned point was not known to be final when its pass ran (feasible input, polish skipped or 0, max_iter,
@@ -529,11 +574,15 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
   if (lam && status != SNAP_ST_NONFINITE) {
     const bool late_copy = (ustar == uh) && (cur != ustar);   // in place: u_hat survives until lam is known finite
     double* ucopy = (cur != ustar && !late_copy) ? ustar : nullptr;
-    const double chk = bwd_pass2d<PR>(P, g, ring, qpl, red, cur, lam, ucopy, A.ns_exact, active, nwarp);
+    const bool pull = un_b && !late_copy && status == 0;
+    const double chk = bwd_pass2d<PR>(P, g, ring, qpl, red, cur, lam, ucopy, A.ns_exact, active, nwarp,
+                                      pull ? up_b : nullptr, pull ? un_b : nullptr, A.taun);
     ++passes; inner += (long long)A.ns_exact * (nt - 1);
-    rows_rd += 2 * nt; rows_wr += nt + (ucopy ? nt : 0);
+    rows_rd += 2 * nt + (pull ? nt : 0); rows_wr += nt + (ucopy ? nt : 0) + (pull ? nt : 0);
+    pulled = pull;
     if (!finite_d(chk)) {
       status = SNAP_ST_NONFINITE;
+      pulled = false;
     } else if (late_copy) {
       for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = cur[i];
       rows_rd += nt; rows_wr += nt;
@@ -545,6 +594,14 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
       for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = uh[i];
     if (lam)
       for (size_t i = tid; i < n; i += blockDim.x) lam[i] = 0.0;
+  }
+  if (un_b && !pulled) {   // pull-back of whatever u* holds (statuses that did not stream the final iterate)
+    __syncthreads();
+    for (size_t i = tid; i < n; i += blockDim.x) {
+      const double u0p = up_b[i];
+      un_b[i] = fma(A.taun, ustar[i] - u0p, u0p);
+    }
+    rows_rd += 2 * nt; rows_wr += nt;
   }
   if (tid == 0) {
     A.iters[b] = (status == 0) ? solves : status;
@@ -562,7 +619,7 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
 // (the caller then takes the PCG kernel).
 int launch_project2d_direct(snap_problem* p, int batch, const double* u_hat, const double* cdata,
                                    double* u_star, double* lambda, int* iters, void* workspace, long long* stats,
-                                   cudaStream_t st) {
+                                   const FlowArgs* flow, cudaStream_t st) {
   const DevParams& d = p->dp;
   if (d.nx % 4 != 0 || d.ny % 2 != 0) return 1;
   const int PR = (d.ny % 4 == 0) ? 4 : 2;
@@ -581,6 +638,12 @@ int launch_project2d_direct(snap_problem* p, int batch, const double* u_hat, con
   a.ws = reinterpret_cast<double*>(workspace);
   a.stats = stats;
   a.npx = npx; a.nthr = nthr;
+  a.vel = flow ? flow->vel : nullptr;
+  a.u_prior = flow ? flow->u_prior : nullptr;
+  a.u_next = flow ? flow->u_next : nullptr;
+  a.omt = flow ? flow->omt : 0.0;
+  a.taun = flow ? flow->taun : 0.0;
+  if (flow && !(al16(flow->vel) && al16(flow->u_prior) && al16(flow->u_next))) return 1;
   // error after s full sweeps <= rho^(2 s) ||q||_inf (initial guess rhs / D is already within rho); 2.2e-16 is rounding
   a.log_rho2 = (rho > 0.0) ? 2.0 * log(rho) : -1e30;
   a.ns_exact = (rho > 0.0) ? (int)ceil(log(2.2e-16) / a.log_rho2) : 0;

@@ -325,4 +325,19 @@ __global__ void __launch_bounds__(kMiscThreads) heat_project_kernel(const __grid
   if (threadIdx.x == 0) iters[b] = solves;
 }
 
+// ---- PCFM step, unfused parts (paths whose projection kernel does not fuse them): Eq. 1 and Eq. 3 ----
+__global__ void __launch_bounds__(kMiscThreads) flow_shoot_kernel(size_t total, double* __restrict__ u, const double* __restrict__ vel,
+                                                                 double omt) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x)
+    u[i] = fma(omt, vel[i], u[i]);                 // u_hat = u_tau + (1 - tau) v, in place
+}
+__global__ void __launch_bounds__(kMiscThreads) flow_pullback_kernel(size_t total, const double* __restrict__ u1,
+                                                                    const double* __restrict__ u_prior,
+                                                                    double* __restrict__ u_next, double taun) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const double u0p = u_prior[i];
+    u_next[i] = fma(taun, u1[i] - u0p, u0p);       // u_tau' = u_0 + tau' (u_1 - u_0)
+  }
+}
+
 }  // namespace snap

@@ -7,8 +7,17 @@
 
 namespace snap {
 
+// PCFM step arguments handed through the launch layers (null = plain projection)
+struct FlowArgs {
+  const double* vel;
+  const double* u_prior;
+  double* u_next;
+  double omt, taun;
+};
+
+
 // buffers of the fused path addressed through tensor maps (one row = one box)
-enum { TM_UHAT = 0, TM_BUFA = 1, TM_BUFB = 2, TM_USTAR = 3, TM_LAM = 4, TM_COUNT = 5 };
+enum { TM_UHAT = 0, TM_BUFA = 1, TM_BUFB = 2, TM_USTAR = 3, TM_LAM = 4, TM_VEL = 5, TM_COUNT = 6 };
 
 struct Proj1dArgs {
   alignas(64) CUtensorMap tm[TM_COUNT];   // fused path only: [sample][line of 16 doubles][16], 128-byte swizzle
@@ -24,6 +33,11 @@ struct Proj1dArgs {
   double* aux;   // [batch][2*nt]  level sums and null-space coefficients (min-norm multiplier, kind 4)
   long long* stats;  // [batch][SNAP_STAT_COUNT]  work counters (snap_project_stats)
   int variant;       // SNAP_VAR_* recorded in the stats
+  // PCFM step fused around the projection (snap_flow_step; Eq. 1, 3): all null / 0 for a plain projection
+  const double* vel;      // [batch][n] velocity values: the first pass forms u_hat = u_tau + omt * vel (in place in u_hat)
+  const double* u_prior;  // [batch][n] prior sample u_0 of the OT interpolant
+  double* u_next;         // [batch][n] out: u_0 + taun (u* - u_0)
+  double omt, taun;       // 1 - tau, tau'
   int fuse;      // cap on Gauss-Newton iterations per forward pass (0 = as many as the kernel supports)
   int nst;       // ring depth (levels in flight per warp)
   int rp;        // shared-memory row pitch in doubles (even; nx + halo + padding)
@@ -60,6 +74,7 @@ int launch_project2d(snap_problem* p, int batch, const double* u_hat, const doub
 
 // proj2d_direct.cu: product-form path of kind 3; returns +1 when the shape / parameters / alignment are outside it
 int launch_project2d_direct(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
-                            double* lambda, int* iters, void* workspace, long long* stats, cudaStream_t st);
+                            double* lambda, int* iters, void* workspace, long long* stats, const FlowArgs* flow,
+                            cudaStream_t st);
 
 }  // namespace snap

@@ -368,6 +368,76 @@ def test_multiplier_free_host_call(S):
     p.destroy()
 
 
+# ------------------------------------------------------------------------------------------------
+# PCFM step around the projection (Eq. 1-3): snap_flow_step against oracle.flow_step
+# ------------------------------------------------------------------------------------------------
+def _flow_inputs(wl, tau):
+    g = torch.Generator().manual_seed(77)
+    u0p = torch.randn(wl.u_hat.shape, generator=g, dtype=torch.float64)                 # prior sample u_0 ~ N(0, I)
+    u_true = wl.u_true.reshape(wl.u_hat.shape)
+    u_tau = u0p + tau * (u_true - u0p)                                                   # a state on the OT line
+    vel = (u_true - u0p) + 0.05 * torch.randn(wl.u_hat.shape, generator=g, dtype=torch.float64)   # stub velocity: exact + noise
+    return u_tau.contiguous(), vel.contiguous(), u0p.contiguous()
+
+
+@pytest.mark.parametrize("cfg,kw,prm,fused", [
+    (5, dict(batch=3, nx=64, nt=32), {}, True), (2, dict(batch=2, nx=128, nt=20), {}, True), (3, dict(batch=3, nx=64, nt=17), {}, True),
+    (4, dict(batch=2, nx=16, ny=16, nt=5), {}, True), (4, dict(batch=2, nx=64, ny=64, nt=3), {}, True),
+    (5, dict(batch=2, nx=64, nt=12), dict(gn_fuse=-1), False), (2, dict(batch=2, nx=70, nt=12), {}, False),
+    (4, dict(batch=2, nx=12, ny=10, nt=4), dict(gn_fuse=-1), False), (1, dict(batch=3, nx=20, nt=12), {}, False),
+    (6, dict(batch=2, nx=64, nt=16), {}, False)])
+def test_flow_step_matches_oracle(S, cfg, kw, prm, fused):
+    dev = torch.device("cuda:0")
+    wl = W.make_workload(cfg, **kw)
+    params = dict(wl.params, **prm)
+    tau, taun = 0.6, 0.7
+    u_tau, vel, u0p = _flow_inputs(wl, tau)
+    B = wl.batch
+    for with_lam in (True, False):
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, params)
+        d_ut = u_tau.to(dev)
+        u1 = torch.full_like(d_ut, float("nan"))
+        un = torch.full_like(d_ut, float("nan"))
+        lam = torch.full((B, p.m), float("nan"), dtype=torch.float64, device=dev) if with_lam else None
+        it = torch.full((B,), -99, dtype=torch.int32, device=dev)
+        l0 = p.launch_count()
+        ws = S.snap_flow_step(p, B, d_ut, vel.to(dev), u0p.to(dev), tau, taun, wl.cdata.to(dev), u1, un, lam, it)
+        st = torch.zeros(B, S.STAT_COUNT, dtype=torch.int64, device=dev)
+        S.snap_project_stats(p, B, ws, st)
+        torch.cuda.synchronize()
+        launches = p.launch_count() - l0
+        assert launches == (1 if fused else 3), (cfg, kw, prm, launches)        # fused: one launch per flow step
+        assert (it.cpu().numpy() > 0).all(), it
+        for b in range(B):
+            o = O.flow_step(wl.kind, u_tau[b].numpy(), vel[b].numpy(), u0p[b].numpy(), tau, taun, wl.cdata[b].numpy(), params)
+            assert o["status"] == 0
+            sc = np.abs(o["u1"]).max()
+            np.testing.assert_allclose(d_ut[b].cpu().numpy().reshape(o["u_hat"].shape), o["u_hat"], rtol=0, atol=4e-16 * 8)
+            assert np.abs(u1[b].cpu().numpy().reshape(o["u1"].shape) - o["u1"]).max() <= TOL_U * sc
+            assert np.abs(un[b].cpu().numpy().reshape(o["u1"].shape) - o["u_next"]).max() <= TOL_U * max(sc, np.abs(o["u_next"]).max())
+            if with_lam:
+                assert rel_lam(lam[b].cpu().numpy(), o["lam"]) <= TOL_L
+        # Eq. 3 exactly on the library's own u1 (one fma per cell)
+        expect = u0p + taun * (u1.cpu().reshape(u0p.shape) - u0p)
+        np.testing.assert_allclose(un.cpu().numpy().reshape(u0p.shape), expect.numpy(), rtol=0, atol=1e-15 * max(1.0, float(expect.abs().max())))
+        p.destroy()
+
+
+def test_flow_step_rejects_aliased_buffers_and_bad_times(S):
+    dev = torch.device("cuda:0")
+    wl = W.make_workload(5, batch=2, nx=64, nt=12)
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    u_tau, vel, u0p = (t.to(dev) for t in _flow_inputs(wl, 0.5))
+    u1, un = torch.empty_like(u_tau), torch.empty_like(u_tau)
+    it = torch.zeros(2, dtype=torch.int32, device=dev)
+    with pytest.raises(S.SnapError):
+        S.snap_flow_step(p, 2, u_tau, vel, u0p, 0.5, 0.6, wl.cdata.to(dev), u_tau, un, None, it)
+    with pytest.raises(S.SnapError):
+        S.snap_flow_step(p, 2, u_tau, vel, u0p, 1.5, 0.6, wl.cdata.to(dev), u1, un, None, it)
+    assert p.launch_count() == 0
+    p.destroy()
+
+
 def test_direct2d_matches_oracle_and_pcg_path(S):
     """Kind 3, product-form path (in-SMEM red-black level solves): same limit point as the oracle
     and as the PCG kernel (gn_fuse = -1) on 2-row and 4-row patches, one and several warps, nt = 2."""

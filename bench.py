@@ -311,6 +311,52 @@ def e2e_steps(run: GpuRun, steps: int, warmup: int):
     return run.projections_per_step() * steps / dt, h2d, d2h, ok
 
 
+def flow_step_lines(run, steps, warmup):
+    """PCFM step around the projection (Eq. 1-3): the fused snap_flow_step (one launch per
+    flow step, multiplier-free) against the same three operations as separate launches (torch elementwise shoot, snap_project,
+    torch elementwise pull-back).  Stub velocity = 0, so u_hat_j is the headline workload's input j and the projections are
+    the headline's; the velocity, prior and u_next fields are still read / written."""
+    S, p, B, dev = run.S, run.p, run.B, run.dev
+    n = run.wl.n
+    vel = torch.zeros(B, n, dtype=torch.float64, device=dev)
+    g = torch.Generator(device=dev).manual_seed(99)
+    prior = torch.randn(B, n, generator=g, dtype=torch.float64, device=dev)
+    u1 = torch.empty(B, n, dtype=torch.float64, device=dev)
+    un = torch.empty(B, n, dtype=torch.float64, device=dev)
+    uh_tmp = torch.empty(B, n, dtype=torch.float64, device=dev)
+    taus = [(c + 1) / N_TAU for c in range(run.calls)]
+
+    def fused():
+        for c, ut in enumerate(run.inputs):
+            S.snap_flow_step(p, B, ut.view(B, n), vel, prior, taus[c], min(1.0, taus[c] + 1.0 / N_TAU), run.cdata, u1, un, None,
+                             run.iters[c], workspace=run.ws)
+
+    def unfused():
+        for c, ut in enumerate(run.inputs):
+            torch.add(ut.view(B, n), vel, alpha=1.0 - taus[c], out=uh_tmp)                      # Eq. 1
+            S.snap_project(p, B, uh_tmp, run.cdata, u1, None, run.iters[c], workspace=run.ws)   # Eq. 2
+            torch.lerp(prior, u1, min(1.0, taus[c] + 1.0 / N_TAU), out=un)                      # Eq. 3
+
+    out = {}
+    for name, fn in (("fused", fused), ("separate_launches", unfused)):
+        for _ in range(warmup):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        out[name] = {"ms_per_step": ms, "flow_steps_per_s": B * run.calls / (ms * 1e-3), "converged_all": bool((run.iters > 0).all())}
+    S.snap_project_stats(p, B, run.ws, run.stats)
+    torch.cuda.synchronize()
+    out["note"] = ("50 flow steps x 1024 samples, multiplier-free; fused = snap_flow_step (Eq. 1 in the first forward pass, Eq. 3 in "
+                   "the final stream), separate = torch.add + snap_project + torch.lerp")
+    return out
+
+
 KERNEL_NAMES = {5: "project1d_fused_kernel<KB,1,8,3> (Burgers family, nx=256)", 2: "project1d_fused_kernel<KB,1,4,4> (nx=128)",
                 3: "project1d_fused_kernel<KF,1,4,3> (Fisher, nx=128)",
                 4: "project2d_direct_kernel<4,256> (variant 6; variant 5 = project2d_kernel, PCG)",
@@ -427,6 +473,8 @@ def run_gpu(args):
                                "alg_bytes_per_projection": sum(ab_f) / (run.B * run.calls), "roofline": rf,
                                "note": "snap_project(lambda = NULL): u* only, as PCFM's pull-back needs (PAPER.md Eq. 3 L54)"}
         run.lam_free = False
+    if rank == 0 and world == 1 and args.others and cfg == 5:
+        line["flow_step"] = flow_step_lines(run, args.steps, args.warmup)
     if rank == 0 and world == 1 and args.others and cfg == 5:
         others = {}
         for c in (1, 2, 3, 4, 6, 7):

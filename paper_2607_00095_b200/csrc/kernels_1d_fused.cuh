@@ -956,6 +956,44 @@ __device__ __noinline__ void fused_min_norm(const DevParams& P, RowPipe<W, Q>& p
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
 }
 
+// Streaming epilogue of a group of GT threads over one sample (n doubles, n % 2 == 0, 16-byte aligned rows):
+//   ucopy != nullptr:  ucopy = x ;   unext != nullptr:  unext = uprior + taun (x - uprior)     (Eq. 3)
+// 128-bit accesses, kU independent iterations in flight per thread (a scalar loop of one warp is latency-bound).
+template <int GT>
+__device__ __forceinline__ void stream_epilogue(int gtid, size_t n, const double* __restrict__ x, double* __restrict__ ucopy,
+                                                const double* __restrict__ uprior, double* __restrict__ unext, double taun) {
+  constexpr int kU = 8;
+  const size_t n2 = n >> 1;
+  const double2* x2 = reinterpret_cast<const double2*>(x);
+  const double2* p2 = reinterpret_cast<const double2*>(uprior);
+  double2* c2 = reinterpret_cast<double2*>(ucopy);
+  double2* o2 = reinterpret_cast<double2*>(unext);
+  size_t i = gtid;
+  for (; i + (size_t)(kU - 1) * GT < n2; i += (size_t)kU * GT) {
+    double2 xv[kU], pv[kU];
+#pragma unroll
+    for (int u = 0; u < kU; ++u) xv[u] = x2[i + (size_t)u * GT];
+    if (unext) {
+#pragma unroll
+      for (int u = 0; u < kU; ++u) pv[u] = p2[i + (size_t)u * GT];
+    }
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      if (ucopy) c2[i + (size_t)u * GT] = xv[u];
+      if (unext)
+        o2[i + (size_t)u * GT] = make_double2(fma(taun, xv[u].x - pv[u].x, pv[u].x), fma(taun, xv[u].y - pv[u].y, pv[u].y));
+    }
+  }
+  for (; i < n2; i += GT) {
+    const double2 xv = x2[i];
+    if (ucopy) c2[i] = xv;
+    if (unext) {
+      const double2 pv = p2[i];
+      o2[i] = make_double2(fma(taun, xv.x - pv.x, pv.x), fma(taun, xv.y - pv.y, pv.y));
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // the persistent Gauss-Newton driver (a8, a9); every warp of a group runs it with identical values
 // ------------------------------------------------------------------------------------------------
@@ -1188,15 +1226,11 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
     // multiplier-free call: no y emission, no multiplier sweep, no min-norm correction; u* = the final iterate
     const double* xf = (status == SNAP_ST_LINESEARCH) ? cur : xfin;
     if (un_b) {          // one stream: u* (if it is not in place already) and the pull-back
-      for (size_t i = gtid; i < n; i += GT) {
-        const double x = xf[i], u0p = up_b[i];
-        if (xf != ustar) ustar[i] = x;
-        un_b[i] = fma(A.taun, x - u0p, u0p);
-      }
+      stream_epilogue<GT>(gtid, n, xf, xf != ustar ? ustar : nullptr, up_b, un_b, A.taun);
       pulled = true;
       if (gtid == 0) { pp.rows_rd += 2 * nt; pp.rows_wr += nt + (xf != ustar ? nt : 0); }
     } else if (xf != ustar) {
-      for (size_t i = gtid; i < n; i += GT) ustar[i] = xf[i];
+      stream_epilogue<GT>(gtid, n, xf, ustar, nullptr, nullptr, 0.0);
       if (gtid == 0) { pp.rows_rd += nt; pp.rows_wr += nt; }
     }
   } else {
@@ -1246,10 +1280,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   if (un_b && !pulled) {   // pull-back of whatever u* holds (statuses that did not stream the final iterate)
     pp.gsync();
     __threadfence_block();
-    for (size_t i = gtid; i < n; i += GT) {
-      const double u0p = up_b[i];
-      un_b[i] = fma(A.taun, ustar[i] - u0p, u0p);
-    }
+    stream_epilogue<GT>(gtid, n, ustar, nullptr, up_b, un_b, A.taun);
     if (gtid == 0) { pp.rows_rd += 2 * nt; pp.rows_wr += nt; }
   }
   if (gtid == 0) {

@@ -550,18 +550,30 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     // multiplier-free call: u* = the returned iterate, nothing else to do
     if (status != SNAP_ST_NONFINITE && cur != ustar) {
       __syncthreads();
-      if (un_b) {     // one stream: u* and its pull-back
-        for (size_t i = tid; i < n; i += blockDim.x) {
-          const double xx = cur[i], u0p = up_b[i];
-          ustar[i] = xx;
-          un_b[i] = fma(A.taun, xx - u0p, u0p);
+      // one stream: u* and (PCFM step) its pull-back; 128-bit accesses, 4 independent iterations per thread
+      const double2* x2 = reinterpret_cast<const double2*>(cur);
+      const double2* p2 = reinterpret_cast<const double2*>(up_b);
+      double2* c2 = reinterpret_cast<double2*>(ustar);
+      double2* o2 = reinterpret_cast<double2*>(un_b);
+      const size_t n2 = n >> 1, T4 = 4 * (size_t)blockDim.x;
+      for (size_t i0 = tid; i0 < n2; i0 += T4) {
+        double2 xv[4], pv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const size_t i = i0 + (size_t)u * blockDim.x;
+          if (i < n2) { xv[u] = x2[i]; if (un_b) pv[u] = p2[i]; }
         }
-        pulled = true;
-        rows_rd += 2 * nt; rows_wr += 2 * nt;
-      } else {
-        for (size_t i = tid; i < n; i += blockDim.x) ustar[i] = cur[i];
-        rows_rd += nt; rows_wr += nt;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const size_t i = i0 + (size_t)u * blockDim.x;
+          if (i < n2) {
+            c2[i] = xv[u];
+            if (un_b) o2[i] = make_double2(fma(A.taun, xv[u].x - pv[u].x, pv[u].x), fma(A.taun, xv[u].y - pv[u].y, pv[u].y));
+          }
+        }
       }
+      if (un_b) pulled = true;
+      rows_rd += nt + (un_b ? nt : 0); rows_wr += nt + (un_b ? nt : 0);
     }
   } else if (status == SNAP_ST_LINESEARCH || (status != SNAP_ST_NONFINITE && !have_y)) {
     // the returned point was not known to be final when its pass ran (feasible input, polish skipped or 0, max_iter,

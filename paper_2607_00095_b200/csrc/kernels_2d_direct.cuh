@@ -49,6 +49,7 @@ struct Geo2d {
   int offN, offS;             // plane offsets of the halo rows above / below (same columns)
   int rowW, rowE;             // plane offsets of the halo columns left / right of patch row 0
   int nat;                    // natural-layout offset of patch row 0: j0 nx + i0
+  bool swap;                  // this lane fetches its east halo first (see gs_half)
 };
 
 struct Ring2d {
@@ -131,9 +132,19 @@ __device__ __forceinline__ void gs_half(double* __restrict__ pl, const Geo2d& g,
   const double* po = pl + (1 - C) * g.psz;
   const double2 nN = *reinterpret_cast<const double2*>(po + g.offN);
   const double2 nS = *reinterpret_cast<const double2*>(po + g.offS);
-  double hWE[PR];   // row r: west halo if (r & 1) == C, else east halo
+  // row r needs its west halo if (r & 1) == C, else its east halo: PR/2 of each.  A 64-bit load of 16 lanes at a
+  // 16-byte stride is a 2-way bank conflict; pairing a west row with an east row and letting every other group of 8
+  // lanes fetch the east one first puts the 16 lanes of a phase on 16 different bank pairs (odd / even 8-byte slots).
+  double hWE[PR];
 #pragma unroll
-  for (int r = 0; r < PR; ++r) hWE[r] = po[(((r & 1) == C) ? g.rowW : g.rowE) + r * g.hx];
+  for (int rp = 0; rp < PR; rp += 2) {
+    const int rw = rp + C, re = rp + 1 - C;          // west row, east row of this pair
+    const int ow = g.rowW + rw * g.hx, oe = g.rowE + re * g.hx;
+    const double first = po[g.swap ? oe : ow];
+    const double second = po[g.swap ? ow : oe];
+    hWE[rw] = g.swap ? second : first;
+    hWE[re] = g.swap ? first : second;
+  }
 #pragma unroll
   for (int r = 0; r < PR; ++r) {
 #pragma unroll
@@ -422,6 +433,7 @@ __global__ void __launch_bounds__(MAXT, 1) project2d_direct_kernel(const __grid_
     g.rowW = j0 * g.hx + pw;
     g.rowE = j0 * g.hx + pe;
     g.nat = j0 * P.nx + 4 * pi;
+    g.swap = (pi & 8) != 0;
   }
   double* sm = reinterpret_cast<double*>(smem_d2);
   Ring2d ring;

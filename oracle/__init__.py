@@ -23,11 +23,11 @@ prints no numeric values of any projected field; only the converged (u*, lambda*
 """
 from .constraints import (  # noqa: F401
     residual, jacobian, row_slices, full_rank_rows, num_rows, residual_norms,
-    paper_example_jacobian, godunov_flux, godunov_flux_grad, fluxk_counts,
+    paper_example_jacobian, godunov_flux, godunov_flux_grad, fluxk_counts, lagrangian_hessian, HESS_SAFEGUARD,
 )
 from .linsolve import (  # noqa: F401
     solve_kkt_dense_lu, solve_schur_pinv, solve_schur_banded_cholesky, solve_schur_cg, solve_schur_dense_cholesky,
-    min_norm_multiplier,
+    min_norm_multiplier, solve_kkt_sparse_lu,
 )
 from .project import project, project_batch  # noqa: F401
 from .flow import flow_step  # noqa: F401

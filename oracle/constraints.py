@@ -324,6 +324,53 @@ def jacobian(kind: int, u: np.ndarray, p: dict) -> sp.csr_matrix:
     return J.tocsr()        # duplicates (tiny periodic grids where i+1 == i-1) are summed
 
 
+HESS_SAFEGUARD = 0.1     # a free level's W_k is used only if its smallest eigenvalue a - 2|b| is at least this (else I)
+
+
+def lagrangian_hessian(kind: int, u: np.ndarray, lam: np.ndarray, p: dict) -> sp.csr_matrix:
+    """W = d^2/du^2 [ 1/2 ||u - u_hat||^2 + lam^T h(u) ] = I + sum_i lam_i grad^2 h_i(u)   (Eq. 5, Eq. 25)
+    restricted to where it can change the Newton-KKT step (R22):
+
+    * kinds whose local rows are square (1-4) and the pinned levels 0..K of kind 5: the step is fixed by J_loc du = -h
+      whatever W is, so W = I there (kind 0 is affine: W = I exactly);
+    * kind 5, free level k = K+1+f: only the energy rows are non-linear.  Row E_f = E(u[k]) - E(u[k-1]) + dt nu D(u[k-1])
+      has grad^2 = dx I on level k and -dx I + dt nu (2/dx) L on level k-1 (E = dx/2 sum u^2, D = sum (u_{i+1}-u_i)^2 / dx,
+      L = periodic second difference 2, -1, -1), so
+          W_k = (1 + dx lam_E[f] - dx lam_E[f+1]) I + dt nu (2/dx) lam_E[f+1] L      (lam_E[F] := 0),
+      a symmetric circulant tridiagonal with eigenvalues in [a - 2|b|, a + 2|b|], a = diagonal, b = off-diagonal.
+      Inertia safeguard: if a - 2|b| < HESS_SAFEGUARD the level uses W_k = I (a Gauss-Newton level).
+    Mass rows are linear.  Returns an n x n CSR matrix."""
+    u = np.asarray(u, dtype=np.float64)
+    nt, ny, nx = u.shape
+    n = nt * ny * nx
+    if kind != BURGERS1D_FLUXK:
+        return sp.identity(n, format="csr")
+    K, F, E = fluxk_counts(p, nt)
+    if E == 0:
+        return sp.identity(n, format="csr")
+    lamE = np.concatenate([np.asarray(lam, dtype=np.float64)[row_slices(kind, nx, ny, nt, p)["energy"]], [0.0]])
+    dx, cD = p["dx"], p["dt"] * p["nu"] * 2.0 / p["dx"]
+    diag = np.ones(n)
+    rows, cols, vals = [], [], []
+    i = np.arange(nx)
+    for f in range(F):
+        k = K + 1 + f
+        a = 1.0 + dx * (lamE[f] - lamE[f + 1]) + 2.0 * cD * lamE[f + 1]
+        b = -cD * lamE[f + 1]
+        if a - 2.0 * abs(b) < HESS_SAFEGUARD:
+            continue                                 # W_k = I
+        diag[k * nx:(k + 1) * nx] = a
+        if b != 0.0:
+            for sh in (1, -1):
+                rows.append(k * nx + i)
+                cols.append(k * nx + (i + sh) % nx)
+                vals.append(np.full(nx, b))
+    W = sp.diags(diag, format="csr")
+    if rows:
+        W = W + sp.coo_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))), shape=(n, n)).tocsr()
+    return W
+
+
 def paper_example_jacobian(nx: int, nt: int) -> np.ndarray:
     """The paper's own worked example (Appendix C, Eq. 26): IC rows first, then for
     k = 2..nt the left-Riemann mass row  sum_{i<nx} u_i^(k) - sum_{i<nx} u_i^(1)  (no dx weight,

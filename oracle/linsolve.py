@@ -108,3 +108,20 @@ def min_norm_multiplier(J: sp.spmatrix, lam_any: np.ndarray) -> np.ndarray:
     N = (J.T @ J).tocsr()
     z = solve_schur_banded_cholesky(N, g, refine=1)
     return J @ z
+
+
+def solve_kkt_sparse_lu(W: sp.spmatrix, J: sp.spmatrix, w: np.ndarray, h: np.ndarray):
+    """Newton-KKT step with a general (symmetric) Lagrangian Hessian W (Eq. 24):
+        [ W  J^T ] [ du  ]   [ -w ]
+        [ J   0  ] [ lam ] = [ -h ]
+    by sparse LU (SuperLU) of the full (n+m) x (n+m) matrix -- the paper's own formulation (sparse LDL^T of the KKT
+    matrix, L114-116), no Schur complement.  One step of iterative refinement.  Returns (du, lam)."""
+    import scipy.sparse.linalg as spla
+    n, m = W.shape[0], J.shape[0]
+    Kmat = sp.bmat([[W, J.T], [J, None]], format="csc")
+    rhs = -np.concatenate([w, h])
+    lu = spla.splu(Kmat)
+    x = lu.solve(rhs)
+    x += lu.solve(rhs - Kmat @ x)
+    return x[:n], x[n:]
+

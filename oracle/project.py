@@ -87,6 +87,9 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     mu_rule = p.get("mu_rule", "nw18_36")
     if mu_rule not in ("nw18_36", "lam_inf"):
         raise ValueError(f"unknown mu_rule {mu_rule!r}")
+    # hessian = 1: exact Lagrangian Hessian W = I + sum lam_i grad^2 h_i at the multipliers of the previous solve
+    # (Eq. 5 / 25); 0: Gauss-Newton, W = I (R1).  Same KKT points, different rate.
+    exact_w = int(p.get("hessian", 0)) == 1
     cg_state = {"rtol": 1e-13, "maxiter": 20000, "iters": 0}
     uh = u_hat.ravel()
     shape = u_hat.shape
@@ -94,15 +97,32 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     def h_of(v):
         return C.residual(kind, v.reshape(shape), u0, p)
 
-    def lin(v):
+    W_cur = [None]      # Hessian of the last linearisation (exact_w only): for the step and the model term d^T W d
+
+    def lin(v, lam_prev=None):
         h = h_of(v)
         J = C.jacobian(kind, v.reshape(shape), p)
         try:
             with np.errstate(all="ignore"):
-                lam = _solve_basic(J, v - uh, h, keep, backend, cg_state)
-        except (np.linalg.LinAlgError, ValueError):     # overflowed / non-SPD Schur matrix (R16)
+                if exact_w:
+                    W = C.lagrangian_hessian(kind, v.reshape(shape), lam_prev, p)
+                    W_cur[0] = W
+                    Jk = J[keep] if not keep.all() else J
+                    _, lam_k = L.solve_kkt_sparse_lu(W, Jk, v - uh, h[keep])
+                    lam = np.zeros(J.shape[0])
+                    lam[keep] = lam_k
+                else:
+                    lam = _solve_basic(J, v - uh, h, keep, backend, cg_state)
+        except (np.linalg.LinAlgError, ValueError, RuntimeError):     # overflowed / singular / non-SPD system (R16)
             lam = np.full(J.shape[0], np.nan)
         return h, J, lam
+
+    def full_step(v, J, lam):
+        """u + du of the Newton-KKT step: W du = -(u - u_hat) - J^T lam+   (W = I: u_hat - J^T lam+)."""
+        if not exact_w:
+            return uh - J.T @ lam
+        import scipy.sparse.linalg as spla
+        return v - spla.spsolve(W_cur[0].tocsc(), (v - uh) + J.T @ lam)
 
     u = uh.copy()
     mu = 0.0
@@ -113,7 +133,7 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     lam = np.zeros(C.num_rows(kind, nx, ny, nt, p))
     J = None
     while True:
-        h, J, lam = lin(u)
+        h, J, lam = lin(u, lam)
         solves += 1
         hinf = float(np.abs(h).max())
         if history is not None:
@@ -123,7 +143,7 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
             u = uh.copy()
             lam[:] = 0.0
             break
-        u_full = uh - J.T @ lam
+        u_full = full_step(u, J, lam)
         # Wide J (kind 5): Gauss-Newton with W = I contracts only linearly and ||h|| alone says nothing about
         # stationarity, so convergence also asks for a small step, RMS(d) <= tol (R18).  For the square
         # kinds d = -J^-1 h and the paper's/north_star's rule ||h||_inf < tol stands alone.
@@ -135,9 +155,9 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
             if hinf > POLISH_SKIP_FACTOR * tol:
                 for _ in range(polish):        # R4: full step(s), then the multiplier at the polished point
                     u = u_full
-                    h, J, lam = lin(u)
+                    h, J, lam = lin(u, lam)
                     solves += 1
-                    u_full = uh - J.T @ lam
+                    u_full = full_step(u, J, lam)
                     hinf = float(np.abs(h).max())
                     if history is not None:
                         history.append(hinf)
@@ -156,7 +176,9 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
         if mu_rule == "nw18_36":
             # penalty parameter from the predicted decrease of the quadratic model (N&W Eq. 18.36, sigma = 1):
             # needs no multiplier, so an implementation may postpone the multiplier solve (R2)
-            mu = max(mu, MU_FLOOR, (float((u - uh) @ d) + 0.5 * float(d @ d)) / ((1.0 - MU_RHO) * h1))
+            # (exact Hessian: the model term is d^T W d, N&W Eq. 18.36 with sigma = 1 where it is positive)
+            quad = float(d @ (W_cur[0] @ d)) if exact_w else float(d @ d)
+            mu = max(mu, MU_FLOOR, (float((u - uh) @ d) + 0.5 * max(quad, 0.0)) / ((1.0 - MU_RHO) * h1))
         else:
             # mu >= 1.1 ||lam+||_inf (+ floor) makes the l1 penalty exact (N&W Thm 17.3)
             mu = max(mu, 1.1 * float(np.abs(lam).max()) + MU_FLOOR)

@@ -289,7 +289,7 @@ __device__ void step_pass(const DevParams& P, const Ctx2d& c, const double* __re
 // ---- a6: PCG on S lam = b.  Returns 0 on success, 1 if pcg_max was hit ----------------------------------
 __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __restrict__ u, const double* __restrict__ b,
                          double* __restrict__ x, double* __restrict__ r, double* __restrict__ z, double* __restrict__ p,
-                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n, const double rtol,
+                         double* __restrict__ q, double* __restrict__ y, bool warm, size_t n, const double forcing_abs,
                          long long& rows_rd, long long& rows_wr, int& its_total) {
   const int tid = threadIdx.x;
   // level rows this solve asks HBM for (every vector pass = nt rows), per function:
@@ -302,6 +302,9 @@ __device__ int pcg_solve(const DevParams& P, const Ctx2d& c, const double* __res
   for (size_t i = tid; i < n; i += kT2) bb = fma(b[i], b[i], bb);
   bb = blk_sum(c, bb);
   const double bnorm = sqrt(bb);
+  // forcing_abs > 0: inexact Gauss-Newton solve, stop at ||r||_2 <= forcing_abs (an ABSOLUTE bound tied to ||h||, not to
+  // ||b|| = ||h - J(u - u_hat)||, which can be much larger than ||h||), never tighter than pcg_rtol nor looser than 1e-4 ||b||
+  const double rtol = (forcing_abs > 0.0 && bnorm > 0.0) ? fmax(P.pcg_rtol, fmin(1e-4, forcing_abs / bnorm)) : P.pcg_rtol;
   if (bnorm == 0.0) {
     for (size_t i = tid; i < n; i += kT2) x[i] = 0.0;
     return 0;
@@ -456,8 +459,11 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     // Inexact Gauss-Newton: a step taken from a point that is still far from feasible does not need the Schur
     // system solved to pcg_rtol; the forcing term shrinks with ||h||_inf, and every solve whose multiplier is
     // returned or used for the polish step (||h||_inf < tol) runs to the full pcg_rtol (R15).
-    const double rt = (polishing || hinf < P.tol) ? P.pcg_rtol : fmax(P.pcg_rtol, fmin(1e-4, 1e-3 * hinf));
-    const int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n, rt, rows_rd, rows_wr, pcg_its);
+    // forcing term eta = 1e-3 ||h||_inf relative to ||h||_2 >= ||h||_1 / sqrt(n)  (||J d + h|| <= eta ||h||: contraction
+    // is guaranteed whatever the size of J (u - u_hat))
+    const bool exact = polishing || hinf < P.tol;
+    const double forcing = exact ? 0.0 : 1e-3 * hinf * (h1 / sqrt((double)n));
+    int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n, forcing, rows_rd, rows_wr, pcg_its);
     have_lam = true;
     __syncthreads();
     if (prc == 2) { status = SNAP_ST_NONFINITE; break; }
@@ -473,6 +479,13 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     } else if (steps >= P.max_iter) {
       status = SNAP_ST_MAXITER;
       final_solve = true;
+      if (!exact) {   // the returned multiplier is always solved to pcg_rtol (R15): tighten the inexact solve
+        __syncthreads();
+        prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, true, n, 0.0, rows_rd, rows_wr, pcg_its);
+        __syncthreads();
+        if (prc == 2) { status = SNAP_ST_NONFINITE; break; }
+        if (prc == 1) { status = SNAP_ST_PCG; break; }
+      }
     }
     if (final_solve) break;
     double linf, wd, dd;

@@ -134,6 +134,12 @@ typedef struct {
   int flux_steps;     /* kind BURGERS1D_FLUXK: K, number of leading steps that carry flux rows (0 <= K <= nt-1)     */
   int energy_rows;    /* kind BURGERS1D_FLUXK: 1 = add the energy-evolution row of every later step                  */
   int flux_kind;      /* kind BURGERS1D_FLUXK: 0 = Lax-Friedrichs (alpha), 1 = Godunov                               */
+  int hessian;        /* 0 = Gauss-Newton, W = I (default, R1); 1 = exact Lagrangian Hessian
+                         W = I + sum lam_i grad^2 h_i at the multipliers of the previous solve (Eq. 5,
+                         Eq. 25), with an inertia safeguard per level (a level whose W_k has
+                         an eigenvalue below 0.1 uses I).  It changes the step only where J is wide: kind BURGERS1D_FLUXK
+                         with energy rows (quadratic instead of linear convergence); for the square kinds the step is
+                         J du = -h whatever W is, and the setting is accepted and has no effect (R22).   */
 } snap_params;
 
 /* Fill *p with the defaults listed above (grid steps 1, physical constants 0, alpha = 1). */

@@ -39,7 +39,7 @@ class SnapParams(C.Structure):
         ("ls_max", C.c_int),
         ("pcg_rtol", C.c_double),
         ("pcg_max", C.c_int), ("precond", C.c_int), ("lambda_mode", C.c_int), ("gn_fuse", C.c_int),
-        ("flux_steps", C.c_int), ("energy_rows", C.c_int), ("flux_kind", C.c_int),
+        ("flux_steps", C.c_int), ("energy_rows", C.c_int), ("flux_kind", C.c_int), ("hessian", C.c_int),
     ]
 
 

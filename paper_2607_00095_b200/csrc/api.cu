@@ -157,7 +157,7 @@ int project_fluxk(snap_problem* p, int batch, const double* u_hat, const double*
   bool found = false;
   for (; spc >= 1 && !found; --spc) {
     for (int nst = 4; nst >= 2; --nst) {
-      const size_t sb = align_up(((size_t)2 * nst * rp + (size_t)11 * (F > 0 ? F : 1) + nst) * 8, 1024);
+      const size_t sb = align_up(((size_t)2 * nst * rp + (size_t)12 * (F > 0 ? F : 1) + nst) * 8, 1024);
       if (sb * spc + 1024 <= (size_t)p->max_smem_optin) {
         pl.wpc = spc; pl.nst = nst; pl.warp_bytes = (int)sb; pl.smem = sb * spc + 1024;
         pl.grid = (batch + spc - 1) / spc;
@@ -213,6 +213,7 @@ void snap_params_default(snap_params* p) {
   p->flux_steps = 0;
   p->energy_rows = 0;
   p->flux_kind = 0;
+  p->hessian = 0;
 }
 
 int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, const snap_params* prm) {
@@ -234,6 +235,7 @@ int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, co
   if (!(prm->ls_shrink > 0.0 && prm->ls_shrink < 1.0) || !(prm->ls_c1 > 0.0 && prm->ls_c1 < 1.0)) return SNAP_EINVAL;
   if (prm->gn_fuse < -1 || prm->gn_fuse > 64) return SNAP_EINVAL;
   if (prm->precond < 0 || prm->precond > 2 || prm->lambda_mode < 0 || prm->lambda_mode > 1) return SNAP_EINVAL;
+  if (prm->hessian < 0 || prm->hessian > 1) return SNAP_EINVAL;
 
   snap_problem* p = new (std::nothrow) snap_problem();
   if (!p) return SNAP_ENOMEM;
@@ -247,6 +249,7 @@ int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, co
   d.m = (kind == SNAP_HEAT1D_IC_MASS) ? nx + nt : d.n + (d.has_mass ? nt : 0);
   if (kind == SNAP_BURGERS1D_FLUXK) {
     d.fk_K = prm->flux_steps; d.fk_energy = prm->energy_rows; d.fk_flux = prm->flux_kind;
+    d.fk_hess = (prm->hessian == 1 && prm->energy_rows == 1) ? 1 : 0;
     const int F = nt - 1 - d.fk_K;
     d.m = (d.fk_K + 1) * nx + F + (d.fk_energy ? F : 0);
     d.fk_s = prm->dt / prm->dx;

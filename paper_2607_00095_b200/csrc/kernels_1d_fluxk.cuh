@@ -115,6 +115,68 @@ __device__ __forceinline__ void energy_b(const DevParams& P, const double (&v)[Q
   sD = acc;   // per-lane part of sum_i (v_{i+1} - v_i)^2
 }
 
+// ---- exact Lagrangian Hessian on a free level (snap_params::hessian; Eq. 5) --------
+// W_k = a I + b (S + S^-1): a = 1 + dx (lamE[f] - lamE[f+1]) + 2 cD lamE[f+1],  b = -cD lamE[f+1]  (symmetric circulant
+// tridiagonal, eigenvalues in [a - 2|b|, a + 2|b|]).  Inertia safeguard: a - 2|b| < 0.1  =>  W_k = I (a Gauss-Newton level).
+constexpr double kHessSafeguard = 0.1;
+__device__ __forceinline__ void hess_coeffs(const DevParams& P, double lamE0, double lamE1, double& a, double& b) {
+  a = 1.0 + P.dx * (lamE0 - lamE1) + 2.0 * P.fk_cD * lamE1;
+  b = -P.fk_cD * lamE1;
+  if (!(a - 2.0 * fabs(b) >= kHessSafeguard)) { a = 1.0; b = 0.0; }
+}
+
+// g <- W^-1 g over the warp's 32 Q cells (lane owns Q contiguous cells, periodic).  W = kap (I - r S)(I - r S^-1) with
+// kap = (a + sqrt(a^2 - 4 b^2)) / 2, r = -b / kap, |r| < 1: two cyclic first-order recurrences
+//     y_i = g_i / kap + r y_{i-1} ,   x_i = y_i + r x_{i+1} ,
+// each = a local pass per lane with zero carry, the carry into a lane C_l = sum_j R^j P_{l-1-j} / (1 - R^32) (R = r^Q,
+// P = the lane's last local value) by a Kogge-Stone scan over the lanes (cut off once R^s is below rounding), and the
+// correction r^(j+1) C_l of the local values.  a, b are warp-uniform.
+template <int Q>
+__device__ __forceinline__ void circ_solve(double a, double b, double (&g)[Q], int lane) {
+  if (b == 0.0) {
+    const double ia = 1.0 / a;
+#pragma unroll
+    for (int c = 0; c < Q; ++c) g[c] *= ia;
+    return;
+  }
+  const double kap = 0.5 * (a + sqrt(a * a - 4.0 * b * b));
+  const double r = -b / kap, ik = 1.0 / kap;
+  double rp[Q];                       // r^(j+1)
+  rp[0] = r;
+#pragma unroll
+  for (int j = 1; j < Q; ++j) rp[j] = rp[j - 1] * r;
+  const double R = rp[Q - 1];
+  // forward recurrence (carry from the previous lane)
+  g[0] *= ik;
+#pragma unroll
+  for (int j = 1; j < Q; ++j) g[j] = fma(r, g[j - 1], g[j] * ik);
+  {
+    double T = __shfl_sync(SNAP_FULL, g[Q - 1], (lane + 31) & 31), Rs = R;
+    for (int s = 1; s < 32; s <<= 1) {
+      if (fabs(Rs) < 1e-20) { Rs = 0.0; break; }
+      T = fma(Rs, __shfl_sync(SNAP_FULL, T, (lane + 32 - s) & 31), T);
+      Rs *= Rs;
+    }
+    T /= (1.0 - Rs);                  // Rs = R^32 after a complete scan, 0 after a cut-off
+#pragma unroll
+    for (int j = 0; j < Q; ++j) g[j] = fma(rp[j], T, g[j]);
+  }
+  // backward recurrence (carry from the next lane)
+#pragma unroll
+  for (int j = Q - 2; j >= 0; --j) g[j] = fma(r, g[j + 1], g[j]);
+  {
+    double T = __shfl_sync(SNAP_FULL, g[0], (lane + 1) & 31), Rs = R;
+    for (int s = 1; s < 32; s <<= 1) {
+      if (fabs(Rs) < 1e-20) { Rs = 0.0; break; }
+      T = fma(Rs, __shfl_sync(SNAP_FULL, T, (lane + s) & 31), T);
+      Rs *= Rs;
+    }
+    T /= (1.0 - Rs);
+#pragma unroll
+    for (int j = 0; j < Q; ++j) g[j] = fma(rp[Q - 1 - j], T, g[j]);
+  }
+}
+
 // per-sample band system in shared memory: 10 doubles per free level f (level k = K+1+f), rows E_{k-1} then M_k
 // (arrays live in shared memory and are addressed in the .shared space explicitly: through generic pointers every
 // access was a generic LD.E / ST.E tracked by the long scoreboard, profiles/r02_fluxk.md)
@@ -133,13 +195,14 @@ struct Band {
   SmemArr rM;    // [F]
   SmemArr lE;    // [F] multipliers of the last solve: energy rows
   SmemArr lM;    // [F]                               mass rows
-  SmemArr jw;    // [2F] J_b^f w_f (for the penalty parameter), E rows then M rows
+  SmemArr jw;    // [2F] J_b^f W^-1 w_f (right-hand side and penalty parameter), E rows then M rows
+  SmemArr lW;    // [F] energy multipliers that defined W at the current linearisation (exact Hessian: the step needs them)
   __device__ __forceinline__ void carve(double* base, int F) {
     const uint32_t b = smem_u32(base), s = 8u * (uint32_t)F;
     dE.a = b; dM.a = b + s; eM.a = b + 2 * s; eE.a = b + 3 * s; mE.a = b + 4 * s; rE.a = b + 5 * s; rM.a = b + 6 * s;
-    lE.a = b + 7 * s; lM.a = b + 8 * s; jw.a = b + 9 * s;
+    lE.a = b + 7 * s; lM.a = b + 8 * s; jw.a = b + 9 * s; lW.a = b + 11 * s;
   }
-  static __host__ __device__ constexpr int doubles_per_level() { return 11; }
+  static __host__ __device__ constexpr int doubles_per_level() { return 12; }
 };
 
 // group-uniform results of one pass
@@ -147,7 +210,7 @@ struct FluxkSums {
   double hlev;      // ||h||_inf against (tol, kPolishSkip tol): 0, 1, 2 as in hinf_level
   double h1, f;     // ||h||_1, 1/2 ||u - u_hat||^2 at the point the pass produced
   double wq, qq;    // pinned levels: w^T q', ||q'||^2 of the Newton direction d = -q' at that point
-  double ww;        // free levels: ||w_f||^2
+  double ww;        // free levels: w_f^T W^-1 w_f  (= ||w_f||^2 for W = I)
   double dstep;     // update passes: ||t - x||^2 / alpha^2 = ||d||^2 of the step just applied, summed directly
   bool bad;
 };
@@ -169,7 +232,7 @@ __device__ __forceinline__ void warp_sum_n(double (&r)[N]) {
 // the pinned levels (iteration "B": q', for the next step and the coupling term of energy row K) and the band
 // system S_b, its right-hand side and J_b^f w_f.
 // ------------------------------------------------------------------------------------------------
-template <int Q, int FLUX>
+template <int Q, int FLUX, bool HESS>
 __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_ref, const Buf x, const Buf uh,
                                         const double* __restrict__ u0, double* __restrict__ xo, bool update,
                                         double alpha, double M0, Band bd, FluxkSums& S) {
@@ -190,7 +253,8 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   double ds2 = 0.0;
   int hmx = 0;
   // carried from the previous level (warp-uniform): energy, dissipation, and the dot products of its b vector
-  double E_prev = 0.0, D_prev = 0.0, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, bq_K = 0.0;
+  double E_prev = 0.0, D_prev = 0.0, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, bq_K = 0.0, gam_prev = 1.0;
+  constexpr bool hess = HESS;
 
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, k, x.tm, tm_uh);
@@ -240,62 +304,105 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
     } else {
       // ---- free level f: step with the border multipliers, then the dot products of the next band system ----
       const int f = k - K - 1;
+      const double lamE0 = energy ? bd.lE.get(f) : 0.0;
+      const double lamE1 = (energy && f + 1 < F) ? bd.lE.get(f + 1) : 0.0;
       if (update) {
-        const double lamM = bd.lM.get(f), lamE0 = energy ? bd.lE.get(f) : 0.0;
-        const double lamE1 = (energy && f + 1 < F) ? bd.lE.get(f + 1) : 0.0;
-        double b[Q], sDx;
+        const double lamM = bd.lM.get(f);
+        double b[Q], sDx, gv[Q];
         energy_b<Q>(P, v, lane, b, sDx);
 #pragma unroll
-        for (int c = 0; c < Q; ++c) {
-          const double full = uhr[c] - (dx * lamM + lamE0 * dx * v[c] + lamE1 * b[c]);
-          t[c] = fma(alpha, full - v[c], v[c]);
+        for (int c = 0; c < Q; ++c) gv[c] = (v[c] - uhr[c]) + (dx * lamM + lamE0 * dx * v[c] + lamE1 * b[c]);   // w + J_b^T lam_b
+        if constexpr (HESS) {   // d = -W^-1 (w + J^T lam), W of the linearisation at x (its energy multipliers were saved in lW)
+          double wa, wb;
+          hess_coeffs(P, bd.lW.get(f), (f + 1 < F) ? bd.lW.get(f + 1) : 0.0, wa, wb);
+          circ_solve<Q>(wa, wb, gv, lane);
         }
+#pragma unroll
+        for (int c = 0; c < Q; ++c) t[c] = fma(-alpha, gv[c], v[c]);
       } else {
 #pragma unroll
         for (int c = 0; c < Q; ++c) t[c] = v[c];
       }
       double b[Q], sD;
       energy_b<Q>(P, t, lane, b, sD);
-      // r: s1 = sum t, s2 = sum t^2, sD, bb = b.b, tb = t.b, sw = sum w, tw = t.w, bw = b.w, ww = w.w
-      double r[9] = {0.0, 0.0, sD, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+      // W of the NEXT linearisation (at t, multipliers of the last solve): zt = W^-1 t, zw = W^-1 w, zb = W^-1 b = (-dx + cD L) zt
+      double wa = 1.0, wb = 0.0;
+      if constexpr (HESS) hess_coeffs(P, lamE0, lamE1, wa, wb);
+      const double gam = HESS ? 1.0 / (wa + 2.0 * wb) : 1.0;          // W^-1 1 = gam 1
+      // r: s1 = sum t, s2 = sum t^2, sD, bzb = b.zb, tzb = t.zb, sw = sum w, tzw = t.zw, bzw = b.zw, wzw = w.zw [, tzt = t.zt, ww]
+      constexpr int NS = HESS ? 11 : 9;
+      double r[NS];
 #pragma unroll
-      for (int c = 0; c < Q; ++c) {
-        const double w = t[c] - uhr[c];
-        r[0] += t[c];
-        r[1] = fma(t[c], t[c], r[1]);
-        r[3] = fma(b[c], b[c], r[3]);
-        r[4] = fma(t[c], b[c], r[4]);
-        r[5] += w;
-        r[6] = fma(t[c], w, r[6]);
-        r[7] = fma(b[c], w, r[7]);
-        r[8] = fma(w, w, r[8]);
+      for (int i = 0; i < NS; ++i) r[i] = 0.0;
+      r[2] = sD;
+      if constexpr (HESS) {
+        double zt[Q], zw[Q], zb[Q];
+#pragma unroll
+        for (int c = 0; c < Q; ++c) { zt[c] = t[c]; zw[c] = t[c] - uhr[c]; }
+        if (!(wa == 1.0 && wb == 0.0)) {
+          circ_solve<Q>(wa, wb, zt, lane);
+          circ_solve<Q>(wa, wb, zw, lane);
+          double sdum;
+          energy_b<Q>(P, zt, lane, zb, sdum);
+        } else {
+#pragma unroll
+          for (int c = 0; c < Q; ++c) zb[c] = b[c];
+        }
+#pragma unroll
+        for (int c = 0; c < Q; ++c) {
+          const double w = t[c] - uhr[c];
+          r[0] += t[c];
+          r[1] = fma(t[c], t[c], r[1]);
+          r[3] = fma(b[c], zb[c], r[3]);
+          r[4] = fma(t[c], zb[c], r[4]);
+          r[5] += w;
+          r[6] = fma(t[c], zw[c], r[6]);
+          r[7] = fma(b[c], zw[c], r[7]);
+          r[8] = fma(w, zw[c], r[8]);
+          r[9] = fma(t[c], zt[c], r[9]);
+          r[10] = fma(w, w, r[10]);
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < Q; ++c) {
+          const double w = t[c] - uhr[c];
+          r[0] += t[c];
+          r[1] = fma(t[c], t[c], r[1]);
+          r[3] = fma(b[c], b[c], r[3]);
+          r[4] = fma(t[c], b[c], r[4]);
+          r[5] += w;
+          r[6] = fma(t[c], w, r[6]);
+          r[7] = fma(b[c], w, r[7]);
+          r[8] = fma(w, w, r[8]);
+        }
       }
-      warp_sum_n<9>(r);
+      warp_sum_n<NS>(r);
+      const double tzt = HESS ? r[HESS ? 9 : 1] : r[1], wwp = HESS ? r[HESS ? 10 : 8] : r[8];
       const double E_k = 0.5 * dx * r[1], D_k = r[2] / dx;
       const double hM = fma(dx, r[0], -M0);
       const double hE = energy ? (E_k - E_prev) + dtnu * D_prev : 0.0;
       const double aM = fabs(hM), aE = fabs(hE);
       hmx = max(hmx, max(__double2hiint(aM), __double2hiint(aE)));
       if (lane == 0) { h1 += aM + aE; ww_free += r[8]; }
-      f2 += (lane == 0) ? r[8] : 0.0;
+      f2 += (lane == 0) ? wwp : 0.0;
       if (lane == 0) {
-        const double aa = dx * dx * r[1], ab = dx * r[4], aw = dx * r[6];
+        const double aa = dx * dx * tzt, aw = dx * r[6];
         if (energy) {
           bd.dE.set(f, aa + (f > 0 ? bb_prev : 0.0));
-          bd.eM.set(f, (f > 0) ? -dx * dx * s1_prev : 0.0);       // M_{k-1} . b_{k-1} = dx sum b = -dx^2 sum t
-          bd.eE.set(f, (f > 0) ? ab_prev : 0.0);                  // a_{k-1} . b_{k-1}
-          bd.mE.set(f, dx * dx * r[0]);                           // M_k . a_k
+          bd.eM.set(f, (f > 0) ? -dx * dx * gam_prev * s1_prev : 0.0);   // M_{k-1} W^-1 b_{k-1} = dx gam sum b = -dx^2 gam sum t
+          bd.eE.set(f, (f > 0) ? ab_prev : 0.0);                  // a_{k-1} W^-1 b_{k-1}
+          bd.mE.set(f, dx * dx * gam * r[0]);                     // M_k W^-1 a_k
           const double jwE = aw + (f > 0 ? bw_prev : 0.0);
           bd.jw.set(f, jwE);
-          bd.rE.set(f, hE - jwE - (f == 0 ? bq_K : 0.0));         // h + J^{<=K} d^{<=K} - J^f w ,  d_K = -q'_K
+          bd.rE.set(f, hE - jwE - (f == 0 ? bq_K : 0.0));         // h + J^{<=K} d^{<=K} - J^f W^-1 w ,  d_K = -q'_K
         } else {
           bd.dE.set(f, 1.0); bd.eM.set(f, 0.0); bd.eE.set(f, 0.0); bd.mE.set(f, 0.0); bd.jw.set(f, 0.0); bd.rE.set(f, 0.0);
         }
-        bd.dM.set(f, (double)nx * dx * dx);
-        bd.jw.set(F + f, dx * r[5]);
-        bd.rM.set(f, hM - dx * r[5]);
-        (void)ab;
+        bd.dM.set(f, (double)nx * dx * dx * gam);
+        bd.jw.set(F + f, dx * gam * r[5]);
+        bd.rM.set(f, hM - dx * gam * r[5]);
       }
+      gam_prev = gam;
       E_prev = E_k; D_prev = D_k; bb_prev = r[3]; ab_prev = dx * r[4]; bw_prev = r[7]; s1_prev = r[0];
     }
     if (update) {
@@ -439,7 +546,7 @@ __device__ __noinline__ bool fluxk_local_multipliers(const DevParams& P, int lan
 // ------------------------------------------------------------------------------------------------
 // the persistent Gauss-Newton driver of kind 5 (a8, a9): one warp per sample
 // ------------------------------------------------------------------------------------------------
-template <int Q, int FLUX>
+template <int Q, int FLUX, bool HESS>
 __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_constant__ Proj1dArgs A) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   using G = RowGeom<1, Q>;
@@ -471,6 +578,8 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
     mbar_fence_init();
     fence_proxy_async_smem();
   }
+  // no multipliers yet: the first linearisation uses W = I (the iterate starts at u_hat with lam = 0, R3)
+  for (int f = lane; f < F; f += 32) { bd.lE.set(f, 0.0); bd.lM.set(f, 0.0); bd.lW.set(f, 0.0); }
   __syncwarp();
 
   const double* uh = A.u_hat + (size_t)b * n;
@@ -501,13 +610,17 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
   int polish_left = 0, steps = 0, solves = 0, status = 0, passes = 0, nback = 0;
   double mu = 0.0;
   FluxkSums S;
-  fluxk_pass<Q, FLUX>(P, pp, mk(cur), mk(uh), u0, nullptr, false, 1.0, M0, bd, S);
+  fluxk_pass<Q, FLUX, HESS>(P, pp, mk(cur), mk(uh), u0, nullptr, false, 1.0, M0, bd, S);
   ++passes;
   while (true) {
     if (S.bad) { status = SNAP_ST_NONFINITE; break; }
     // ---- border solve (the SMW / Schur-complement step) ----
     double lam_jw = 0.0, lam_rho = 0.0;
     int okb = 1;
+    __syncwarp();
+    // the energy multipliers that defined W in this linearisation: the step of this solve is taken with that W
+    if constexpr (HESS)
+      for (int f = lane; f < F; f += 32) bd.lW.set(f, bd.lE.get(f));
     __syncwarp();
     if (lane == 0 && F > 0) okb = band_solve(bd, F, lam_jw, lam_rho) ? 1 : 0;
     __syncwarp();
@@ -553,7 +666,7 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
     double* xo = (cur == buf0) ? buf1 : buf0;
     FluxkSums St;
     while (true) {
-      fluxk_pass<Q, FLUX>(P, pp, mk(cur), mk(uh), u0, xo, true, alpha, M0, bd, St);
+      fluxk_pass<Q, FLUX, HESS>(P, pp, mk(cur), mk(uh), u0, xo, true, alpha, M0, bd, St);
       ++passes;
       if (free_step) break;
       const double phi_t = St.f + mu * St.h1;
@@ -615,9 +728,9 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
   }
 }
 
-template <int Q, int FLUX>
+template <int Q, int FLUX, bool HESS>
 inline int launch_fluxk_variant(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
-  auto kern = project1d_fluxk_kernel<Q, FLUX>;
+  auto kern = project1d_fluxk_kernel<Q, FLUX, HESS>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess)
     return SNAP_ECUDA;
   kern<<<pl.grid, pl.wpc * 32, pl.smem, st>>>(a);

@@ -101,13 +101,21 @@ int launch_residual_fluxk(const DevParams& P, int batch, const double* u, const 
   return cudaGetLastError() == cudaSuccess ? SNAP_OK : SNAP_ECUDA;
 }
 
-int launch_project1d_fluxk(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
+template <int Q>
+static int launch_fluxk_q(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
   const bool god = a.P.fk_flux == FLUX_GODUNOV;
+  if (a.P.fk_hess) {   // exact Lagrangian Hessian on the free levels (only meaningful with energy rows)
+    return god ? launch_fluxk_variant<Q, FLUX_GODUNOV, true>(a, pl, st) : launch_fluxk_variant<Q, FLUX_LF, true>(a, pl, st);
+  }
+  return god ? launch_fluxk_variant<Q, FLUX_GODUNOV, false>(a, pl, st) : launch_fluxk_variant<Q, FLUX_LF, false>(a, pl, st);
+}
+
+int launch_project1d_fluxk(const Proj1dArgs& a, const Plan1d& pl, cudaStream_t st) {
   switch (a.P.nx) {
-    case 32: return god ? launch_fluxk_variant<1, FLUX_GODUNOV>(a, pl, st) : launch_fluxk_variant<1, FLUX_LF>(a, pl, st);
-    case 64: return god ? launch_fluxk_variant<2, FLUX_GODUNOV>(a, pl, st) : launch_fluxk_variant<2, FLUX_LF>(a, pl, st);
-    case 128: return god ? launch_fluxk_variant<4, FLUX_GODUNOV>(a, pl, st) : launch_fluxk_variant<4, FLUX_LF>(a, pl, st);
-    case 256: return god ? launch_fluxk_variant<8, FLUX_GODUNOV>(a, pl, st) : launch_fluxk_variant<8, FLUX_LF>(a, pl, st);
+    case 32: return launch_fluxk_q<1>(a, pl, st);
+    case 64: return launch_fluxk_q<2>(a, pl, st);
+    case 128: return launch_fluxk_q<4>(a, pl, st);
+    case 256: return launch_fluxk_q<8>(a, pl, st);
   }
   return SNAP_EINVAL;
 }

@@ -31,7 +31,7 @@ struct DevParams {
   double ac_ax, ac_ay;                // dt eps^2 / dx^2 , dt eps^2 / dy^2
   // kind 5 (BURGERS1D_FLUXK): K flux steps, energy rows on/off, flux kind; s = dt/dx, c = nu dt/dx^2,
   // cD = 2 dt nu / dx, dtnu = dt nu
-  int fk_K, fk_energy, fk_flux;
+  int fk_K, fk_energy, fk_flux, fk_hess;   // fk_hess: exact Lagrangian Hessian on the free levels (snap_params::hessian)
   double fk_s, fk_c, fk_cD, fk_dtnu, fk_alpha;
   // solver knobs
   double tol, ls_c1, ls_shrink, pcg_rtol;

@@ -786,7 +786,33 @@ def test_fluxk_line_search_is_live_far_from_the_feasible_set(S):
     p.destroy()
 
 
-@pytest.mark.parametrize("cfg", [6, 7])
+def test_fluxk_exact_hessian_matches_oracle_and_converges_faster(S):
+    """snap_params::hessian = 1 (SURVEY.md 8(f) NEXT-2): same KKT point as the oracle's exact-Hessian Newton-KKT iteration (and
+    as Gauss-Newton), fewer linearisations, P4's stationarity bound again (quadratic rate)."""
+    for kw in [dict(batch=3, nx=64, nt=96, noise=0.3), dict(batch=2, nx=32, nt=20), dict(batch=2, nx=128, nt=17),
+               dict(batch=2, nx=256, nt=24), dict(batch=2, nx=64, nt=12, params=dict(flux_steps=0)),
+               dict(batch=2, nx=32, nt=64, noise=0.5)]:
+        wl = W.make_workload(6, **kw)
+        prm = dict(hessian=1)
+        g = gpu_project(S, wl, wl.u_hat, params=prm)
+        gn = gpu_project(S, wl, wl.u_hat)
+        assert (g["iters"] > 0).all() and (gn["iters"] > 0).all(), (kw, g["iters"], gn["iters"])
+        assert (g["iters"] <= gn["iters"]).all(), (kw, g["iters"], gn["iters"])
+        assert g["norms"][:, 0].max() < 1e-10
+        np.testing.assert_allclose(g["u"], gn["u"], rtol=0, atol=3e-9)
+        for b in range(wl.batch):
+            o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), dict(wl.params, **prm))
+            assert o["status"] == 0
+            ru = np.abs(g["u"][b] - o["u"]).max() / np.abs(o["u"]).max()
+            rl = rel_lam(g["lam"][b], o["lam"])
+            assert ru <= TOL_U and rl <= TOL_L, (kw, b, ru, rl)
+            assert abs(int(g["iters"][b]) - int(o["iters"])) <= 1, (kw, b, g["iters"][b], o["iters"])
+            ks, _ = kkt_invariants(wl, wl.u_hat[b].numpy(), g["u"][b], g["lam"][b])
+            assert ks <= TOL_KKT, (kw, b, ks)
+        print(f"cfg6 {kw}: iters exact W {g['iters'].tolist()} / Gauss-Newton {gn['iters'].tolist()}")
+
+
+@pytest.mark.parametrize("cfg", [6, 7, 8])
 def test_fluxk_full_size(S, cfg):
     """256 x 256, batch 1024, Flux(5): oracle on three samples, invariants on 64, pinned levels on all."""
     wl = W.make_workload(cfg)
@@ -806,4 +832,4 @@ def test_fluxk_full_size(S, cfg):
         ks, _ = kkt_invariants(wl, wl.u_hat[b].numpy(), g["u"][b], g["lam"][b])
         worst = max(worst, ks)
     print(f"cfg{cfg}: stationarity on 64 samples {worst:.1e}, iters {np.bincount(g['iters'])}")
-    assert worst <= 1e-9      # R18: RMS(d) <= tol bounds stationarity only to first order (see the small-shape test)
+    assert worst <= (TOL_KKT if cfg == 8 else 1e-9)      # R18: RMS(d) <= tol bounds stationarity only to first order (see the small-shape test)

@@ -43,9 +43,11 @@ CONFIG_SHAPES = {
     # (Eq. 14, Table XVIII) at the scale of cfg 5.
     6: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1006),   # Lax-Friedrichs flux rows + energy-evolution rows (Eq. 11)
     7: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1007),   # Godunov flux rows (L555), inviscid, no energy rows
+    8: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1006),   # config 6 (same inputs) with the exact Lagrangian Hessian (NEXT-2)
 }
 CONFIG_EXTRA = {6: dict(flux_steps=5, energy_rows=1, flux_kind=0),
-                7: dict(flux_steps=5, energy_rows=0, flux_kind=1, nu=0.0)}
+                7: dict(flux_steps=5, energy_rows=0, flux_kind=1, nu=0.0),
+                8: dict(flux_steps=5, energy_rows=1, flux_kind=0, hessian=1)}
 
 F64 = torch.float64
 

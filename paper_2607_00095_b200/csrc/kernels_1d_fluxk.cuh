@@ -197,7 +197,12 @@ struct Band {
   SmemArr lM;    // [F]                               mass rows
   SmemArr jw;    // [2F] J_b^f W^-1 w_f (right-hand side and penalty parameter), E rows then M rows
   SmemArr lW;    // [F] energy multipliers that defined W at the current linearisation (exact Hessian: the step needs them)
+  // During a pass the arrays dE..rM and jw double as the store of the level totals (slot q of level f): the band entries
+  // are assembled from them afterwards, 32 levels at a time (fluxk_assemble).
+  uint32_t base_a, stride;
+  __device__ __forceinline__ uint32_t slot(int q, int f) const { return base_a + (uint32_t)(q < 7 ? q : q + 2) * stride + 8u * (uint32_t)f; }
   __device__ __forceinline__ void carve(double* base, int F) {
+    base_a = smem_u32(base); stride = 8u * (uint32_t)F;
     const uint32_t b = smem_u32(base), s = 8u * (uint32_t)F;
     dE.a = b; dM.a = b + s; eM.a = b + 2 * s; eE.a = b + 3 * s; mE.a = b + 4 * s; rE.a = b + 5 * s; rM.a = b + 6 * s;
     lE.a = b + 7 * s; lM.a = b + 8 * s; jw.a = b + 9 * s; lW.a = b + 11 * s;
@@ -222,6 +227,88 @@ __device__ __forceinline__ void warp_sum_n(double (&r)[N]) {
 #pragma unroll
     for (int i = 0; i < N; ++i) r[i] += __shfl_xor_sync(SNAP_FULL, r[i], o);
   }
+}
+
+// Eight per-lane partial sums -> eight warp totals with 9 instead of 40 64-bit shuffles: every round halves the values a
+// lane carries (the half it does not keep goes to its butterfly partner).  Lane l ends with the total of value
+// (l >> 2) & 7 (the four lanes of a group hold the same total).  Fixed order: run-to-run deterministic.
+__device__ __forceinline__ double warp_transpose_sum8(const double (&p)[8], int lane) {
+  const bool h16 = (lane & 16) != 0, h8 = (lane & 8) != 0, h4 = (lane & 4) != 0;
+  double b4[4], c2[2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) b4[i] = (h16 ? p[i + 4] : p[i]) + __shfl_xor_sync(SNAP_FULL, h16 ? p[i] : p[i + 4], 16);
+#pragma unroll
+  for (int i = 0; i < 2; ++i) c2[i] = (h8 ? b4[i + 2] : b4[i]) + __shfl_xor_sync(SNAP_FULL, h8 ? b4[i] : b4[i + 2], 8);
+  double d = (h4 ? c2[1] : c2[0]) + __shfl_xor_sync(SNAP_FULL, h4 ? c2[0] : c2[1], 4);
+  d += __shfl_xor_sync(SNAP_FULL, d, 2);
+  d += __shfl_xor_sync(SNAP_FULL, d, 1);
+  return d;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Band system from the level totals a pass left in the slots (see Band::slot): lane l assembles the free levels
+// [l c, (l+1) c), c = ceil(F / 32).  Level f needs its own totals and those of level f - 1 (level K for f = 0), read
+// before anything is overwritten.  Also adds |h_M|, |h_E| of its levels to the lane's h1 / hmx.
+//   S_b rows (E_f, M_f) of level k = K+1+f, with a = dx t, b = (-dx + cD L) t, m = dx 1, gam = 1 / (wa + 2 wb) (W^-1 1 = gam 1):
+//     (E_f,E_f) = dx^2 t.zt + b'.zb'      (E_f,M_f) = dx^2 gam s1       (M_f,M_f) = nx dx^2 gam
+//     (E_f,M_f-1) = -dx^2 gam' s1'        (E_f,E_f-1) = dx t'.zb'       ( ' = level f - 1 )
+//     rhs_E = h_E - (dx t.zw + b'.zw') - [f = 0] b_K.q'_K               rhs_M = h_M - dx gam sw
+// ------------------------------------------------------------------------------------------------
+template <bool HESS>
+__device__ __forceinline__ void fluxk_assemble(const DevParams& P, Band bd, int F, int nx, int lane, double M0, double E_K,
+                                               double D_K, double bq_K, double& h1, int& hmx) {
+  const bool energy = P.fk_energy != 0;
+  const double dx = P.dx, dtnu = P.fk_dtnu;
+  const int chunk = (F + 31) >> 5;
+  const int f0 = lane * chunk, f1 = (f0 + chunk < F) ? f0 + chunk : F;
+  auto gam_of = [&](int f) -> double {
+    if constexpr (!HESS) return 1.0;
+    double wa, wb;
+    hess_coeffs(P, bd.lE.get(f), (f + 1 < F) ? bd.lE.get(f + 1) : 0.0, wa, wb);
+    return 1.0 / (wa + 2.0 * wb);
+  };
+  // predecessor level
+  double E_prev = E_K, D_prev = D_K, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, gam_prev = 1.0;
+  if (f0 > 0 && f0 < F) {
+    const int g = f0 - 1;
+    s1_prev = lds_f64(bd.slot(0, g));
+    E_prev = 0.5 * dx * lds_f64(bd.slot(1, g));
+    D_prev = lds_f64(bd.slot(2, g)) / dx;
+    bb_prev = lds_f64(bd.slot(3, g));
+    ab_prev = dx * lds_f64(bd.slot(4, g));
+    bw_prev = lds_f64(bd.slot(7, g));
+    gam_prev = gam_of(g);
+  }
+  __syncwarp();
+  for (int f = f0; f < f1; ++f) {
+    const double s1 = lds_f64(bd.slot(0, f)), s2 = lds_f64(bd.slot(1, f)), sD = lds_f64(bd.slot(2, f));
+    const double bzb = lds_f64(bd.slot(3, f)), tzb = lds_f64(bd.slot(4, f)), sw = lds_f64(bd.slot(5, f));
+    const double tzw = lds_f64(bd.slot(6, f)), bzw = lds_f64(bd.slot(7, f));
+    const double tzt = HESS ? lds_f64(bd.slot(8, f)) : s2;
+    const double gam = gam_of(f);
+    const double E_k = 0.5 * dx * s2, D_k = sD / dx;
+    const double hM = fma(dx, s1, -M0);
+    const double hE = energy ? (E_k - E_prev) + dtnu * D_prev : 0.0;
+    const double aM = fabs(hM), aE = fabs(hE);
+    hmx = max(hmx, max(__double2hiint(aM), __double2hiint(aE)));
+    h1 += aM + aE;
+    if (energy) {
+      bd.dE.set(f, dx * dx * tzt + (f > 0 ? bb_prev : 0.0));
+      bd.eM.set(f, (f > 0) ? -dx * dx * gam_prev * s1_prev : 0.0);
+      bd.eE.set(f, (f > 0) ? ab_prev : 0.0);
+      bd.mE.set(f, dx * dx * gam * s1);
+      const double jwE = dx * tzw + (f > 0 ? bw_prev : 0.0);
+      bd.jw.set(f, jwE);
+      bd.rE.set(f, hE - jwE - (f == 0 ? bq_K : 0.0));
+    } else {
+      bd.dE.set(f, 1.0); bd.eM.set(f, 0.0); bd.eE.set(f, 0.0); bd.mE.set(f, 0.0); bd.jw.set(f, 0.0); bd.rE.set(f, 0.0);
+    }
+    bd.dM.set(f, (double)nx * dx * dx * gam);
+    bd.jw.set(F + f, dx * gam * sw);
+    bd.rM.set(f, hM - dx * gam * sw);
+    E_prev = E_k; D_prev = D_k; bb_prev = bzb; ab_prev = dx * tzb; bw_prev = bzw; s1_prev = s1; gam_prev = gam;
+  }
+  __syncwarp();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -249,11 +336,11 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   double phiA[Q], ccA[Q], phiB[Q], ccB[Q];
 #pragma unroll
   for (int c = 0; c < Q; ++c) { phiA[c] = u0[first + c]; phiB[c] = phiA[c]; ccA[c] = 0.0; ccB[c] = 0.0; }
-  double h1 = 0.0, f2 = 0.0, wq = 0.0, qq = 0.0, ww_free = 0.0;   // h1 / ww_free: lane 0 adds the warp-uniform row values
+  double h1 = 0.0, f2 = 0.0, wq = 0.0, qq = 0.0, wzw = 0.0;   // per-lane partial sums (wzw: w^T W^-1 w over the free levels)
   double ds2 = 0.0;
   int hmx = 0;
   // carried from the previous level (warp-uniform): energy, dissipation, and the dot products of its b vector
-  double E_prev = 0.0, D_prev = 0.0, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, bq_K = 0.0, gam_prev = 1.0;
+  double E_K = 0.0, D_K = 0.0, bq_K = 0.0;   // level K (warp-uniform): energy, dissipation, b_K . q'_K
   constexpr bool hess = HESS;
 
   const int npro = nst < nt ? nst : nt;
@@ -297,8 +384,8 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
 #pragma unroll
         for (int c = 0; c < Q; ++c) { r[0] = fma(t[c], t[c], r[0]); r[2] = fma(b[c], qb[c], r[2]); }
         warp_sum_n<3>(r);
-        E_prev = 0.5 * dx * r[0];
-        D_prev = r[1] / dx;
+        E_K = 0.5 * dx * r[0];
+        D_K = r[1] / dx;
         bq_K = r[2];
       }
     } else {
@@ -328,13 +415,14 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       // W of the NEXT linearisation (at t, multipliers of the last solve): zt = W^-1 t, zw = W^-1 w, zb = W^-1 b = (-dx + cD L) zt
       double wa = 1.0, wb = 0.0;
       if constexpr (HESS) hess_coeffs(P, lamE0, lamE1, wa, wb);
-      const double gam = HESS ? 1.0 / (wa + 2.0 * wb) : 1.0;          // W^-1 1 = gam 1
-      // r: s1 = sum t, s2 = sum t^2, sD, bzb = b.zb, tzb = t.zb, sw = sum w, tzw = t.zw, bzw = b.zw, wzw = w.zw [, tzt = t.zt, ww]
-      constexpr int NS = HESS ? 11 : 9;
-      double r[NS];
+      // level sums of the next band system: s1 = sum t, s2 = sum t^2, sD, bzb = b.zb, tzb = t.zb, sw = sum w, tzw = t.zw,
+      // bzw = b.zw [, tzt = t.zt]  (W = I: zt = t, zw = w, zb = b).  They go to the level's slots of the band arrays; the
+      // band entries, h_M, h_E are assembled after the pass (fluxk_assemble): nothing of a level is carried to the next.
+      double r[8];
 #pragma unroll
-      for (int i = 0; i < NS; ++i) r[i] = 0.0;
+      for (int i = 0; i < 8; ++i) r[i] = 0.0;
       r[2] = sD;
+      double tzt = 0.0;
       if constexpr (HESS) {
         double zt[Q], zw[Q], zb[Q];
 #pragma unroll
@@ -358,9 +446,9 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
           r[5] += w;
           r[6] = fma(t[c], zw[c], r[6]);
           r[7] = fma(b[c], zw[c], r[7]);
-          r[8] = fma(w, zw[c], r[8]);
-          r[9] = fma(t[c], zt[c], r[9]);
-          r[10] = fma(w, w, r[10]);
+          tzt = fma(t[c], zt[c], tzt);
+          wzw = fma(w, zw[c], wzw);
+          f2 = fma(w, w, f2);
         }
       } else {
 #pragma unroll
@@ -373,37 +461,18 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
           r[5] += w;
           r[6] = fma(t[c], w, r[6]);
           r[7] = fma(b[c], w, r[7]);
-          r[8] = fma(w, w, r[8]);
+          f2 = fma(w, w, f2);
+          wzw = fma(w, w, wzw);
         }
       }
-      warp_sum_n<NS>(r);
-      const double tzt = HESS ? r[HESS ? 9 : 1] : r[1], wwp = HESS ? r[HESS ? 10 : 8] : r[8];
-      const double E_k = 0.5 * dx * r[1], D_k = r[2] / dx;
-      const double hM = fma(dx, r[0], -M0);
-      const double hE = energy ? (E_k - E_prev) + dtnu * D_prev : 0.0;
-      const double aM = fabs(hM), aE = fabs(hE);
-      hmx = max(hmx, max(__double2hiint(aM), __double2hiint(aE)));
-      if (lane == 0) { h1 += aM + aE; ww_free += r[8]; }
-      f2 += (lane == 0) ? wwp : 0.0;
-      if (lane == 0) {
-        const double aa = dx * dx * tzt, aw = dx * r[6];
-        if (energy) {
-          bd.dE.set(f, aa + (f > 0 ? bb_prev : 0.0));
-          bd.eM.set(f, (f > 0) ? -dx * dx * gam_prev * s1_prev : 0.0);   // M_{k-1} W^-1 b_{k-1} = dx gam sum b = -dx^2 gam sum t
-          bd.eE.set(f, (f > 0) ? ab_prev : 0.0);                  // a_{k-1} W^-1 b_{k-1}
-          bd.mE.set(f, dx * dx * gam * r[0]);                     // M_k W^-1 a_k
-          const double jwE = aw + (f > 0 ? bw_prev : 0.0);
-          bd.jw.set(f, jwE);
-          bd.rE.set(f, hE - jwE - (f == 0 ? bq_K : 0.0));         // h + J^{<=K} d^{<=K} - J^f W^-1 w ,  d_K = -q'_K
-        } else {
-          bd.dE.set(f, 1.0); bd.eM.set(f, 0.0); bd.eE.set(f, 0.0); bd.mE.set(f, 0.0); bd.jw.set(f, 0.0); bd.rE.set(f, 0.0);
+      {
+        const double tot = warp_transpose_sum8(r, lane);
+        if ((lane & 3) == 0) sts_f64(bd.slot((lane >> 2) & 7, f), tot);
+        if constexpr (HESS) {
+          const double tt = warp_sum(tzt);
+          if (lane == 1) sts_f64(bd.slot(8, f), tt);
         }
-        bd.dM.set(f, (double)nx * dx * dx * gam);
-        bd.jw.set(F + f, dx * gam * r[5]);
-        bd.rM.set(f, hM - dx * gam * r[5]);
       }
-      gam_prev = gam;
-      E_prev = E_k; D_prev = D_k; bb_prev = r[3]; ab_prev = dx * r[4]; bw_prev = r[7]; s1_prev = r[0];
     }
     if (update) {
 #pragma unroll
@@ -415,13 +484,14 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
     if (++s == nst) s = 0;
   }
   pp.drain();
+  if (F > 0) fluxk_assemble<HESS>(P, bd, F, nx, lane, M0, E_K, D_K, bq_K, h1, hmx);
   S.hlev = hinf_level(hmx, tol, skip);
   S.h1 = warp_sum(h1);
   const double f2s = warp_sum(f2);
   S.f = 0.5 * f2s;
   S.wq = warp_sum(wq);
   S.qq = warp_sum(qq);
-  S.ww = __shfl_sync(SNAP_FULL, ww_free, 0);
+  S.ww = warp_sum(wzw);
   S.dstep = warp_sum(ds2) / (alpha * alpha);
   S.bad = !(finite_d(S.h1) && finite_d(f2s) && finite_d(S.wq) && finite_d(S.qq));
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;

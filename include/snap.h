@@ -122,7 +122,7 @@ typedef struct {
   double ls_shrink;   /* step-length reduction factor                       (default 0.5)                     */
   int ls_max;         /* maximum number of reductions per step              (default 20)                      */
   double pcg_rtol;    /* 2D: PCG stops at ||r - S lam||_2 <= pcg_rtol ||r||_2 (default 1e-13);
-                         steps taken while ||h||_inf >= tol stop at ||r||_2 <= 1e-3 ||h||_inf ||h||_1/sqrt(n)
+                         steps taken while ||h||_inf >= tol stop at ||r||_2 <= 1e-2 ||h||_inf ||h||_1/sqrt(n)
                          (never tighter than pcg_rtol ||b||, never looser than 1e-4 ||b||)                     */
   int pcg_max;        /* 2D: PCG iteration cap per solve                    (default 200)                     */
   int precond;        /* 2D: 0 none, 1 time-line, 2 time-line x ADI         (default 2)                       */

@@ -459,10 +459,10 @@ __global__ void __launch_bounds__(kT2, 1) project2d_kernel(const __grid_constant
     // Inexact Gauss-Newton: a step taken from a point that is still far from feasible does not need the Schur
     // system solved to pcg_rtol; the forcing term shrinks with ||h||_inf, and every solve whose multiplier is
     // returned or used for the polish step (||h||_inf < tol) runs to the full pcg_rtol (R15).
-    // forcing term eta = 1e-3 ||h||_inf relative to ||h||_2 >= ||h||_1 / sqrt(n)  (||J d + h|| <= eta ||h||: contraction
+    // forcing term eta = 1e-2 ||h||_inf relative to ||h||_2 >= ||h||_1 / sqrt(n)  (||J d + h|| <= eta ||h||: contraction
     // is guaranteed whatever the size of J (u - u_hat))
     const bool exact = polishing || hinf < P.tol;
-    const double forcing = exact ? 0.0 : 1e-3 * hinf * (h1 / sqrt((double)n));
+    const double forcing = exact ? 0.0 : 1e-2 * hinf * (h1 / sqrt((double)n));
     int prc = pcg_solve(P, c, cur, bv, lam, rv, zv, pv, qv, yv, have_lam, n, forcing, rows_rd, rows_wr, pcg_its);
     have_lam = true;
     __syncthreads();

@@ -222,7 +222,7 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
                            double* __restrict__ uh_out = nullptr) {
   const int nt = P.nt, L = g.L;
   const double ax = P.ac_ax, ay = P.ac_ay, dt = P.dt;
-  const double c0 = 1.0 + 2.0 * ax + 2.0 * ay - dt, dt3 = 3.0 * dt;
+  const double c0 = 1.0 + 2.0 * ax + 2.0 * ay - dt, dt3 = 3.0 * dt, c1 = 2.0 * ax + 2.0 * ay - dt;
   double a_inf = 0.0, a_1 = 0.0, a_f = 0.0, a_wd = 0.0, a_dd = 0.0;
   double q[PR][4], rhs[PR][4], invD[PR][4];
   // PCFM step: x holds u_tau and the second row of a stage carries the velocity; the pass forms u_hat (Eq. 1) per level,
@@ -288,12 +288,17 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
           const double E = (e == 3) ? hE[r] : xv[r][e == 3 ? 3 : e + 1];
           const double N = (r == 0) ? hN[e] : xv[r == 0 ? 0 : r - 1][e];
           const double S = (r == PR - 1) ? hS[e] : xv[r == PR - 1 ? r : r + 1][e];
-          const double h = (v - rhs[r][e]) - ax * ((W - v) + (E - v)) - ay * ((N - v) + (S - v)) + dt * (v * v * v - v);
+          // h = (v - x_{k-1}) - ax (W + E - 2v) - ay (N + S - 2v) + dt (v^3 - v), grouped as
+          //     (v - x_{k-1}) + v (2ax + 2ay - dt + dt v^2) - ax (W + E) - ay (N + S):  9 instead of 16 FP64 operations with D
+          const double v2 = v * v;
+          double h = fma(fma(dt, v2, c1), v, v - rhs[r][e]);
+          h = fma(-ax, W + E, h);
+          h = fma(-ay, N + S, h);
           const double ah = fabs(h);
           a_inf = fmax(a_inf, ah);
           a_1 += ah;
           rhs[r][e] = h + q[r][e];
-          invD[r][e] = rcp_pos(fma(dt3, v * v, c0));
+          invD[r][e] = rcp_pos(fma(dt3, v2, c0));
         }
       level_solve<PR>(qpl, g, q, rhs, invD, ax, ay, ns);
     }

@@ -8,7 +8,7 @@
 namespace snap {
 
 constexpr int kWarp = 32;
-constexpr int kHostChunksMax = 4;   // snap_project_host pipelines the batch in at most this many chunks
+constexpr int kHostChunksMax = 16;   // snap_project_host pipelines the batch in at most this many chunks
 constexpr double kPolishSkip = 1e-3;  // polish skipped when ||h||_inf <= kPolishSkip * tol
 // l1-merit penalty parameter (R2; Nocedal-Wright Eq. 18.36 with sigma = 1, Hessian of f = I):
 //   mu <- max(mu, kMuFloor, (w^T d + 1/2 ||d||^2) / ((1 - kMuRho) ||h||_1))   -- needs no multiplier

@@ -503,33 +503,37 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
 // pivot.  Also returns lam^T (J_b^f w_f) and lam^T rho = y^T D^-1 y (for the penalty parameter).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ bool band_solve(Band bd, int F, double& lam_jw, double& lam_rho) {
-  // forward: factor and L y = rho.  Carried: D, L1 (entry to the row before) and y of the previous two rows.
-  double Dm2 = 1.0, Dm1 = 1.0, L1m1 = 0.0, ym2 = 0.0, ym1 = 0.0;   // rows i-2, i-1
+  // forward: factor and L y = rho.  Carried: 1 / D, L1 (entry to the row before) and y of the previous two rows.  One fast
+  // reciprocal per row (the arrays dE / dM keep 1 / D): the recurrence is serial on one lane, IEEE divisions were 7 per level.
+  double iDm2 = 1.0, iDm1 = 1.0, L1m1 = 0.0, ym2 = 0.0, ym1 = 0.0;   // rows i-2, i-1
   double acc = 0.0;
   bool ok = true;
   for (int f = 0; f < F; ++f) {
     // row E_f (i = 2f): a2 = eE (to E_{f-1} = row i-2), a1 = eM (to M_{f-1} = row i-1)
     {
       const double a2 = bd.eE.get(f), a1 = bd.eM.get(f), a0 = bd.dE.get(f);
-      const double l2 = a2 / Dm2;
-      const double l1 = (a1 - l2 * Dm2 * L1m1) / Dm1;
-      const double D = a0 - l2 * l2 * Dm2 - l1 * l1 * Dm1;
+      const double l2 = a2 * iDm2;                     // l2 D_{i-2} = a2
+      const double t1 = fma(-a2, L1m1, a1);            // l1 D_{i-1}
+      const double l1 = t1 * iDm1;
+      const double D = fma(-l1, t1, fma(-l2, a2, a0));
       const double y = bd.rE.get(f) - l1 * ym1 - l2 * ym2;
       ok = ok && (D > 0.0) && finite_d(D) && finite_d(y);
-      bd.eE.set(f, l2); bd.eM.set(f, l1); bd.dE.set(f, D); bd.rE.set(f, y);
-      acc = fma(y, y / D, acc);
-      Dm2 = Dm1; Dm1 = D; L1m1 = l1; ym2 = ym1; ym1 = y;
+      const double iD = rcp_pos(D);
+      bd.eE.set(f, l2); bd.eM.set(f, l1); bd.dE.set(f, iD); bd.rE.set(f, y);
+      acc = fma(y * y, iD, acc);
+      iDm2 = iDm1; iDm1 = iD; L1m1 = l1; ym2 = ym1; ym1 = y;
     }
     // row M_f (i = 2f+1): a2 = 0 (to M_{f-1}), a1 = mE (to E_f)
     {
       const double a1 = bd.mE.get(f), a0 = bd.dM.get(f);
-      const double l1 = a1 / Dm1;
-      const double D = a0 - l1 * l1 * Dm1;
+      const double l1 = a1 * iDm1;
+      const double D = fma(-l1, a1, a0);
       const double y = bd.rM.get(f) - l1 * ym1;
       ok = ok && (D > 0.0) && finite_d(D) && finite_d(y);
-      bd.mE.set(f, l1); bd.dM.set(f, D); bd.rM.set(f, y);
-      acc = fma(y, y / D, acc);
-      Dm2 = Dm1; Dm1 = D; L1m1 = l1; ym2 = ym1; ym1 = y;
+      const double iD = rcp_pos(D);
+      bd.mE.set(f, l1); bd.dM.set(f, iD); bd.rM.set(f, y);
+      acc = fma(y * y, iD, acc);
+      iDm2 = iDm1; iDm1 = iD; L1m1 = l1; ym2 = ym1; ym1 = y;
     }
   }
   lam_rho = acc;
@@ -541,7 +545,7 @@ __device__ __forceinline__ bool band_solve(Band bd, int F, double& lam_jw, doubl
   for (int f = F - 1; f >= 0; --f) {
     // row M_f (i = 2f+1): rows above it: i+1 = E_{f+1} (L1 = eM[f+1], L2 = eE[f+1] points to E_f), i+2 = M_{f+1} (L2 = 0)
     {
-      const double x = bd.rM.get(f) / bd.dM.get(f) - L1p1 * xp1 - L2p2 * xp2;
+      const double x = bd.rM.get(f) * bd.dM.get(f) - L1p1 * xp1 - L2p2 * xp2;
       bd.lM.set(f, x);
       dot = fma(x, bd.jw.get(F + f), dot);
       xp2 = xp1; xp1 = x;
@@ -550,7 +554,7 @@ __device__ __forceinline__ bool band_solve(Band bd, int F, double& lam_jw, doubl
     }
     // row E_f (i = 2f)
     {
-      const double x = bd.rE.get(f) / bd.dE.get(f) - L1p1 * xp1 - L2p2 * xp2;
+      const double x = bd.rE.get(f) * bd.dE.get(f) - L1p1 * xp1 - L2p2 * xp2;
       bd.lE.set(f, x);
       dot = fma(x, bd.jw.get(f), dot);
       xp2 = xp1; xp1 = x;

@@ -71,16 +71,6 @@ struct Ring2d {
   }
 };
 
-// 1 / d for d of order one (the level diagonal 1 + 2ax + 2ay + dt (3 u^2 - 1) > 0): hardware seed (>= 20 bits) and two
-// Newton steps, no special-case path.  The relaxation only needs a fixed multiplier within a few ulp of 1 / D.
-__device__ __forceinline__ double rcp_pos(double d) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-  r = fma(r, fma(-d, r, 1.0), r);
-  r = fma(r, fma(-d, r, 1.0), r);
-  return r;
-}
-
 // sums a pass returns (block-reduced, identical in every thread)
 struct Pass2d {
   double hinf, h1, f, wd, dd;

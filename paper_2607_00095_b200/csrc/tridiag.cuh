@@ -5,6 +5,7 @@
 
 namespace snap {
 
+// (pivots of the diagonally dominant SPD level matrices are positive and of order one: reciprocals by rcp_pos)
 // ------------------------------------------------------------------------------------------------
 // warp tridiagonal solve (Fisher): rows owned contiguously, Q per lane; partition method —
 // each lane eliminates its Q-1 interior unknowns against its own last unknown (the separator) and the
@@ -20,7 +21,7 @@ __device__ __forceinline__ void warp_tridiag(const double (&a)[Q], const double 
   if (Q > 1) {
     double cp[Q];
     {
-      const double inv = 1.0 / b[0];
+      const double inv = rcp_pos(b[0]);
       cp[0] = (Q > 2 ? c[0] : 0.0) * inv;
       v[0] = d[0] * inv;
       al[0] = a[0] * inv;
@@ -28,7 +29,7 @@ __device__ __forceinline__ void warp_tridiag(const double (&a)[Q], const double 
     }
 #pragma unroll
     for (int j = 1; j < Q - 1; ++j) {
-      const double inv = 1.0 / (b[j] - a[j] * cp[j - 1]);
+      const double inv = rcp_pos(b[j] - a[j] * cp[j - 1]);
       cp[j] = (j < Q - 2 ? c[j] : 0.0) * inv;
       v[j] = (d[j] - a[j] * v[j - 1]) * inv;
       al[j] = (-a[j] * al[j - 1]) * inv;
@@ -58,7 +59,7 @@ __device__ __forceinline__ void warp_tridiag(const double (&a)[Q], const double 
   if (lane == 0) ra = 0.0;
   // parallel cyclic reduction over the 32 lanes, rows kept normalised (rb == 1)
   {
-    const double inv = 1.0 / rb;
+    const double inv = rcp_pos(rb);
     ra *= inv;
     rc *= inv;
     rd *= inv;
@@ -72,7 +73,7 @@ __device__ __forceinline__ void warp_tridiag(const double (&a)[Q], const double 
     if (lane < s) { alo = 0.0; clo = 0.0; dlo = 0.0; }
     if (lane + s > 31) { ahi = 0.0; chi = 0.0; dhi = 0.0; }
     const double nb = 1.0 - clo * ra - ahi * rc;
-    const double inv = 1.0 / nb;
+    const double inv = rcp_pos(nb);
     const double nd = (rd - dlo * ra - dhi * rc) * inv;
     const double na = (-alo * ra) * inv;
     const double nc = (-chi * rc) * inv;

@@ -134,13 +134,13 @@ __device__ __forceinline__ void hess_coeffs(const DevParams& P, double lamE0, do
 template <int Q>
 __device__ __forceinline__ void circ_solve(double a, double b, double (&g)[Q], int lane) {
   if (b == 0.0) {
-    const double ia = 1.0 / a;
+    const double ia = rcp_pos(a);
 #pragma unroll
     for (int c = 0; c < Q; ++c) g[c] *= ia;
     return;
   }
   const double kap = 0.5 * (a + sqrt(a * a - 4.0 * b * b));
-  const double r = -b / kap, ik = 1.0 / kap;
+  const double ik = rcp_pos(kap), r = -b * ik;
   double rp[Q];                       // r^(j+1)
   rp[0] = r;
 #pragma unroll
@@ -157,7 +157,7 @@ __device__ __forceinline__ void circ_solve(double a, double b, double (&g)[Q], i
       T = fma(Rs, __shfl_sync(SNAP_FULL, T, (lane + 32 - s) & 31), T);
       Rs *= Rs;
     }
-    T /= (1.0 - Rs);                  // Rs = R^32 after a complete scan, 0 after a cut-off
+    T *= rcp_pos(1.0 - Rs);           // Rs = R^32 after a complete scan, 0 after a cut-off
 #pragma unroll
     for (int j = 0; j < Q; ++j) g[j] = fma(rp[j], T, g[j]);
   }
@@ -171,7 +171,7 @@ __device__ __forceinline__ void circ_solve(double a, double b, double (&g)[Q], i
       T = fma(Rs, __shfl_sync(SNAP_FULL, T, (lane + s) & 31), T);
       Rs *= Rs;
     }
-    T /= (1.0 - Rs);
+    T *= rcp_pos(1.0 - Rs);
 #pragma unroll
     for (int j = 0; j < Q; ++j) g[j] = fma(rp[Q - 1 - j], T, g[j]);
   }
@@ -265,7 +265,7 @@ __device__ __forceinline__ void fluxk_assemble(const DevParams& P, Band bd, int 
     if constexpr (!HESS) return 1.0;
     double wa, wb;
     hess_coeffs(P, bd.lE.get(f), (f + 1 < F) ? bd.lE.get(f + 1) : 0.0, wa, wb);
-    return 1.0 / (wa + 2.0 * wb);
+    return rcp_pos(wa + 2.0 * wb);
   };
   // predecessor level
   double E_prev = E_K, D_prev = D_K, bb_prev = 0.0, ab_prev = 0.0, bw_prev = 0.0, s1_prev = 0.0, gam_prev = 1.0;

@@ -423,6 +423,63 @@ def test_flow_step_matches_oracle(S, cfg, kw, prm, fused):
         p.destroy()
 
 
+def test_flow_step_non_finite_sample_keeps_the_contract(S):
+    """Status -3 inside a flow step: u1 = u_hat_1 (R16), u_next = the pull-back of that u1, lam = 0; the other sample is unaffected."""
+    dev = torch.device("cuda:0")
+    for cfg, kw in ((5, dict(batch=2, nx=64, nt=16)), (4, dict(batch=2, nx=16, ny=16, nt=4))):
+        wl = W.make_workload(cfg, **kw)
+        tau, taun = 0.5, 0.75
+        u_tau, vel, u0p = _flow_inputs(wl, tau)
+        u_tau[0] *= 1e160                                        # sample 0 overflows in the first linearisation
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        d_ut = u_tau.to(dev)
+        u1, un = torch.full_like(d_ut, float("nan")), torch.full_like(d_ut, float("nan"))
+        lam = torch.full((2, p.m), float("nan"), dtype=torch.float64, device=dev)
+        it = torch.zeros(2, dtype=torch.int32, device=dev)
+        S.snap_flow_step(p, 2, d_ut, vel.to(dev), u0p.to(dev), tau, taun, wl.cdata.to(dev), u1, un, lam, it)
+        torch.cuda.synchronize()
+        assert int(it[0]) == -3 and int(it[1]) > 0
+        uh0 = (u_tau[0] + (1.0 - tau) * vel[0]).numpy()
+        np.testing.assert_array_equal(d_ut[0].cpu().numpy().reshape(uh0.shape), uh0)
+        np.testing.assert_array_equal(u1[0].cpu().numpy().reshape(uh0.shape), uh0)
+        assert float(lam[0].abs().max()) == 0.0
+        exp = u0p[0].numpy() + taun * (uh0 - u0p[0].numpy())
+        np.testing.assert_allclose(un[0].cpu().numpy().reshape(uh0.shape), exp, rtol=1e-15, atol=0)
+        o = O.flow_step(wl.kind, u_tau[1].numpy(), vel[1].numpy(), u0p[1].numpy(), tau, taun, wl.cdata[1].numpy(), wl.params)
+        assert np.abs(un[1].cpu().numpy().reshape(o["u_next"].shape) - o["u_next"]).max() <= TOL_U * np.abs(o["u_next"]).max()
+        p.destroy()
+
+
+def test_exact_hessian_setting_has_no_effect_where_the_rows_are_square(S):
+    """DESIGN.md R22: for kinds 1-4 (and kind 5 without energy rows) J_loc du = -h fixes the step whatever W is: bit-identical results."""
+    for cfg, kw in ((2, dict(batch=2, nx=64, nt=12)), (3, dict(batch=2, nx=64, nt=12)), (4, dict(batch=2, nx=16, ny=16, nt=4)),
+                    (5, dict(batch=2, nx=64, nt=12)), (1, dict(batch=2, nx=20, nt=8)), (7, dict(batch=2, nx=64, nt=14))):
+        wl = W.make_workload(cfg, **kw)
+        a = gpu_project(S, wl, wl.u_hat)
+        b = gpu_project(S, wl, wl.u_hat, params=dict(hessian=1))
+        np.testing.assert_array_equal(a["u"], b["u"])
+        np.testing.assert_array_equal(a["lam"], b["lam"])
+        np.testing.assert_array_equal(a["iters"], b["iters"])
+
+
+def test_exact_hessian_multiplier_free_and_line_search(S):
+    wl = W.make_workload(6, batch=2, nx=32, nt=12, noise=1.0, params=dict(max_iter=400, hessian=1))
+    g = gpu_project(S, wl, wl.u_hat)
+    assert (g["iters"] > 0).all()
+    for b in range(wl.batch):
+        o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+        assert o["status"] == 0
+        assert np.abs(g["u"][b] - o["u"]).max() <= 1e-8 * np.abs(o["u"]).max()
+    dev = torch.device("cuda:0")
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    us = torch.empty_like(wl.u_hat, device=dev)
+    it = torch.zeros(wl.batch, dtype=torch.int32, device=dev)
+    S.snap_project(p, wl.batch, wl.u_hat.to(dev), wl.cdata.to(dev), us, None, it)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(us.cpu().numpy().reshape(g["u"].shape), g["u"])
+    p.destroy()
+
+
 def test_flow_step_rejects_aliased_buffers_and_bad_times(S):
     dev = torch.device("cuda:0")
     wl = W.make_workload(5, batch=2, nx=64, nt=12)

@@ -7,7 +7,7 @@ flow-matching times tau_j = j/50 with the multiplier warm start carried from tau
 One "step" = that whole 50-call sequence = 51 200 projections.  All 50 inputs (25.6 GB) are resident in
 HBM before the timed region, so the working set is far larger than L2 and no L2 flush is needed.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg1..cfg4|cfg6|cfg7] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg1..cfg4|cfg6|cfg7|cfg8] [--impl reference]
 
 Multi-GPU (torchrun): samples are independent blocks, so each rank projects its own
 batch of the same size with no data-path collective ("scaling": "weak"); NCCL carries only the barrier

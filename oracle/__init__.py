@@ -23,7 +23,7 @@ prints no numeric values of any projected field; only the converged (u*, lambda*
 """
 from .constraints import (  # noqa: F401
     residual, jacobian, row_slices, full_rank_rows, num_rows, residual_norms,
-    paper_example_jacobian, godunov_flux, godunov_flux_grad, fluxk_counts, lagrangian_hessian, HESS_SAFEGUARD,
+    paper_example_jacobian, godunov_flux, godunov_flux_grad, fluxk_counts, lagrangian_hessian, HESS_SAFEGUARD, NS2D_VORT_ENST,
 )
 from .linsolve import (  # noqa: F401
     solve_kkt_dense_lu, solve_schur_pinv, solve_schur_banded_cholesky, solve_schur_cg, solve_schur_dense_cholesky,

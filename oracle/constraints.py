@@ -25,6 +25,7 @@ FISHER1D_IE = 2
 ALLENCAHN2D_IE = 3
 BURGERS1D_LF_MASS = 4
 BURGERS1D_FLUXK = 5
+NS2D_VORT_ENST = 6
 
 _HAS_MASS = (HEAT1D_IC_MASS, BURGERS1D_LF_MASS)
 
@@ -46,6 +47,17 @@ _HAS_MASS = (HEAT1D_IC_MASS, BURGERS1D_LF_MASS)
 # (each energy row couples two consecutive levels) and Gauss-Newton with W = I converges only linearly.
 
 
+# Kind 6, NS2D_VORT_ENST — the paper's Navier-Stokes constraint set (Eq. 20; Table row "IC | Mass | Enstrophy" L684):
+#   IC block        [ny][nx] : w[0] - w_IC
+#   vorticity block [nt-1]   : dx dy sum w[k] - dx dy sum w_IC            (total vorticity, "vorticity-mass", k = 1..nt-1)
+#   enstrophy block [nt-1]   : dx dy sum w[k]^2 - dx dy sum w_IC^2        (Eq. 20 as printed: no factor 1/2)
+# Riemann sums over all nodes (R7); the rows of level 0 are implied by the IC rows and omitted as the paper omits its
+# implied first row (L493).  No local PDE rows: every level k >= 1 is constrained only by its two global rows, so the
+# levels decouple and the projection of one level is the projection onto a sphere inside a hyperplane:
+#     w* = m + (r / ||dev||) dev ,  m = mean(w_IC), r = ||w_IC - m||_2, dev = w_hat - mean(w_hat)
+# (tests/test_oracle_ns.py pins the generic Newton-KKT route against this closed form).
+
+
 def fluxk_counts(p: dict, nt: int):
     """(K, F, E): flux steps, free levels, energy rows of kind 5."""
     K = int(p.get("flux_steps", 0))
@@ -61,6 +73,8 @@ def num_rows(kind: int, nx: int, ny: int, nt: int, p: dict = None) -> int:
     if kind == BURGERS1D_FLUXK:
         K, F, E = fluxk_counts(p, nt)
         return (K + 1) * nx + F + E
+    if kind == NS2D_VORT_ENST:
+        return nx * ny + 2 * (nt - 1)
     n = nx * ny * nt
     return n + nt if kind == BURGERS1D_LF_MASS else n
 
@@ -74,6 +88,9 @@ def row_slices(kind: int, nx: int, ny: int, nt: int, p: dict = None):
         K, F, E = fluxk_counts(p, nt)
         loc = (K + 1) * nx
         return {"ic": slice(0, nx), "pde": slice(nx, loc), "mass": slice(loc, loc + F), "energy": slice(loc + F, loc + F + E)}
+    if kind == NS2D_VORT_ENST:       # "mass" = total-vorticity rows, "energy" = enstrophy rows
+        return {"ic": slice(0, lvl), "pde": slice(lvl, lvl), "mass": slice(lvl, lvl + nt - 1),
+                "energy": slice(lvl + nt - 1, lvl + 2 * (nt - 1))}
     n = lvl * nt
     mass = slice(n, n + nt) if kind == BURGERS1D_LF_MASS else slice(n, n)
     return {"ic": slice(0, lvl), "pde": slice(lvl, n), "mass": mass}
@@ -88,8 +105,8 @@ def full_rank_rows(kind: int, nx: int, ny: int, nt: int, p: dict = None) -> np.n
     tests/test_oracle_pins.py verifies both statements by numerical rank on tiny grids."""
     m = num_rows(kind, nx, ny, nt, p)
     keep = np.ones(m, dtype=bool)
-    if kind == BURGERS1D_FLUXK:
-        return keep                      # implied rows are not part of this kind's row set
+    if kind in (BURGERS1D_FLUXK, NS2D_VORT_ENST):
+        return keep                      # implied rows are not part of these kinds' row sets
     s = row_slices(kind, nx, ny, nt)["mass"]
     if kind == HEAT1D_IC_MASS:
         keep[s.start] = False
@@ -161,6 +178,12 @@ def residual(kind: int, u: np.ndarray, u0: np.ndarray, p: dict) -> np.ndarray:
     ic = (u[0] - u0).ravel()
     if kind == HEAT1D_IC_MASS:
         return np.concatenate([ic, _mass_rows(u, u0, dx)])
+    if kind == NS2D_VORT_ENST:
+        a = dx * p["dy"]
+        s1, s2 = math.fsum(u0.ravel().tolist()), math.fsum((u0 * u0).ravel().tolist())
+        vort = [a * (math.fsum(u[k].ravel().tolist()) - s1) for k in range(1, nt)]
+        enst = [a * (math.fsum((u[k] * u[k]).ravel().tolist()) - s2) for k in range(1, nt)]
+        return np.concatenate([ic, np.array(vort, dtype=np.float64), np.array(enst, dtype=np.float64)])
     if kind == BURGERS1D_FLUXK:
         K, F, E = fluxk_counts(p, nt)
         loc = [ic] + [_fv_step_residual(u[k, 0], u[k + 1, 0], p) for k in range(K)]
@@ -298,6 +321,11 @@ def jacobian(kind: int, u: np.ndarray, p: dict) -> sp.csr_matrix:
             add(r, base + xm, -ax)
             add(r, base + yp, -ay)
             add(r, base + ym, -ay)
+    elif kind == NS2D_VORT_ENST:
+        a = dx * p["dy"]
+        for k in range(1, nt):
+            add(np.full(lvl, lvl + (k - 1)), k * lvl + cell, a)                          # total vorticity: a 1
+            add(np.full(lvl, lvl + (nt - 1) + (k - 1)), k * lvl + cell, 2.0 * a * u[k].ravel())   # enstrophy: 2 a w
     elif kind != HEAT1D_IC_MASS:
         raise ValueError(f"unknown kind {kind}")
 
@@ -343,6 +371,15 @@ def lagrangian_hessian(kind: int, u: np.ndarray, lam: np.ndarray, p: dict) -> sp
     u = np.asarray(u, dtype=np.float64)
     nt, ny, nx = u.shape
     n = nt * ny * nx
+    if kind == NS2D_VORT_ENST:       # enstrophy row of level k: grad^2 = 2 dx dy I on that level => W_k = (1 + 2 a lam_Z[k]) I
+        a = p["dx"] * p["dy"]
+        lamZ = np.asarray(lam, dtype=np.float64)[row_slices(kind, nx, ny, nt, p)["energy"]]
+        diag = np.ones(n)
+        for k in range(1, nt):
+            wk = 1.0 + 2.0 * a * lamZ[k - 1]
+            if wk >= HESS_SAFEGUARD:
+                diag[k * ny * nx:(k + 1) * ny * nx] = wk
+        return sp.diags(diag, format="csr")
     if kind != BURGERS1D_FLUXK:
         return sp.identity(n, format="csr")
     K, F, E = fluxk_counts(p, nt)

@@ -76,7 +76,7 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
     nt, ny, nx = u_hat.shape
     if backend == "auto":
         # kind 5: few rows (m ~ (K+1) nx + 2 nt) with dense border rows: dense Cholesky of the assembled J J^T
-        backend = {C.ALLENCAHN2D_IE: "cg", C.BURGERS1D_FLUXK: "dense_chol"}.get(kind, "banded")
+        backend = {C.ALLENCAHN2D_IE: "cg", C.BURGERS1D_FLUXK: "dense_chol", C.NS2D_VORT_ENST: "banded"}.get(kind, "banded")
     keep = C.full_rank_rows(kind, nx, ny, nt, p)
     tol = p.get("tol", 1e-10)
     max_iter = int(p.get("max_iter", 50))
@@ -148,7 +148,7 @@ def project(kind: int, u_hat: np.ndarray, u0: np.ndarray, p: dict, backend: str 
         # stationarity, so convergence also asks for a small step, RMS(d) <= tol (R18).  For the square
         # kinds d = -J^-1 h and the paper's/north_star's rule ||h||_inf < tol stands alone.
         small_step = True
-        if kind == C.BURGERS1D_FLUXK:
+        if kind in (C.BURGERS1D_FLUXK, C.NS2D_VORT_ENST):
             d0 = u_full - u
             small_step = float(d0 @ d0) <= d0.size * tol * tol
         if hinf < tol and small_step:

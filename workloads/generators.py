@@ -27,9 +27,10 @@ KIND_FISHER1D_IE = 2
 KIND_ALLENCAHN2D_IE = 3
 KIND_BURGERS1D_LF_MASS = 4
 KIND_BURGERS1D_FLUXK = 5
+KIND_NS2D_VORT_ENST = 6
 KIND_NAMES = {
     0: "HEAT1D_IC_MASS", 1: "BURGERS1D_LF", 2: "FISHER1D_IE",
-    3: "ALLENCAHN2D_IE", 4: "BURGERS1D_LF_MASS", 5: "BURGERS1D_FLUXK",
+    3: "ALLENCAHN2D_IE", 4: "BURGERS1D_LF_MASS", 5: "BURGERS1D_FLUXK", 6: "NS2D_VORT_ENST",
 }
 
 # cfg -> (kind, batch, nx, ny, nt, seed)   (BASELINE.json configs[0..4] = cfg 1..5)
@@ -44,6 +45,9 @@ CONFIG_SHAPES = {
     6: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1006),   # Lax-Friedrichs flux rows + energy-evolution rows (Eq. 11)
     7: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1007),   # Godunov flux rows (L555), inviscid, no energy rows
     8: (KIND_BURGERS1D_FLUXK, 1024, 256, 1, 256, 1006),   # config 6 (same inputs) with the exact Lagrangian Hessian (NEXT-2)
+    # the paper's Navier-Stokes row set (Eq. 20: IC + total vorticity + enstrophy) at the paper's grid 16 x 16 x 50
+    # (L398); the paper samples 2 fields, here a batch of 256
+    9: (KIND_NS2D_VORT_ENST, 256, 16, 16, 50, 1009),
 }
 CONFIG_EXTRA = {6: dict(flux_steps=5, energy_rows=1, flux_kind=0),
                 7: dict(flux_steps=5, energy_rows=0, flux_kind=1, nu=0.0),
@@ -68,6 +72,8 @@ def default_params(kind: int, nx: int, ny: int, nt: int) -> Dict[str, float]:
         p.update(dx=1.0 / nx, dt=1.0 / max(nt - 1, 1), D=0.01, rho=1.0)
     elif kind == KIND_ALLENCAHN2D_IE:
         p.update(dx=1.0 / nx, dy=1.0 / ny, dt=1e-3, eps=0.05)
+    elif kind == KIND_NS2D_VORT_ENST:
+        p.update(dx=1.0 / nx, dy=1.0 / ny, dt=1.0)       # Omega = [0, 1]^2, unit time step (Eq. 19)
     else:
         raise ValueError(f"unknown kind {kind}")
     return p
@@ -103,6 +109,8 @@ class Workload:
             K = int(self.params["flux_steps"])
             F = self.nt - 1 - K
             return (K + 1) * self.nx + F * (2 if int(self.params["energy_rows"]) else 1)
+        if self.kind == KIND_NS2D_VORT_ENST:
+            return self.nx * self.ny + 2 * (self.nt - 1)
         return self.n
 
 
@@ -297,6 +305,21 @@ def make_workload(cfg: int, batch: Optional[int] = None, nx: Optional[int] = Non
         u_true[:, 0] = u0
         for k in range(nt - 1):
             u_true[:, k + 1] = _allencahn_ie_step(u_true[:, k], p["dx"], p["dy"], p["dt"], p["eps"])
+        sigma = 0.05 if noise is None else noise
+    elif kind == KIND_NS2D_VORT_ENST:
+        # IC: a random Fourier field as for cfg 4 plus a non-zero mean; clean field: the IC advected by one cell per
+        # step (a periodic shift keeps sum w and sum w^2, so it is feasible for Eq. 20 whatever the flow is)
+        x = torch.arange(nx, dtype=F64, device=dev) * p["dx"]
+        y = torch.arange(ny, dtype=F64, device=dev) * p["dy"]
+        modes = [(kx, ky) for kx in range(-3, 4) for ky in range(-3, 4) if 0 < kx * kx + ky * ky <= 9]
+        coef = torch.randn(B, len(modes), 2, generator=g, dtype=F64, device=dev)
+        mean = 0.2 * torch.randn(B, 1, 1, generator=g, dtype=F64, device=dev)
+        u0 = torch.zeros(B, ny, nx, dtype=F64, device=dev)
+        for mi, (kx, ky) in enumerate(modes):
+            ph = 2.0 * math.pi * (kx * x[None, :] + ky * y[:, None])
+            u0 += coef[:, mi, 0, None, None] * torch.cos(ph)[None] + coef[:, mi, 1, None, None] * torch.sin(ph)[None]
+        u0 = u0 / u0.abs().amax((-1, -2), keepdim=True) + mean
+        u_true = torch.stack([torch.roll(u0, shifts=(k % ny, (2 * k) % nx), dims=(-2, -1)) for k in range(nt)], dim=1)
         sigma = 0.05 if noise is None else noise
     else:
         raise ValueError(kind)

@@ -160,7 +160,7 @@ def run_reference(args):
     cfg = int(args.workload[3:])
     cores = os.cpu_count() or 1
     workers = min(cores, 16)
-    n_samples = workers if cfg in (4, 5, 6, 7, 8) else max(workers, 16)
+    n_samples = workers if cfg in (4, 5, 6, 7, 8, 9) else max(workers, 16)
     times = []
     desc = ""
     for s in range(args.warmup + args.steps):
@@ -192,6 +192,7 @@ def workload_name(cfg: int) -> str:
         6: "cfg6 (SURVEY 8(f) NEXT-1): Burgers IC + Flux(k=5, Lax-Friedrichs) + mass + energy rows, batch 1024, 256x256 (wide J, banded border solve)",
         7: "cfg7 (SURVEY 8(f) NEXT-1/4): inviscid Burgers IC + Flux(k=5, Godunov) + mass rows, batch 1024, 256x256",
         8: "cfg8 (SURVEY 8(f) NEXT-2): cfg6 with the exact Lagrangian Hessian (Newton-KKT, quadratic rate)",
+        9: "cfg9 (paper Eq. 20): 2D Navier-Stokes vorticity rows IC + total vorticity + enstrophy, batch 256, 16x16x50 (closed form per level)",
     }[cfg]
 
 
@@ -362,7 +363,7 @@ KERNEL_NAMES = {5: "project1d_fused_kernel<KB,1,8,3> (Burgers family, nx=256)", 
                 3: "project1d_fused_kernel<KF,1,4,3> (Fisher, nx=128)",
                 4: "project2d_direct_kernel<4,256> (variant 6; variant 5 = project2d_kernel, PCG)",
                 1: "heat_project_kernel", 6: "project1d_fluxk_kernel<8,LF>", 7: "project1d_fluxk_kernel<8,Godunov>",
-                8: "project1d_fluxk_kernel<8,LF> (hessian = 1)"}
+                8: "project1d_fluxk_kernel<8,LF> (hessian = 1)", 9: "ns_project_kernel"}
 
 
 def roofline_of(run, cfg, kern_s, alg_bytes_call, steps, peak, peak_src):
@@ -457,7 +458,7 @@ def run_gpu(args):
         cores = os.cpu_count() or 1
         workers = min(cores, 16)
         taus = (1, 25, 49) if cfg == 5 else (25,)
-        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5, 6, 7, 8) else max(workers, 16), workers, taus=taus)
+        v, dt, desc, used = oracle_sample(cfg, workers if cfg in (4, 5, 6, 7, 8, 9) else max(workers, 16), workers, taus=taus)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "host_cpu_count": cores, "kind": "oracle",
                                 "sample": desc, "seconds": dt}
     if rank == 0 and world == 1 and args.others:
@@ -479,7 +480,7 @@ def run_gpu(args):
         line["flow_step"] = flow_step_lines(run, args.steps, args.warmup)
     if rank == 0 and world == 1 and args.others and cfg == 5:
         others = {}
-        for c in (1, 2, 3, 4, 6, 7, 8):
+        for c in (1, 2, 3, 4, 6, 7, 8, 9):
             r = GpuRun(S, c, dev)
             ms, km, _ = time_steps(r, 5, 3, None)
             okc, hm, itc = r.check()
@@ -492,7 +493,8 @@ def run_gpu(args):
                                           4: "64 samples, 64 MiB per field; 64 CTAs on 148 SMs: level solves bound by shared-memory latency (DESIGN.md 6.2)",
                                           6: "not a BASELINE.json config: the paper's IC + Mass + Flux(k=5) row set with energy rows at cfg-5 scale",
                                           7: "not a BASELINE.json config: Godunov flux variant",
-                                          8: "cfg6's inputs and row set, exact Lagrangian Hessian on the free levels (circulant tridiagonal solves per level)"}[c]}
+                                          8: "cfg6's inputs and row set, exact Lagrangian Hessian on the free levels (circulant tridiagonal solves per level)",
+                                          9: "the paper's Navier-Stokes row set at its own grid; 25 MiB per field: fits L2, latency-bound"}[c]}
             del r
         line["other_workloads"] = others
     if rank == 0:
@@ -518,7 +520,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "cfg6", "cfg7", "cfg8"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "cfg6", "cfg7", "cfg8", "cfg9"])
     ap.add_argument("--impl", default="snap", choices=["snap", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

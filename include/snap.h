@@ -62,6 +62,11 @@ enum {
                                  Godunov flux, L555), a mass row per later level, optionally the energy-evolution row
                                  of Eq. 11 (L336, L603-607) per later step.  J is wide; the border rows are genuinely
                                  coupled (banded SPD Schur complement, banded Cholesky)       */
+  ,
+  SNAP_NS2D_VORT_ENST = 6     /* the paper's Navier-Stokes row set (Eq. 20): IC rows, total vorticity and enstrophy
+                                 (dx dy sum w, dx dy sum w^2) of every later level.  No local PDE rows: the levels decouple
+                                 and each is projected onto a sphere inside a hyperplane in closed form (2D, nx ny <= 4096,
+                                 nt <= 2048).  m = ny nx + 2 (nt-1): [IC][vorticity nt-1][enstrophy nt-1]              */
 };
 
 /* Return codes. */
@@ -89,7 +94,8 @@ enum {
   SNAP_VAR_FUSED_TMA = 4,        /* project1d_fused_kernel, tensor-map TMA rows, several GN iterations per pass   */
   SNAP_VAR_PCG2D = 5,            /* project2d_kernel: PCG on J J^T (precond 0, 1, 2)                              */
   SNAP_VAR_DIRECT2D = 6,         /* project2d_direct_kernel: product-form sweeps with in-SMEM level solves        */
-  SNAP_VAR_FLUXK_BAND = 7        /* project1d_fluxk_kernel: product form on the pinned levels + banded border solve */
+  SNAP_VAR_FLUXK_BAND = 7,       /* project1d_fluxk_kernel: product form on the pinned levels + banded border solve */
+  SNAP_VAR_NS_CLOSED_FORM = 8    /* ns_project_kernel: per-level sphere-in-hyperplane projection (kind 6)             */
 };
 
 /* Slots of one sample's work-counter record (snap_project_stats), 8 x int64. */
@@ -205,7 +211,7 @@ int snap_project_host(snap_problem* p, int batch, const double* u_hat_host, cons
                       double* u_star_host, double* lambda_host, int* iters_host, int warm, snap_stream stream);
 
 /* Constraint residual and the per-type norms of the paper's constraint-error metric
- * (Eq. 27).
+ * (Eq. 27).  Kind 6: the mass slot holds the total-vorticity rows, the energy slot the enstrophy rows.
  *   h      dev [batch][m] or NULL.
  *   norms  dev [batch][5] or NULL: ||h||_inf, ||h_IC||_2, ||h_PDE||_2, ||h_mass||_2, ||h_energy||_2 (0 where a type
  *          is absent). */

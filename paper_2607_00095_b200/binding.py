@@ -8,12 +8,12 @@ from typing import Dict, Optional
 HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(HERE, "libsnap.so")
 
-HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS, BURGERS1D_FLUXK = range(6)
+HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS, BURGERS1D_FLUXK, NS2D_VORT_ENST = range(7)
 # include/snap.h SNAP_STAT_* (slots of one sample's work-counter record) and SNAP_VAR_* (kernel variants)
 (STAT_LINEARISATIONS, STAT_PASSES, STAT_ROWS_READ, STAT_ROWS_WRITTEN, STAT_VARIANT, STAT_INNER, STAT_ROW_DOUBLES,
  STAT_BACKTRACKS, STAT_COUNT) = range(9)
 (VAR_NONE, VAR_HEAT_CLOSED_FORM, VAR_CLASSIC_BULK, VAR_CLASSIC_PLAIN, VAR_FUSED_TMA, VAR_PCG2D, VAR_DIRECT2D,
- VAR_FLUXK_BAND) = range(8)
+ VAR_FLUXK_BAND, VAR_NS_CLOSED_FORM) = range(9)
 
 EXPORTS = [
     "snap_params_default", "snap_problem_create", "snap_problem_destroy", "snap_num_unknowns", "snap_num_rows",

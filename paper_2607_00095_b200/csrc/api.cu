@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "kernels_misc.cuh"
+#include "kernels_ns.cuh"
 #include "launch.h"
 #include "snap_internal.h"
 
@@ -17,7 +18,7 @@ namespace {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-bool is_1d(int kind) { return kind != SNAP_ALLENCAHN2D_IE; }
+bool is_1d(int kind) { return kind != SNAP_ALLENCAHN2D_IE && kind != SNAP_NS2D_VORT_ENST; }
 
 // Green's function of the cyclic tridiagonal (-a, 1+2a, -a) of size N, truncated where it drops below
 // kGreenTol of its peak; g[t], t = 0..K, applied symmetrically (t = -K..K).
@@ -218,7 +219,8 @@ void snap_params_default(snap_params* p) {
 
 int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, const snap_params* prm) {
   if (!out || !prm) return SNAP_EINVAL;
-  if (kind < SNAP_HEAT1D_IC_MASS || kind > SNAP_BURGERS1D_FLUXK) return SNAP_EINVAL;
+  if (kind < SNAP_HEAT1D_IC_MASS || kind > SNAP_NS2D_VORT_ENST) return SNAP_EINVAL;
+  if (kind == SNAP_NS2D_VORT_ENST && nt > kNsMaxLevels) return SNAP_EINVAL;
   if (kind == SNAP_BURGERS1D_FLUXK) {
     if (!(nx == 32 || nx == 64 || nx == 128 || nx == 256) || nt > 512) return SNAP_EINVAL;
     if (prm->flux_steps < 0 || prm->flux_steps > nt - 1) return SNAP_EINVAL;
@@ -247,6 +249,7 @@ int snap_problem_create(snap_problem** out, int kind, int nx, int ny, int nt, co
   d.n = d.lvl * nt;
   d.has_mass = (kind == SNAP_HEAT1D_IC_MASS || kind == SNAP_BURGERS1D_LF_MASS);
   d.m = (kind == SNAP_HEAT1D_IC_MASS) ? nx + nt : d.n + (d.has_mass ? nt : 0);
+  if (kind == SNAP_NS2D_VORT_ENST) d.m = d.lvl + 2 * (nt - 1);
   if (kind == SNAP_BURGERS1D_FLUXK) {
     d.fk_K = prm->flux_steps; d.fk_energy = prm->energy_rows; d.fk_flux = prm->flux_kind;
     d.fk_hess = (prm->hessian == 1 && prm->energy_rows == 1) ? 1 : 0;
@@ -324,7 +327,7 @@ size_t snap_workspace_bytes(const snap_problem* p, int batch) {
   const size_t head = 256 + stats_bytes(B);   // alignment slack + work counters
   // tail: a multiplier array for multiplier-free calls (lambda == NULL) served by a kernel that needs the storage
   const size_t lam_scratch = align_up(B * (size_t)p->dp.m * 8, 256);
-  if (p->dp.kind == SNAP_HEAT1D_IC_MASS) return head + lam_scratch;
+  if (p->dp.kind == SNAP_HEAT1D_IC_MASS || p->dp.kind == SNAP_NS2D_VORT_ENST) return head + lam_scratch;
   if (p->dp.kind == SNAP_ALLENCAHN2D_IE) return head + align_up(B * n * 8 * kPcgVectors, 256) + lam_scratch;
   return head + align_up(B * n * 8, 256) * 2 + aux_bytes(p, B) + lam_scratch;
 }
@@ -367,6 +370,13 @@ static int project_impl(const snap_problem* cp, int batch, const double* u_hat, 
     int rc = flow_unfused_shoot(p, batch, u_hat, flow, st);
     if (rc != SNAP_OK) return rc;
     heat_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lam_any, iters, stats);
+    rc = check_launch(p);
+    return rc != SNAP_OK ? rc : flow_unfused_pullback(p, batch, u_star, flow, st);
+  }
+  if (d.kind == SNAP_NS2D_VORT_ENST) {     // closed form per level; lambda == NULL: the multipliers are simply not written
+    int rc = flow_unfused_shoot(p, batch, u_hat, flow, st);
+    if (rc != SNAP_OK) return rc;
+    ns_project_kernel<<<batch, kMiscThreads, 0, st>>>(d, batch, u_hat, cdata, u_star, lambda, iters, stats);
     rc = check_launch(p);
     return rc != SNAP_OK ? rc : flow_unfused_pullback(p, batch, u_star, flow, st);
   }
@@ -551,6 +561,10 @@ int snap_residual(const snap_problem* cp, int batch, const double* u, const doub
     p->launches++;
     return launch_residual_fluxk(p->dp, batch, u, cdata, h, norms, static_cast<cudaStream_t>(stream));
   }
+  if (p->dp.kind == SNAP_NS2D_VORT_ENST) {
+    ns_residual_kernel<<<batch, kMiscThreads, 0, static_cast<cudaStream_t>(stream)>>>(p->dp, batch, u, cdata, h, norms);
+    return check_launch(p);
+  }
   residual_kernel<<<batch, kMiscThreads, 0, static_cast<cudaStream_t>(stream)>>>(p->dp, batch, u, cdata, h, norms);
   return check_launch(p);
 }
@@ -561,7 +575,7 @@ int snap_schur_apply(const snap_problem* cp, int batch, const double* u, const d
   if (!p || batch < 0) return SNAP_EINVAL;
   if (batch == 0) return SNAP_OK;
   if (!u || !x || !out || !workspace) return SNAP_EINVAL;
-  if (p->dp.kind == SNAP_BURGERS1D_FLUXK) return SNAP_EINVAL;   // kinds 0-4 only (include/snap.h)
+  if (p->dp.kind >= SNAP_BURGERS1D_FLUXK) return SNAP_EINVAL;   // kinds 0-4 only (include/snap.h)
   if (workspace_bytes < (size_t)batch * p->dp.n * 8) return SNAP_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   double* g = static_cast<double*>(workspace);

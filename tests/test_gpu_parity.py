@@ -495,6 +495,51 @@ def test_flow_step_rejects_aliased_buffers_and_bad_times(S):
     p.destroy()
 
 
+# ------------------------------------------------------------------------------------------------
+# kind 6, NS2D_VORT_ENST (Eq. 20): closed-form per-level projection against the oracle's generic Newton-KKT route
+# ------------------------------------------------------------------------------------------------
+def test_ns_vorticity_enstrophy_matches_oracle(S):
+    dev = torch.device("cuda:0")
+    for kw in [dict(batch=3, nx=8, ny=6, nt=7), dict(batch=2, nx=16, ny=16, nt=50), dict(batch=2, nx=64, ny=64, nt=3),
+               dict(batch=2, nx=12, ny=10, nt=2)]:
+        wl = W.make_workload(9, **kw)
+        g = gpu_project(S, wl, wl.u_hat)
+        assert (g["iters"] == 1).all()
+        assert g["norms"][:, 0].max() < 1e-12
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        assert p.m == wl.m == O.num_rows(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        h = torch.empty(wl.batch, p.m, dtype=torch.float64, device=dev)
+        nrm = torch.empty(wl.batch, 5, dtype=torch.float64, device=dev)
+        S.snap_residual(p, wl.batch, wl.u_hat.to(dev), wl.cdata.to(dev), h, nrm)
+        torch.cuda.synchronize()
+        for b in range(wl.batch):
+            uh, u0 = wl.u_hat[b].numpy(), wl.cdata[b].numpy()
+            h_ref = O.residual(wl.kind, uh, u0, wl.params)
+            np.testing.assert_allclose(h[b].cpu().numpy(), h_ref, rtol=0, atol=1e-13 * max(1, np.abs(h_ref).max()))
+            np.testing.assert_allclose(nrm[b].cpu().numpy(), O.residual_norms(wl.kind, uh, u0, wl.params), rtol=1e-12, atol=1e-15)
+            o = O.project(wl.kind, uh, u0, dict(wl.params, hessian=1))
+            assert o["status"] == 0
+            assert np.abs(g["u"][b] - o["u"]).max() <= TOL_U * np.abs(o["u"]).max()
+            assert rel_lam(g["lam"][b], o["lam"]) <= TOL_L
+            ks, _ = kkt_invariants(wl, uh, g["u"][b], g["lam"][b])
+            assert ks <= TOL_KKT
+        p.destroy()
+    # feasible input (a shifted IC): returned to rounding, zero multipliers; in place; multiplier-free; non-finite sample
+    wl = W.make_workload(9, batch=2, nx=16, ny=16, nt=6)
+    g = gpu_project(S, wl, wl.u_true)
+    np.testing.assert_allclose(g["u"], wl.u_true.numpy(), rtol=0, atol=1e-14)
+    assert np.abs(g["lam"]).max() <= 1e-11
+    ref = gpu_project(S, wl, wl.u_hat)
+    inp = gpu_project(S, wl, wl.u_hat.clone(), in_place=True)
+    np.testing.assert_array_equal(inp["u"], ref["u"])
+    big = wl.u_hat.clone(); big[0] *= 1e200
+    gb = gpu_project(S, wl, big, in_place=True)
+    assert int(gb["iters"][0]) == -3 and int(gb["iters"][1]) == 1
+    np.testing.assert_array_equal(gb["u"][0], big[0].numpy())
+    assert np.all(gb["lam"][0] == 0)
+    np.testing.assert_array_equal(gb["u"][1], ref["u"][1])
+
+
 def test_direct2d_matches_oracle_and_pcg_path(S):
     """Kind 3, product-form path (in-SMEM red-black level solves): same limit point as the oracle
     and as the PCG kernel (gn_fuse = -1) on 2-row and 4-row patches, one and several warps, nt = 2."""

@@ -204,6 +204,18 @@ int snap_flow_step(const snap_problem* p, int batch, double* u_tau, const double
                    double tau_next, const double* cdata, double* u1, double* u_next, double* lambda, int* iters,
                    void* workspace, size_t workspace_bytes, snap_stream stream);
 
+/* Float32 mode (the paper's models are Float32 with solver tolerance 1e-5): the
+ * multiplier-free projection of the Burgers kinds (BURGERS1D_LF, BURGERS1D_LF_MASS; nx in {32, 64, 128, 256}) computed
+ * entirely in fp32 -- same method (forward passes carrying several Gauss-Newton iterations per level), full steps, stop
+ * when ||h||_inf < tol (local and mass rows) and `polish` more steps were taken.  All field buffers are fp32, 16-byte aligned:
+ *   u_hat dev [batch][nt][nx] in (may alias u_star), cdata dev [batch][nx] in, u_star dev [batch][nt][nx] out,
+ *   iters dev [batch] out: residual evaluations used, or SNAP_ST_MAXITER / SNAP_ST_NONFINITE (u* = u_hat) /
+ *   SNAP_ST_LINESEARCH (a full step that did not reduce ||h||_inf; u* = the iterate before it).
+ *   tol > 0 (the paper's 1e-5); workspace as snap_project (only 2 n floats per sample are used).
+ * Other kinds / sizes: SNAP_EINVAL. */
+int snap_project_f32(const snap_problem* p, int batch, const float* u_hat, const float* cdata, float* u_star, int* iters,
+                     float tol, void* workspace, size_t workspace_bytes, snap_stream stream);
+
 /* Same computation with HOST buffers (pinned or pageable): copies inputs to a device staging area owned by
  * the handle, runs snap_project, copies u_star / lambda / iters back, and synchronises `stream` before
  * returning.  lambda is read only if warm != 0; lambda_host == NULL = multiplier-free call (no lambda copy either way). */

@@ -18,7 +18,7 @@ HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS, BU
 EXPORTS = [
     "snap_params_default", "snap_problem_create", "snap_problem_destroy", "snap_num_unknowns", "snap_num_rows",
     "snap_workspace_bytes", "snap_project", "snap_project_host", "snap_residual", "snap_schur_apply",
-    "snap_project_stats", "snap_launch_count", "snap_strerror", "snap_flow_step",
+    "snap_project_stats", "snap_launch_count", "snap_strerror", "snap_flow_step", "snap_project_f32",
 ]
 
 
@@ -76,6 +76,8 @@ def load_library():
     lib.snap_project.restype = C.c_int
     lib.snap_flow_step.argtypes = [vp, C.c_int, dp, dp, dp, C.c_double, C.c_double, dp, dp, dp, dp, ip, vp, C.c_size_t, vp]
     lib.snap_flow_step.restype = C.c_int
+    lib.snap_project_f32.argtypes = [vp, C.c_int, vp, vp, vp, ip, C.c_float, vp, C.c_size_t, vp]
+    lib.snap_project_f32.restype = C.c_int
     lib.snap_project_host.argtypes = [vp, C.c_int, dp, dp, dp, dp, ip, C.c_int, vp]
     lib.snap_project_host.restype = C.c_int
     lib.snap_residual.argtypes = [vp, C.c_int, dp, dp, dp, dp, vp]
@@ -224,6 +226,22 @@ def snap_flow_step(p: Problem, batch: int, u_tau, vel, u_prior, tau: float, tau_
                                        _ptr(cdata), _ptr(u1), _ptr(u_next), _ptr(lam), _ptr(iters), _ptr(workspace),
                                        _nbytes(workspace), _stream_handle(stream))
     _check(rc, "snap_flow_step")
+    return workspace
+
+
+def snap_project_f32(p: Problem, batch: int, u_hat, cdata, u_star, iters, tol: float = 1e-5, workspace=None, stream=None):
+    """Float32 mode (include/snap.h): multiplier-free projection of the Burgers kinds in fp32; torch.float32 CUDA tensors."""
+    import torch
+    for name, t, ne, dt in (("u_hat", u_hat, batch * p.n, torch.float32), ("cdata", cdata, batch * p.nx * p.ny, torch.float32),
+                            ("u_star", u_star, batch * p.n, torch.float32), ("iters", iters, batch, torch.int32)):
+        _need(t, ne, name, dt)
+        if not t.is_cuda:
+            raise SnapError(f"{name} must be a CUDA tensor")
+    if workspace is None:
+        workspace = torch.empty(snap_workspace_bytes(p, batch), dtype=torch.uint8, device=u_hat.device)
+    rc = load_library().snap_project_f32(p.handle, int(batch), _ptr(u_hat), _ptr(cdata), _ptr(u_star), _ptr(iters), float(tol),
+                                         _ptr(workspace), _nbytes(workspace), _stream_handle(stream))
+    _check(rc, "snap_project_f32")
     return workspace
 
 

@@ -13,8 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsnap.so")
-SOURCES = ["api.cu", "proj1d_burgers.cu", "proj1d_burgers_fused.cu", "proj1d_fisher.cu", "proj1d_fisher_fused.cu", "proj1d_fluxk.cu", "proj2d.cu", "proj2d_direct.cu"]
-HEADERS = ["snap_internal.h", "launch.h", "device_utils.cuh", "kernels_1d.cuh", "kernels_1d_fused.cuh", "kernels_1d_fluxk.cuh", "tridiag.cuh", "kernels_2d.cuh", "kernels_2d_direct.cuh", "kernels_misc.cuh", "kernels_ns.cuh",
+SOURCES = ["api.cu", "proj1d_burgers.cu", "proj1d_burgers_fused.cu", "proj1d_fisher.cu", "proj1d_fisher_fused.cu", "proj1d_fluxk.cu", "proj2d.cu", "proj2d_direct.cu", "proj1d_f32.cu"]
+HEADERS = ["snap_internal.h", "launch.h", "device_utils.cuh", "kernels_1d.cuh", "kernels_1d_fused.cuh", "kernels_1d_fluxk.cuh", "tridiag.cuh", "kernels_2d.cuh", "kernels_2d_direct.cuh", "kernels_misc.cuh", "kernels_ns.cuh", "kernels_1d_f32.cuh",
            os.path.join("..", "..", "include", "snap.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 

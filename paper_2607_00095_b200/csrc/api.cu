@@ -454,6 +454,21 @@ int snap_project(const snap_problem* p, int batch, const double* u_hat, const do
   return project_impl(p, batch, u_hat, cdata, u_star, lambda, iters, warm, workspace, workspace_bytes, stream, nullptr);
 }
 
+int snap_project_f32(const snap_problem* cp, int batch, const float* u_hat, const float* cdata, float* u_star, int* iters,
+                     float tol, void* workspace, size_t workspace_bytes, snap_stream stream) {
+  snap_problem* p = const_cast<snap_problem*>(cp);
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u_hat || !cdata || !u_star || !iters || !workspace || !(tol > 0.0f)) return SNAP_EINVAL;
+  const DevParams& d = p->dp;
+  if (d.kind != SNAP_BURGERS1D_LF && d.kind != SNAP_BURGERS1D_LF_MASS) return SNAP_EINVAL;
+  if (!(d.nx == 32 || d.nx == 64 || d.nx == 128 || d.nx == 256)) return SNAP_EINVAL;
+  if (workspace_bytes < snap_workspace_bytes(p, batch)) return SNAP_ENOMEM;
+  unsigned char* w = ws_base(workspace) + stats_bytes((size_t)batch);
+  if (!(aligned16(u_hat) && aligned16(cdata) && aligned16(u_star) && aligned16(w))) return SNAP_EINVAL;
+  return launch_project1d_f32(p, batch, u_hat, cdata, u_star, iters, tol, w, static_cast<cudaStream_t>(stream));
+}
+
 int snap_flow_step(const snap_problem* p, int batch, double* u_tau, const double* vel, const double* u_prior, double tau,
                    double tau_next, const double* cdata, double* u1, double* u_next, double* lambda, int* iters,
                    void* workspace, size_t workspace_bytes, snap_stream stream) {

@@ -1,0 +1,197 @@
+// Float32 / tolerance 1e-5 mode ("single-precision floating-point values (Float32) ... convergence tolerance
+// fixed to 1e-5") for the Burgers family (kinds 1, 4), multiplier-free (PCFM's pull-back uses u_1 only,
+// Eq. 3).  Same method as kernels_1d_fused.cuh -- forward passes that carry JT Gauss-Newton iterations per level,
+//     q_0 = h_0 ,  q_k = h_k + A_{k-1} q_{k-1} ,  x+ = x - q     (J_loc square: the step is Newton on h) --
+// in fp32: one warp per sample, lane l owns the Q contiguous cells l Q .., rows move as plain coalesced 128-bit loads with the
+// next level prefetched in registers (a 256-cell row is 1 KB: no shared-memory staging is needed), neighbours by shuffles.
+// A pass runs JT - 1 updates and evaluates ||h||_inf at every iterate it visits (local rows and, kind 4, the mass rows);
+// the sample is done when an iterate met tol and at least `polish` more steps followed it.  Full steps only (the merit
+// test is dormant on these row sets, R17): a step after which ||h||_inf grows ends the sample with status -2.
+#pragma once
+#include "device_utils.cuh"
+#include "snap_internal.h"
+
+namespace snap {
+
+struct ProjF32Args {
+  DevParams P;
+  int batch;
+  const float* u_hat;
+  const float* cdata;
+  float* u_star;
+  int* iters;
+  float* bufA;   // [batch][n]
+  float* bufB;
+  float tol;
+};
+
+template <int Q>
+__device__ __forceinline__ void ldrow_f32(const float* __restrict__ g, float (&x)[Q]) {
+  if constexpr (Q >= 4) {
+#pragma unroll
+    for (int c = 0; c < Q / 4; ++c) {
+      const float4 t = reinterpret_cast<const float4*>(g)[c];
+      x[4 * c] = t.x; x[4 * c + 1] = t.y; x[4 * c + 2] = t.z; x[4 * c + 3] = t.w;
+    }
+  } else {
+#pragma unroll
+    for (int c = 0; c < Q; ++c) x[c] = g[c];
+  }
+}
+template <int Q>
+__device__ __forceinline__ void strow_f32(float* __restrict__ g, const float (&x)[Q]) {
+  if constexpr (Q >= 4) {
+#pragma unroll
+    for (int c = 0; c < Q / 4; ++c) reinterpret_cast<float4*>(g)[c] = make_float4(x[4 * c], x[4 * c + 1], x[4 * c + 2], x[4 * c + 3]);
+  } else {
+#pragma unroll
+    for (int c = 0; c < Q; ++c) g[c] = x[c];
+  }
+}
+__device__ __forceinline__ float wmaxf(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(SNAP_FULL, v, o));
+  return v;
+}
+__device__ __forceinline__ float wsumf(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(SNAP_FULL, v, o);
+  return v;
+}
+
+// One forward pass: T = NU + 1 iterations per level (NU updates, then the evaluation of the last iterate); reads x, writes
+// the iterate x_NU to `xo` (NU > 0).  hmax[t] = ||h(x_t)||_inf, t = 0..NU (warp-uniform on return).
+template <int Q, int JT>
+__device__ __forceinline__ void f32_pass(const DevParams& P, int lane, const float* __restrict__ x, const float* __restrict__ u0,
+                                         float* __restrict__ xo, int NU, float M0, float (&hmax)[JT]) {
+  constexpr int nx = 32 * Q;
+  const int nt = P.nt, first = lane * Q;
+  const float a0 = (float)P.bs_a0, e = (float)P.bs_e, qs = (float)P.bs_qs, hs = (float)P.bs_hs, dxm = (float)P.dx;
+  const bool has_mass = P.has_mass != 0;
+  float phi[JT][Q], cc[JT][Q];
+  {
+    float u0r[Q];
+    ldrow_f32<Q>(u0 + first, u0r);
+#pragma unroll
+    for (int t = 0; t < JT; ++t) {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) { phi[t][c] = u0r[c]; cc[t][c] = 0.f; }
+      hmax[t] = 0.f;
+    }
+  }
+  float vn[Q];
+  ldrow_f32<Q>(x + first, vn);
+  for (int k = 0; k < nt; ++k) {
+    float v[Q];
+#pragma unroll
+    for (int c = 0; c < Q; ++c) v[c] = vn[c];
+    if (k + 1 < nt) ldrow_f32<Q>(x + (size_t)(k + 1) * nx + first, vn);    // next level travels during this one
+    float msum[JT];
+#pragma unroll
+    for (int t = 0; t < JT; ++t) msum[t] = 0.f;
+#pragma unroll
+    for (int t = 0; t < JT; ++t) {
+      if (t <= NU) {
+        float q[Q], hm = 0.f, ms = 0.f;
+#pragma unroll
+        for (int c = 0; c < Q; ++c) {
+          const float h = v[c] - phi[t][c];
+          q[c] = h + cc[t][c];
+          hm = fmaxf(hm, fabsf(h));
+          ms += v[c];
+        }
+        msum[t] = ms;                        // mass row of this level and iterate: reduced after the iterations
+        hmax[t] = fmaxf(hmax[t], hm);
+        const float vL = __shfl_sync(SNAP_FULL, v[Q - 1], (lane + 31) & 31), vR = __shfl_sync(SNAP_FULL, v[0], (lane + 1) & 31);
+        const float qL = __shfl_sync(SNAP_FULL, q[Q - 1], (lane + 31) & 31), qR = __shfl_sync(SNAP_FULL, q[0], (lane + 1) & 31);
+        float um = vL, ql = qL;
+#pragma unroll
+        for (int c = 0; c < Q; ++c) {
+          const float up = (c < Q - 1) ? v[c + 1] : vR, qr = (c < Q - 1) ? q[c + 1] : qR;
+          const float vc = v[c], qc = q[c];
+          phi[t][c] = fmaf(a0, vc, (up + um) * fmaf(-qs, up - um, e));
+          cc[t][c] = fmaf(fmaf(-hs, up, e), qr, fmaf(fmaf(hs, um, e), ql, a0 * qc));
+          um = vc; ql = qc;
+          if (t < NU) v[c] = vc - qc;
+        }
+      }
+    }
+    if (NU > 0) strow_f32<Q>(xo + (size_t)k * nx + first, v);
+    if (has_mass) {     // JT interleaved butterflies, off the critical path of the level recurrence
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int t = 0; t < JT; ++t) msum[t] += __shfl_xor_sync(SNAP_FULL, msum[t], o);
+      }
+#pragma unroll
+      for (int t = 0; t < JT; ++t)
+        if (t <= NU) hmax[t] = fmaxf(hmax[t], fabsf(fmaf(dxm, msum[t], -M0)));
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < JT; ++t) hmax[t] = wmaxf(hmax[t]);
+}
+
+template <int Q, int JT>
+__global__ void __launch_bounds__(256) project1d_f32_kernel(const __grid_constant__ ProjF32Args A) {
+  const DevParams& P = A.P;
+  const int lane = threadIdx.x & 31;
+  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (b >= A.batch) return;
+  constexpr int nx = 32 * Q;
+  const size_t n = (size_t)P.n;
+  const float* uh = A.u_hat + (size_t)b * n;
+  const float* u0 = A.cdata + (size_t)b * nx;
+  float* ustar = A.u_star + (size_t)b * n;
+  float* bufA = A.bufA + (size_t)b * n;
+  float* bufB = A.bufB + (size_t)b * n;
+  float M0 = 0.f;
+  if (P.has_mass) {
+    float s = 0.f;
+    for (int i = lane; i < nx; i += 32) s += u0[i];
+    M0 = (float)P.dx * wsumf(s);
+  }
+  const float tol = A.tol;
+  const float* cur = uh;
+  int steps = 0, lin = 0, status = 0, since = -1;     // since: steps taken after the first iterate that met tol (-1: none yet)
+  float hprev = 3.4e38f;
+  bool done = false, first_pass = true;
+  while (!done) {
+    float* xo = (cur == bufA) ? bufB : bufA;
+    int NU = JT - 1;
+    if (since >= 0 && P.polish - since < NU) NU = P.polish - since;   // only the remaining polish steps
+    if (NU > P.max_iter - steps && since < 0) NU = P.max_iter - steps;
+    if (NU < 0) NU = 0;
+    float hmax[JT];
+    f32_pass<Q, JT>(P, lane, cur, u0, xo, NU, M0, hmax);
+    __syncwarp();
+    // walk the iterates x_0 .. x_NU of this pass (x_0 of a later pass was judged as the last iterate of the previous one)
+    if (!first_pass && NU > 0) { ++steps; if (since >= 0) ++since; }   // the step x_0 -> x_1 of a later pass
+    for (int t = first_pass ? 0 : 1; t <= NU; ++t) {
+      const float hv = hmax[t];
+      ++lin;
+      if (!(hv <= 3.4e38f)) { status = SNAP_ST_NONFINITE; done = true; break; }
+      if (since < 0) {
+        if (hv < tol) since = 0;
+        else if (hv > hprev && t > 0) { status = SNAP_ST_LINESEARCH; done = true; break; }   // a full step that does not descend
+      }
+      hprev = hv;
+      if (t < NU) { ++steps; if (since >= 0) ++since; }
+    }
+    first_pass = false;
+    if (done) break;
+    if (NU > 0) cur = xo;
+    if (since >= P.polish) done = true;                       // converged and polished: cur is final
+    else if (since < 0 && steps >= P.max_iter) { status = SNAP_ST_MAXITER; done = true; }
+  }
+  // u* <- final iterate (u_hat on a non-finite sample, R16)
+  const float* fin = (status == SNAP_ST_NONFINITE) ? uh : cur;
+  if (fin != ustar) {
+    const float4* s4 = reinterpret_cast<const float4*>(fin);
+    float4* d4 = reinterpret_cast<float4*>(ustar);
+    for (size_t i = lane; i < n / 4; i += 32) d4[i] = s4[i];
+  }
+  if (lane == 0) A.iters[b] = (status == 0) ? lin : status;
+}
+
+}  // namespace snap

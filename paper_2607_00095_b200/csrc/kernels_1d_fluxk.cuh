@@ -330,7 +330,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   const bool energy = P.fk_energy != 0;
   const bool same = (x.p == uh.p);
   const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
-  const double dx = P.dx, dtnu = P.fk_dtnu;
+  const double dx = P.dx;
   const double tol = P.tol, skip = kPolishSkip * P.tol;
 
   double phiA[Q], ccA[Q], phiB[Q], ccB[Q];
@@ -339,9 +339,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   double h1 = 0.0, f2 = 0.0, wq = 0.0, qq = 0.0, wzw = 0.0;   // per-lane partial sums (wzw: w^T W^-1 w over the free levels)
   double ds2 = 0.0;
   int hmx = 0;
-  // carried from the previous level (warp-uniform): energy, dissipation, and the dot products of its b vector
   double E_K = 0.0, D_K = 0.0, bq_K = 0.0;   // level K (warp-uniform): energy, dissipation, b_K . q'_K
-  constexpr bool hess = HESS;
 
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, k, x.tm, tm_uh);

@@ -72,6 +72,9 @@ int launch_residual_fluxk(const DevParams& P, int batch, const double* u, const 
 int launch_project2d(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                      double* lambda, int* iters, int warm, void* workspace, long long* stats, cudaStream_t st);
 
+// proj1d_f32.cu: Float32 mode of the Burgers kinds (multiplier-free)
+int launch_project1d_f32(snap_problem* p, int batch, const float* u_hat, const float* cdata, float* u_star, int* iters,
+                         float tol, void* workspace, cudaStream_t st);
 // proj2d_direct.cu: product-form path of kind 3; returns +1 when the shape / parameters / alignment are outside it
 int launch_project2d_direct(snap_problem* p, int batch, const double* u_hat, const double* cdata, double* u_star,
                             double* lambda, int* iters, void* workspace, long long* stats, const FlowArgs* flow,

@@ -540,6 +540,60 @@ def test_ns_vorticity_enstrophy_matches_oracle(S):
     np.testing.assert_array_equal(gb["u"][1], ref["u"][1])
 
 
+# ------------------------------------------------------------------------------------------------
+# Float32 / tolerance 1e-5 mode: snap_project_f32 against the fp64 oracle
+# ------------------------------------------------------------------------------------------------
+def test_float32_mode_matches_the_oracle_to_single_precision(S):
+    dev = torch.device("cuda:0")
+    for cfg, kw in ((2, dict(batch=3, nx=128, nt=40)), (5, dict(batch=3, nx=64, nt=33)), (5, dict(batch=2, nx=256, nt=64)),
+                    (2, dict(batch=2, nx=32, nt=9)), (5, dict(batch=9, nx=32, nt=20))):
+        wl = W.make_workload(cfg, **kw)
+        p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+        B = wl.batch
+        uh = wl.u_hat.to(dev, torch.float32).contiguous()
+        cd = wl.cdata.to(dev, torch.float32).contiguous()
+        us = torch.full_like(uh, float("nan"))
+        it = torch.full((B,), -99, dtype=torch.int32, device=dev)
+        l0 = p.launch_count()
+        S.snap_project_f32(p, B, uh, cd, us, it, tol=1e-5)
+        torch.cuda.synchronize()
+        assert p.launch_count() - l0 == 1
+        assert (it.cpu().numpy() > 0).all(), it
+        # feasibility of the fp32 result, evaluated in fp64 against the fp32 data it was computed from
+        nrm = torch.empty(B, 5, dtype=torch.float64, device=dev)
+        S.snap_residual(p, B, us.double(), cd.double(), None, nrm)
+        torch.cuda.synchronize()
+        assert float(nrm[:, 0].max()) < 2e-5, float(nrm[:, 0].max())         # tol 1e-5 + fp32 rounding of the rows
+        for b in range(B):
+            o = O.project(wl.kind, uh[b].double().cpu().numpy().reshape(wl.nt, 1, wl.nx), cd[b].double().cpu().numpy().reshape(1, wl.nx),
+                          dict(wl.params, tol=1e-5))
+            assert o["status"] == 0
+            err = np.abs(us[b].double().cpu().numpy().reshape(o["u"].shape) - o["u"]).max() / np.abs(o["u"]).max()
+            assert err <= 2e-4, (cfg, kw, b, err)       # ||J^-1|| (85 .. 177) x fp32 residual floor
+        # in place, and a non-finite sample keeps u* = u_hat
+        inp = uh.clone()
+        S.snap_project_f32(p, B, inp, cd, inp, it, tol=1e-5)
+        torch.cuda.synchronize()
+        assert torch.equal(inp, us)
+        bad = uh.clone(); bad[0] = float("inf")
+        out = torch.empty_like(bad)
+        S.snap_project_f32(p, B, bad, cd, out, it, tol=1e-5)
+        torch.cuda.synchronize()
+        assert int(it[0]) == -3 and (it[1:] > 0).all()
+        assert torch.equal(out[0], bad[0]) and torch.equal(out[1:], us[1:])
+        p.destroy()
+
+
+def test_float32_mode_rejects_other_kinds(S):
+    dev = torch.device("cuda:0")
+    wl = W.make_workload(3, batch=2, nx=64, nt=8)
+    p = S.snap_problem_create(wl.kind, wl.nx, wl.ny, wl.nt, wl.params)
+    uh = wl.u_hat.to(dev, torch.float32)
+    with pytest.raises(S.SnapError):
+        S.snap_project_f32(p, 2, uh, wl.cdata.to(dev, torch.float32), torch.empty_like(uh), torch.zeros(2, dtype=torch.int32, device=dev))
+    p.destroy()
+
+
 def test_direct2d_matches_oracle_and_pcg_path(S):
     """Kind 3, product-form path (in-SMEM red-black level solves): same limit point as the oracle
     and as the PCG kernel (gn_fuse = -1) on 2-row and 4-row patches, one and several warps, nt = 2."""

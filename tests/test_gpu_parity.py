@@ -609,6 +609,18 @@ def test_direct2d_matches_oracle_and_pcg_path(S):
         check_against_oracle(wl, wl.u_hat, d, range(wl.batch))
 
 
+def test_2d_shapes_with_more_than_four_rows_per_thread_of_the_pcg_kernel(S):
+    """96 x 42 and 24 x 170 give the PCG kernel's threads a fifth row, which its register arrays do not
+    hold.  The product-form kernel serves them (2-row patches); the PCG kernel refuses them instead of projecting wrongly."""
+    for kw in (dict(batch=1, nx=96, ny=42, nt=3), dict(batch=1, nx=24, ny=170, nt=3)):
+        wl = W.make_workload(4, **kw)
+        d = gpu_project(S, wl, wl.u_hat)
+        assert (d["iters"] > 0).all() and d["norms"][:, 0].max() < 1e-10
+        check_against_oracle(wl, wl.u_hat, d, range(wl.batch))
+        with pytest.raises(S.SnapError):
+            gpu_project(S, wl, wl.u_hat, params=dict(gn_fuse=-1))
+
+
 def test_direct2d_status_codes_and_line_search(S):
     wl = W.make_workload(4, batch=2, nx=16, ny=16, nt=5)
     big = gpu_project(S, wl, wl.u_hat * 1e160)

@@ -92,9 +92,9 @@ bool plan_fused(const snap_problem* p, int batch, Plan1d& pl) {
     for (int nst = 4; nst >= 2; --nst) {   // deeper rings measured no faster
       // ring + output staging rows (W > 1) + exchange slots + reduction scratch + mass-row level sums (W = 1,
       // JT x 8 levels x 34) + suffix sums of the min-norm correction (W = 1) + mbarriers
-      const size_t sb = align_up(((size_t)(2 * nst + (W > 1 ? 4 : 0)) * pl.rp + 2 * W * 8 + W * 24 +
-                                  (W == 1 ? JT * 8 * 34 : 0) +
-                                  (W == 1 ? (p->dp.nt < 512 ? p->dp.nt : 512) : 0) + nst) * 8, 1024);
+      const size_t sb = align_up(((size_t)(2 * nst + (W > 1 ? 4 : 0)) * pl.rp + fused_xch_doubles(W, JT) + W * 24 +
+                                  W * JT * 8 * 34 + (W > 1 ? 2 * W * JT * 8 : 0) +
+                                  (W == 1 ? (p->dp.nt < 512 ? p->dp.nt : 512) : 0) + nst + 1) * 8, 1024);
       if (sb * spc + 1024 <= limit) {
         pl.wpc = spc; pl.nst = nst; pl.warp_bytes = (int)sb; pl.smem = sb * spc + 1024;
         pl.grid = (batch + spc - 1) / spc;

@@ -14,8 +14,8 @@
 // pass is discarded and the sample continues with one iteration per pass (classic back-tracking).
 //
 // Layout: warp w of the group, lane l owns the Q contiguous cells (32 w + l) Q ... + Q - 1; neighbours are
-// register-local except at the two ends of a lane (one shuffle each) and of a warp (a shared-memory slot and
-// one named barrier per iteration; W = 1 needs neither).  A row travels HBM <-> shared memory as ONE tiled TMA
+// register-local except at the two ends of a lane (one shuffle each) and of a warp (a shared-memory slot and one
+// mbarrier exchange per level, fused_fwd_mw_body; W = 1 needs neither).  A row travels HBM <-> shared memory as ONE tiled TMA
 // copy (tensor map [sample][line of 16 doubles][16], box = one row, issued by one elected lane) with the
 // 128-byte swizzle, so that the lanes' 128-bit shared-memory accesses to their contiguous cells are
 // bank-conflict free: the 16-byte chunk c of line r sits at chunk position c ^ (r & 7).
@@ -188,7 +188,9 @@ struct RowPipe {
   double* red;     // [W][kRed] partial sums of a pass
   double* msb;     // W = 1: [JT][8 levels][kMsbPitch] per-lane cell sums of the iterates (mass rows, reduced every 8 levels)
   double* aux;     // W = 1: min(nt, 512) doubles (suffix sums of the min-norm correction)
+  double* mxs;     // W > 1: [2][W][JT][8] level sums of the iterates per warp (mass rows)
   uint32_t bar0, phase;
+  uint32_t xbar, xphase;   // W > 1: the group's exchange mbarrier (one arrive per warp and level) and its parity
   int nst, lane, w, bar_id, first, b;   // first = first cell owned by this lane, b = sample index (TMA coordinate)
   LaneOff<Q> lo;
   long long rows_rd, rows_wr;        // HBM rows requested (counted once per group): the traffic this variant needs
@@ -273,21 +275,18 @@ template <int W, int Q, int JT, int NU, bool EMIT>
 __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
                                        const double* __restrict__ u0, const Buf xout, const Buf yout, const double M0,
                                        FusedStats<JT>& S) {
+  static_assert(W == 1, "one warp per sample (groups of W > 1 warps run fused_fwd_mw_body)");
   using G = RowGeom<W, Q>;
   constexpr int nx = G::NX;
   constexpr int T = NU + (EMIT ? 1 : 0);
   static_assert(T >= 1 && T <= JT, "iterations per pass");
   constexpr bool kFirstPass = (NU == JT && !EMIT);   // this shape is only planned as the first pass: x_0 == u_hat
   RowPipe<W, Q> pp = pp_ref;   // registers; the mutable fields are written back at the end
-  const int nt = P.nt, lane = pp.lane, nst = pp.nst, w = pp.w, first = pp.first;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, first = pp.first;
   const double a0 = P.bs_a0, e = P.bs_e, qs = P.bs_qs, hs = P.bs_hs;
   const bool same = (x0.p == uh.p);
   const bool has_mass = P.has_mass != 0;
-  const int wl = (w + W - 1) % W, wr = (w + 1) % W;
-  // cells just outside this warp's range (periodic), read by lane 0 / lane 31 for iteration 0
-  const int cellL = swz_idx((first + nx - 1) % nx), cellR = swz_idx((first + Q) % nx);
-  bool shoot = false;
-  if constexpr (W == 1) shoot = (pp.vel_tm != nullptr);   // x0 holds u_tau: this pass forms u_hat (Eq. 1) in place
+  const bool shoot = (pp.vel_tm != nullptr);   // x0 holds u_tau: this pass forms u_hat (Eq. 1) in place
   const CUtensorMap* const tm_uh = shoot ? pp.vel_tm : (same ? nullptr : uh.tm);
 
   double phi[T][Q], cc[T][Q];              // Phi(x_t[k-1]) and (A_{k-1} q_{k-1}) of iteration t, own cells
@@ -336,34 +335,24 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     __syncwarp();
   };
 
-  int s = 0, par = 0;
+  int s = 0;
   for (int k = 0; k < nt; ++k) {
     pp.wait(s);
     double v[Q];
     const double* r0 = pp.row(s, 0);
     const double* ruh = same ? r0 : pp.row(s, 1);   // u_hat cells are re-read where needed
     load_cells<Q>(r0, pp.lo, v);
-    if constexpr (W == 1) {
-      if (shoot) {   // u_hat = u_tau + (1 - tau) v_theta: to global (in place over u_tau) and back into the stage row,
-                     // which later iterations of this level re-read as the u_hat row
-        double vv[Q];
-        load_cells<Q>(pp.row(s, 1), pp.lo, vv);
+    if (shoot) {   // u_hat = u_tau + (1 - tau) v_theta: to global (in place over u_tau) and back into the stage row,
+                   // which later iterations of this level re-read as the u_hat row
+      double vv[Q];
+      load_cells<Q>(pp.row(s, 1), pp.lo, vv);
 #pragma unroll
-        for (int c = 0; c < Q; ++c) v[c] = fma(pp.omt, vv[c], v[c]);
-        store_cells<Q>(pp.row(s, 0), pp.lo, v);
-        store_cells_global<Q>(uh.p + (size_t)k * nx + first, v);
-        if (lane == 0) pp.rows_wr += 1;
-      }
+      for (int c = 0; c < Q; ++c) v[c] = fma(pp.omt, vv[c], v[c]);
+      store_cells<Q>(pp.row(s, 0), pp.lo, v);
+      store_cells_global<Q>(uh.p + (size_t)k * nx + first, v);
+      if (lane == 0) pp.rows_wr += 1;
     }
     double vL = shfl_prev(v[Q - 1], lane), vR = shfl_next(v[0], lane);
-    if constexpr (W > 1) {
-      if (lane == 0) vL = r0[cellL];
-      if (lane == 31) vR = r0[cellR];
-    }
-    constexpr bool kDirect = (W == 1);   // W == 1: results go straight to global memory (no staging, no proxy fence)
-    if constexpr (!kDirect) pp.out_ready();
-    double* so_u = pp.out(k & 1);
-    double* so_y = pp.out(2 + (k & 1));
 #pragma unroll
     for (int t = 0; t < T; ++t) {
       double q[Q], uhr[Q];
@@ -385,31 +374,10 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
       }
       // end values of the next iterate (only the two ends are exchanged; the rest is updated in place below)
       const double vn0 = (t < NU) ? v[0] - q[0] : v[0], vnE = (t < NU) ? v[Q - 1] - q[Q - 1] : v[Q - 1];
-      double qL = shfl_prev(q[Q - 1], lane), qR = shfl_next(q[0], lane);
+      const double qL = shfl_prev(q[Q - 1], lane), qR = shfl_next(q[0], lane);
       double vnL = 0.0, vnR = 0.0;
       if (t + 1 < T) { vnL = shfl_prev(vnE, lane); vnR = shfl_next(vn0, lane); }
-      double mtot = 0.0;
-      if constexpr (W > 1) {
-        const double ps = has_mass ? warp_sum(msum) : 0.0;
-        double* xs = pp.xch + (size_t)par * (W * 8);
-        if (lane == 0) { xs[w * 8 + 0] = q[0]; xs[w * 8 + 2] = vn0; xs[w * 8 + 4] = ps; }
-        if (lane == 31) { xs[w * 8 + 1] = q[Q - 1]; xs[w * 8 + 3] = vnE; }
-        pp.gsync();
-        if (lane == 0) { qL = xs[wl * 8 + 1]; vnL = xs[wl * 8 + 3]; }
-        if (lane == 31) { qR = xs[wr * 8 + 0]; vnR = xs[wr * 8 + 2]; }
-        if (has_mass) {
-#pragma unroll
-          for (int i = 0; i < W; ++i) mtot += xs[i * 8 + 4];
-        }
-        par ^= 1;
-        if (has_mass && w == 0 && lane == 0) {
-          const double hm = fabs(fma(dxm, mtot, -M0));
-          hmx[t] = max(hmx[t], __double2hiint(hm));
-          h1[t] += hm;
-        }
-      } else {
-        if (has_mass) sts_f64(msb_a + 8u * (uint32_t)((t * 8 + (k & 7)) * kMsbPitch + lane), msum);
-      }
+      if (has_mass) sts_f64(msb_a + 8u * (uint32_t)((t * 8 + (k & 7)) * kMsbPitch + lane), msum);
       // state for the next level (needs the old v and q with neighbours), then the update in place
       double um = vL, ql = qL;
 #pragma unroll
@@ -424,21 +392,13 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
         else if (EMIT) q[c] = qc - (vc - uhr[c]);   // y
       }
       if (t < NU) { vL = vnL; vR = vnR; }
-      else if constexpr (kDirect) { if (yout.p) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q); }
-      else store_cells<Q>(so_y, pp.lo, q);
+      else if (yout.p) store_cells_global<Q>(yout.p + (size_t)k * nx + first, q);
     }
-    if constexpr (W == 1) {
-      if (has_mass && ((k & 7) == 7 || k == nt - 1)) mass_rows8((k & 7) + 1);
-    }
-    if constexpr (kDirect) {
-      if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
-      if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + ((EMIT && yout.p) ? 1 : 0);
-    } else {
-      if (NU > 0) store_cells<Q>(so_u, pp.lo, v);
-      pp.store_rows(k, NU > 0 ? xout.tm : nullptr, so_u, (EMIT && yout.p) ? yout.tm : nullptr, so_y);
-    }
-    // stage s is free: every warp loaded its cells before the first exchange barrier of this level
-    if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
+    if (has_mass && ((k & 7) == 7 || k == nt - 1)) mass_rows8((k & 7) + 1);
+    // results go straight to global memory (no staging row, no proxy fence)
+    if (NU > 0) store_cells_global<Q>(xout.p + (size_t)k * nx + first, v);
+    if (lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + ((EMIT && yout.p) ? 1 : 0);
+    if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);   // the warp has read stage s
     if (++s == nst) s = 0;
   }
   pp.drain();
@@ -452,24 +412,6 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     part[4 * t + 3] = warp_sum(dd[t]);
   }
   part[4 * T] = warp_sum(f2);
-  if constexpr (W > 1) {
-    if (lane == 0) {
-#pragma unroll
-      for (int i = 0; i < 4 * T + 1; ++i) pp.red[w * kRed + i] = part[i];
-    }
-    pp.gsync();
-#pragma unroll
-    for (int i = 0; i < 4 * T + 1; ++i) {
-      double acc = pp.red[i];
-#pragma unroll
-      for (int ww = 1; ww < W; ++ww) {
-        const double o = pp.red[ww * kRed + i];
-        acc = ((i & 3) == 0 && i < 4 * T) ? fmax(acc, o) : acc + o;
-      }
-      part[i] = acc;
-    }
-    pp.gsync();
-  }
   S.f0 = 0.5 * part[4 * T];
 #pragma unroll
   for (int t = 0; t < T; ++t) {
@@ -480,6 +422,232 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
     S.bad[t] = !(finite_d(a) && finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(part[4 * T]));
   }
   pp_ref.phase = pp.phase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
+}
+
+// ------------------------------------------------------------------------------------------------
+// W > 1: the same fused pass with ONE exchange per level between the warps of a group.  The in-level chain
+// x_t -> h -> q_t -> x_{t+1} is cell-local (it needs Phi and A q of the PREVIOUS level only), so a warp first runs all
+// T iterations of the level on its own cells, publishes the end values (x_t, q_t of its first and last cell, every t)
+// to a shared-memory slot, arrives on the group's mbarrier, does the work that needs no neighbour (sums, row stores,
+// intra-warp shuffles), and only then waits for the other warps' slots and forms Phi / A q for the next level.
+// The warps of a group therefore run at most one level apart and never wait inside an iteration (the per-iteration
+// named barrier of the first W > 1 mapping cost 2.4x, profiles/r02_project1d_fused.md).  Rows leave through direct
+// 128-bit global stores as for W = 1.
+// ------------------------------------------------------------------------------------------------
+template <int W, int Q, int JT, int NU, bool EMIT>
+__device__ __forceinline__ void fused_fwd_mw_body(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
+                                                  const double* __restrict__ u0, const Buf xout, const Buf yout,
+                                                  const double M0, FusedStats<JT>& S) {
+  static_assert(W > 1, "multi-warp groups only");
+  using G = RowGeom<W, Q>;
+  constexpr int nx = G::NX;
+  constexpr int T = NU + (EMIT ? 1 : 0);
+  static_assert(T >= 1 && T <= JT, "iterations per pass");
+  constexpr bool kFirstPass = (NU == JT && !EMIT);   // only planned as the first pass: x_0 == u_hat
+  RowPipe<W, Q> pp = pp_ref;
+  const int nt = P.nt, lane = pp.lane, nst = pp.nst, w = pp.w, first = pp.first;
+  const double a0 = P.bs_a0, e = P.bs_e, qs = P.bs_qs, hs = P.bs_hs;
+  const bool same = (x0.p == uh.p);
+  const bool has_mass = P.has_mass != 0;
+  const int wl = (w + W - 1) % W, wr = (w + 1) % W;
+  const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
+
+  double phi[T][Q], cc[T][Q];
+  double h1[T], wd[T], dd[T];
+  int hmx[T];
+  const double tol = P.tol, skip = kPolishSkip * P.tol;
+  double f2 = 0.0;
+  {
+    double u0r[Q];
+#pragma unroll
+    for (int c = 0; c < Q; ++c) u0r[c] = u0[first + c];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) { phi[t][c] = u0r[c]; cc[t][c] = 0.0; }
+      h1[t] = 0.0; wd[t] = 0.0; dd[t] = 0.0; hmx[t] = 0;
+    }
+  }
+  const int npro = nst < nt ? nst : nt;
+  for (int k = 0; k < npro; ++k) pp.issue(k, k, x0.tm, tm_uh);
+
+  const double dxm = P.dx;
+  const uint32_t msb_a = smem_u32(pp.msb) + 8u * (uint32_t)(w * JT * 8 * kMsbPitch);   // this warp's cell sums
+  const uint32_t mxs_a = smem_u32(pp.mxs);                                              // [2][W][JT][8] level sums per warp (buffer (k >> 3) & 1)
+  const uint32_t xch_a = smem_u32(pp.xch);                                              // [2][W][JT][4] end values
+  // the warp's part of the level sums of the last nv levels -> mxs (before this level's arrive)
+  auto mass_part8 = [&](int mb) {
+    __syncwarp();
+    const int j = lane & 7, pq = lane >> 3;
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      const uint32_t a = msb_a + 8u * (uint32_t)((t * 8 + j) * kMsbPitch + pq * 8);
+      const double2 y0 = lds_v2(a), y1 = lds_v2(a + 16u), y2 = lds_v2(a + 32u), y3 = lds_v2(a + 48u);
+      double sacc = ((y0.x + y0.y) + (y1.x + y1.y)) + ((y2.x + y2.y) + (y3.x + y3.y));
+      sacc += __shfl_xor_sync(SNAP_FULL, sacc, 8);
+      sacc += __shfl_xor_sync(SNAP_FULL, sacc, 16);
+      if (pq == 0) sts_f64(mxs_a + 8u * (uint32_t)(((mb * W + w) * JT + t) * 8 + j), sacc);
+    }
+  };
+  // after the wait: warp 0 joins the W parts (fixed order) and takes the mass rows into its sums
+  auto mass_join8 = [&](int mb, int nv) {
+    const int j = lane & 7, pq = lane >> 3;
+    if (w == 0) {
+#pragma unroll
+      for (int t = 0; t < T; ++t) {
+        double sacc = 0.0;
+#pragma unroll
+        for (int i = 0; i < W; ++i) sacc += lds_f64(mxs_a + 8u * (uint32_t)(((mb * W + i) * JT + t) * 8 + j));
+        const double hm = fabs(fma(dxm, sacc, -M0));
+        const bool on = (pq == 0) && (j < nv);
+        hmx[t] = max(hmx[t], on ? __double2hiint(hm) : 0);
+        h1[t] += on ? hm : 0.0;
+      }
+    }
+  };
+
+  int s = 0;
+  uint32_t xph = pp.xphase;
+  for (int k = 0; k < nt; ++k) {
+    pp.wait(s);
+    double vt[T][Q], qt[T][Q], uhr[Q], vfin[Q];
+    load_cells<Q>(pp.row(s, 0), pp.lo, vt[0]);
+    if (!same) load_cells<Q>(pp.row(s, 1), pp.lo, uhr);
+    else {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) uhr[c] = vt[0][c];
+    }
+    // ---- the cell-local chain of the level: all T iterations --------------------------------------------
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      if (has_mass) sts_f64(msb_a + 8u * (uint32_t)((t * 8 + (k & 7)) * kMsbPitch + lane), tree_sum<Q>(vt[t]));
+#pragma unroll
+      for (int c = 0; c < Q; ++c) {
+        const double v = vt[t][c];
+        const double h = v - phi[t][c];
+        const double q = h + cc[t][c];
+        const double ah = fabs(h);
+        hmx[t] = max(hmx[t], __double2hiint(ah));
+        h1[t] += ah;
+        dd[t] = fma(q, q, dd[t]);
+        if (!(kFirstPass && t == 0)) {
+          const double wv = v - uhr[c];
+          wd[t] = fma(wv, q, wd[t]);
+          if (t == 0) f2 = fma(wv, wv, f2);
+        }
+        qt[t][c] = q;
+        if (t < NU) {
+          const double vn = v - q;
+          if (t + 1 < T) vt[t + 1][c] = vn;
+          else vfin[c] = vn;
+        }
+      }
+    }
+    // ---- publish the end values, arrive -----------------------------------------------------------------
+    {
+      const uint32_t xs = xch_a + 8u * (uint32_t)(((k & 1) * W + w) * JT * 4);
+      if (lane == 0) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) { sts_f64(xs + 32u * t, vt[t][0]); sts_f64(xs + 32u * t + 16u, qt[t][0]); }
+      }
+      if (lane == 31) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) { sts_f64(xs + 32u * t + 8u, vt[t][Q - 1]); sts_f64(xs + 32u * t + 24u, qt[t][Q - 1]); }
+      }
+    }
+    const bool mass_now = has_mass && ((k & 7) == 7 || k == nt - 1);
+    if (mass_now) mass_part8((k >> 3) & 1);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(pp.xbar);
+    // ---- work that needs no other warp ------------------------------------------------------------------
+    double vL[T], vR[T], qL[T], qR[T];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      vL[t] = shfl_prev(vt[t][Q - 1], lane); vR[t] = shfl_next(vt[t][0], lane);
+      qL[t] = shfl_prev(qt[t][Q - 1], lane); qR[t] = shfl_next(qt[t][0], lane);
+    }
+    if (NU > 0) {
+      if constexpr (EMIT) store_cells_global<Q>(xout.p + (size_t)k * nx + first, vt[T - 1]);
+      else store_cells_global<Q>(xout.p + (size_t)k * nx + first, vfin);
+    }
+    if constexpr (EMIT) {
+      if (yout.p) {
+        double y[Q];
+#pragma unroll
+        for (int c = 0; c < Q; ++c) y[c] = qt[T - 1][c] - (vt[T - 1][c] - uhr[c]);
+        store_cells_global<Q>(yout.p + (size_t)k * nx + first, y);
+      }
+    }
+    if (w == 0 && lane == 0) pp.rows_wr += (NU > 0 ? 1 : 0) + ((EMIT && yout.p) ? 1 : 0);
+    // ---- the other warps' end values --------------------------------------------------------------------
+    mbar_wait(pp.xbar, xph);
+    xph ^= 1u;
+    {
+      const uint32_t xl = xch_a + 8u * (uint32_t)(((k & 1) * W + wl) * JT * 4);
+      const uint32_t xr = xch_a + 8u * (uint32_t)(((k & 1) * W + wr) * JT * 4);
+      if (lane == 0) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) { vL[t] = lds_f64(xl + 32u * t + 8u); qL[t] = lds_f64(xl + 32u * t + 24u); }
+      }
+      if (lane == 31) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) { vR[t] = lds_f64(xr + 32u * t); qR[t] = lds_f64(xr + 32u * t + 16u); }
+      }
+    }
+    if (mass_now) mass_join8((k >> 3) & 1, (k & 7) + 1);
+    // every warp of the group has read stage s (its reads precede its arrive): refill it
+    if (k + nst < nt) pp.issue(s, k + nst, x0.tm, tm_uh);
+    // ---- Phi and A q of this level, the state of the next one -------------------------------------------
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+#pragma unroll
+      for (int c = 0; c < Q; ++c) {
+        const double um = (c > 0) ? vt[t][c - 1] : vL[t], up = (c < Q - 1) ? vt[t][c + 1] : vR[t];
+        const double ql = (c > 0) ? qt[t][c - 1] : qL[t], qr = (c < Q - 1) ? qt[t][c + 1] : qR[t];
+        const double vc = vt[t][c], qc = qt[t][c];
+        phi[t][c] = fma(a0, vc, (up + um) * fma(-qs, up - um, e));
+        cc[t][c] = fma(fma(-hs, up, e), qr, fma(fma(hs, um, e), ql, a0 * qc));
+      }
+    }
+    if (++s == nst) s = 0;
+  }
+  pp.xphase = xph;
+  pp.drain();
+  // ---- reduce: lanes -> warp -> group (fixed order) ----------------------------------------------------------
+  double part[4 * T + 1];
+#pragma unroll
+  for (int t = 0; t < T; ++t) {
+    part[4 * t + 0] = hinf_level(hmx[t], tol, skip);
+    part[4 * t + 1] = warp_sum(h1[t]);
+    part[4 * t + 2] = warp_sum(wd[t]);
+    part[4 * t + 3] = warp_sum(dd[t]);
+  }
+  part[4 * T] = warp_sum(f2);
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < 4 * T + 1; ++i) pp.red[w * kRed + i] = part[i];
+  }
+  pp.gsync();
+#pragma unroll
+  for (int i = 0; i < 4 * T + 1; ++i) {
+    double acc = pp.red[i];
+#pragma unroll
+    for (int ww = 1; ww < W; ++ww) {
+      const double o = pp.red[ww * kRed + i];
+      acc = ((i & 3) == 0 && i < 4 * T) ? fmax(acc, o) : acc + o;
+    }
+    part[i] = acc;
+  }
+  pp.gsync();
+  S.f0 = 0.5 * part[4 * T];
+#pragma unroll
+  for (int t = 0; t < T; ++t) {
+    const double a = part[4 * t + 0], b = part[4 * t + 1];
+    const double c1 = -part[4 * t + 2], c2 = part[4 * t + 3];
+    S.hlev[t] = a; S.h1[t] = b; S.wd[t] = c1; S.dd[t] = c2;
+    S.bad[t] = !(finite_d(a) && finite_d(b) && finite_d(c1) && finite_d(c2) && finite_d(part[4 * T]));
+  }
+  pp_ref.phase = pp.phase; pp_ref.xphase = pp.xphase; pp_ref.rows_rd = pp.rows_rd; pp_ref.rows_wr = pp.rows_wr;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -660,7 +828,8 @@ template <int W, int Q, int JT, int NU, bool EMIT>
 __device__ __noinline__ void fused_fwd(const DevParams& P, RowPipe<W, Q>& pp_ref, const Buf x0, const Buf uh,
                                        const double* __restrict__ u0, const Buf xout, const Buf yout, const double M0,
                                        FusedStats<JT>& S) {
-  fused_fwd_body<W, Q, JT, NU, EMIT>(P, pp_ref, x0, uh, u0, xout, yout, M0, S);
+  if constexpr (W > 1) fused_fwd_mw_body<W, Q, JT, NU, EMIT>(P, pp_ref, x0, uh, u0, xout, yout, M0, S);
+  else fused_fwd_body<W, Q, JT, NU, EMIT>(P, pp_ref, x0, uh, u0, xout, yout, M0, S);
 }
 
 template <int KIND, int W, int Q, int JT, int NU, bool EMIT>
@@ -1018,11 +1187,13 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.stage = reinterpret_cast<double*>(base);
   pp.orow = pp.stage + (size_t)A.nst * 2 * G::RP;           // output staging rows: only W > 1 uses them
   pp.xch = pp.orow + (size_t)(W > 1 ? 4 : 0) * G::RP;
-  pp.red = pp.xch + G::XCH;
+  pp.red = pp.xch + fused_xch_doubles(W, JT);
   pp.msb = pp.red + W * kRed;
-  pp.aux = pp.msb + (W == 1 ? JT * 8 * kMsbPitch : 0);
-  pp.bar0 = smem_u32(pp.aux + (W == 1 ? (nt < 512 ? nt : 512) : 0));
-  pp.phase = 0;
+  pp.aux = pp.msb + W * JT * 8 * kMsbPitch;
+  pp.mxs = pp.aux + (W == 1 ? (nt < 512 ? nt : 512) : 0);
+  pp.bar0 = smem_u32(pp.mxs + (W > 1 ? 2 * W * JT * 8 : 0));
+  pp.xbar = pp.bar0 + 8u * A.nst;
+  pp.phase = 0; pp.xphase = 0;
   pp.nst = A.nst; pp.lane = lane; pp.w = w; pp.bar_id = 1 + slot;
   pp.first = (w * 32 + lane) * Q;
   pp.b = b;
@@ -1032,6 +1203,7 @@ __global__ void __launch_bounds__(MAXT) project1d_fused_kernel(const __grid_cons
   pp.uprior = nullptr; pp.unext = nullptr;    // armed below, around the pass that streams the final iterate
   if (gtid == 0) {
     for (int s = 0; s < A.nst; ++s) mbar_init(pp.bar0 + 8u * s, 1);
+    if (W > 1) mbar_init(pp.xbar, W);
     mbar_fence_init();
     fence_proxy_async_smem();
   }

@@ -7,6 +7,12 @@
 
 namespace snap {
 
+// doubles of the exchange slots of a fused group: [parity][warp][8] (sweeps) or [parity][warp][JT][4] (forward passes)
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr int fused_xch_doubles(int W, int JT) { return 2 * W * (4 * JT > 8 ? 4 * JT : 8); }
+
 // PCFM step arguments handed through the launch layers (null = plain projection)
 struct FlowArgs {
   const double* vel;

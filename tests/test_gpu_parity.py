@@ -703,12 +703,20 @@ def test_fused_pass_modes_agree_with_oracle(S, cfg, gn_fuse):
 
 
 def test_fused_path_wide_rows_two_warps_per_sample(S):
-    """nx = 512 runs the fused kernel with two warps per sample (end cells exchanged through shared memory)."""
-    for cfg in (2, 5):
-        wl = W.make_workload(cfg, batch=2, nx=512, nt=12)
+    """nx = 512 runs the fused kernel with two warps per sample: one shared-memory exchange of the end cells per level
+    (mbarrier), mass-row sums joined across the warps every 8 levels (nt = 17 / 41: groups of 8 levels with a ragged
+    tail, and a tail group right after a full one)."""
+    for cfg, nt in ((2, 12), (5, 12), (5, 17), (5, 41)):
+        wl = W.make_workload(cfg, batch=3, nx=512, nt=nt)
         g = gpu_project(S, wl, wl.u_hat)
         assert g["norms"][:, 0].max() < 1e-10
         check_against_oracle(wl, wl.u_hat, g, range(wl.batch))
+    # forced back-tracking: the one-update and evaluation-only pass shapes of the two-warp mapping
+    wl = W.make_workload(5, batch=2, nx=512, nt=17, noise=1.0)
+    ref = gpu_project(S, wl, wl.u_hat)
+    forced = gpu_project(S, wl, wl.u_hat, params=dict(ls_c1=0.9))
+    assert (forced["iters"] > ref["iters"]).all()
+    check_against_oracle(wl, wl.u_hat, forced, range(wl.batch), params=dict(ls_c1=0.9))
 
 
 def test_fused_path_line_search_and_status_codes(S):

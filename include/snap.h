@@ -79,7 +79,10 @@ enum {
 
 /* Per-sample status written to iters[b] when negative; iters[b] >= 0 = number of linear (Schur) solves. */
 enum {
-  SNAP_ST_MAXITER = -1,    /* max_iter Gauss-Newton steps without reaching tol; u* = last iterate            */
+  SNAP_ST_MAXITER = -1,    /* max_iter Gauss-Newton steps without reaching tol; u* = last iterate (kind
+                              ALLENCAHN2D_IE: the last iterate of the INEXACT Newton sequence -- steps taken while
+                              ||h||_inf >= tol are solved to the forcing tolerance of pcg_rtol below, so an
+                              unconverged u* differs from an exactly solved sequence by that tolerance)           */
   SNAP_ST_LINESEARCH = -2, /* Armijo back-tracking exhausted ls_max halvings; u* = last accepted iterate      */
   SNAP_ST_NONFINITE = -3,  /* non-finite residual or direction; u* = u_hat, lam = 0          */
   SNAP_ST_PCG = -4         /* 2D: PCG hit pcg_max without reaching pcg_rtol; u* = last iterate               */
@@ -124,7 +127,10 @@ typedef struct {
   int max_iter;       /* cap on Gauss-Newton steps                          (default 50)                      */
   int polish;         /* extra full steps once tol is met; skipped when
                          ||h||_inf <= 1e-3 * tol already                    (default 1)                       */
-  double ls_c1;       /* Armijo sufficient-decrease constant                (default 1e-4)                    */
+  double ls_c1;       /* Armijo sufficient-decrease constant                (default 1e-4).  Kind HEAT1D_IC_MASS
+                         has linear rows: the full Gauss-Newton step from u_hat IS the projection, the library
+                         takes it in closed form and ls_c1 / ls_shrink / ls_max / max_iter are not consulted
+                         (a merit test with ls_c1 >= 1/2 would reject that step: see DESIGN.md R25)               */
   double ls_shrink;   /* step-length reduction factor                       (default 0.5)                     */
   int ls_max;         /* maximum number of reductions per step              (default 20)                      */
   double pcg_rtol;    /* 2D: PCG stops at ||r - S lam||_2 <= pcg_rtol ||r||_2 (default 1e-13);

@@ -712,6 +712,7 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
     const double noise = 1.8e-15 * (S.qq + S.ww + 2.0 * fabs(lam_jw) + lam_rho);
     const bool conv = S.hlev < 2.0 && dd <= thr && noise <= thr;
     bool final_solve = false;
+    bool last_chance = false;   // step budget spent at a feasible point whose step norm the expanded form cannot certify
     if (polishing) {
       final_solve = (polish_left == 0);
     } else if (conv) {
@@ -719,8 +720,10 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
       polish_left = (S.hlev > 0.0) ? P.polish : 0;
       final_solve = (polish_left == 0);
     } else if (steps >= P.max_iter) {
-      status = SNAP_ST_MAXITER;
-      final_solve = true;
+      // the convergence test comes before the budget test (oracle/project.py): if ||h||_inf < tol the step is measured
+      // by applying it (below); a small one makes `cur` the converged point, otherwise the step is dropped
+      if (S.hlev < 2.0 && !(noise <= thr)) last_chance = true;
+      else { status = SNAP_ST_MAXITER; final_solve = true; }
     }
     if (final_solve) break;
     double phi_cur = 0.0, Dphi = 0.0;
@@ -757,6 +760,7 @@ __global__ void __launch_bounds__(256) project1d_fluxk_kernel(const __grid_const
       S = St;
       continue;
     }
+    if (last_chance) { status = SNAP_ST_MAXITER; break; }   // `cur` stays the returned iterate, lE / lM are its multipliers
     if (!polishing) ++steps;
     cur = xo;
     S = St;

@@ -936,6 +936,26 @@ def test_fluxk_result_depends_on_the_input_and_edge_cases(S):
     np.testing.assert_allclose(capped["u"][0], o["u"], rtol=0, atol=1e-12)
 
 
+def test_fluxk_max_iter_boundary(S):
+    """The convergence test precedes the step-budget test (oracle/project.py): a sample that converges with exactly
+    max_iter steps reports success, one step fewer reports SNAP_ST_MAXITER with the oracle's iterate (R25)."""
+    for cfg, kw in ((6, dict(batch=2, nx=32, nt=12)), (7, dict(batch=2, nx=32, nt=7, noise=0.01)), (8, dict(batch=2, nx=64, nt=12))):
+        wl = W.make_workload(cfg, **kw)
+        for b in range(wl.batch):
+            ref = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), wl.params)
+            assert ref["status"] == 0 and ref["steps"] >= 2
+            for cap in (ref["steps"], ref["steps"] - 1):
+                prm = dict(max_iter=cap)
+                o = O.project(wl.kind, wl.u_hat[b].numpy(), wl.cdata[b].numpy(), dict(wl.params, **prm))
+                g = gpu_project(S, wl, wl.u_hat[b:b + 1].clone(), params=prm, cdata=wl.cdata[b:b + 1])
+                assert o["status"] == (0 if cap == ref["steps"] else -1)
+                if o["status"] == 0:
+                    assert abs(int(g["iters"][0]) - int(o["iters"])) <= 1, (cfg, b, cap, g["iters"], o["iters"])
+                else:
+                    assert int(g["iters"][0]) == -1, (cfg, b, cap, g["iters"])
+                np.testing.assert_allclose(g["u"][0], o["u"], rtol=0, atol=1e-9 * np.abs(o["u"]).max())
+
+
 def test_fluxk_line_search_is_live_far_from_the_feasible_set(S):
     """noise 1.0: Gauss-Newton with W = I contracts slowly and the Armijo test rejects full steps (oracle pin
     test_gauss_newton_converges_linearly...); GPU and oracle take the same decisions and land on the same point."""

@@ -218,6 +218,7 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
   // PCFM step: x holds u_tau and the second row of a stage carries the velocity; the pass forms u_hat (Eq. 1) per level,
   // writes it to `uh_out` (in place over u_tau) and into both stage rows, so the rest of the level sees x = u_hat
   const double* __restrict__ second = vel ? vel : uh;
+  const bool all_active = __syncthreads_and(active ? 1 : 0) != 0;
   if (threadIdx.x == 0) ring.issue(0, x, second);
   for (int k = 0; k < nt; ++k) {
     const int s = k & 1;
@@ -227,6 +228,9 @@ __device__ void fwd_pass2d(const DevParams& P, const Geo2d& g, Ring2d& ring, dou
     if (vel) {
       double vv[PR][4];
       load_nat<PR>(ring.row(s, 1) + g.nat, g.nx, vv);
+      // the spare threads of the last warp shadow patch 0: they must have read its velocity cells before thread 0 (another
+      // warp) overwrites them with u_hat, or one of the two forms u_tau + omt u_hat (found at 96 x 42, 504 of 512 threads)
+      if (!all_active) __syncthreads();
 #pragma unroll
       for (int r = 0; r < PR; ++r)
 #pragma unroll

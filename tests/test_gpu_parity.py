@@ -383,6 +383,7 @@ def _flow_inputs(wl, tau):
 @pytest.mark.parametrize("cfg,kw,prm,fused", [
     (5, dict(batch=3, nx=64, nt=32), {}, True), (2, dict(batch=2, nx=128, nt=20), {}, True), (3, dict(batch=3, nx=64, nt=17), {}, True),
     (4, dict(batch=2, nx=16, ny=16, nt=5), {}, True), (4, dict(batch=2, nx=64, ny=64, nt=3), {}, True),
+    (4, dict(batch=3, nx=96, ny=42, nt=4), {}, True),    # 504 patches on 512 threads: the spare threads sit in another warp
     (5, dict(batch=2, nx=64, nt=12), dict(gn_fuse=-1), False), (2, dict(batch=2, nx=70, nt=12), {}, False),
     (4, dict(batch=2, nx=12, ny=10, nt=4), dict(gn_fuse=-1), False), (1, dict(batch=3, nx=20, nt=12), {}, False),
     (6, dict(batch=2, nx=64, nt=16), {}, False)])

@@ -74,7 +74,8 @@ enum {
   SNAP_OK = 0,
   SNAP_EINVAL = -1,  /* bad kind / size / NULL pointer / ny != 1 for a 1D kind / size above the limits below */
   SNAP_ECUDA = -2,   /* a CUDA call or launch failed (query cudaGetLastError)                                */
-  SNAP_ENOMEM = -3   /* workspace too small / staging allocation failed                                       */
+  SNAP_ENOMEM = -3,  /* workspace too small / staging allocation failed                                       */
+  SNAP_ELIMIT = -4   /* no-allocation entry point: batch*n exceeds the static scratch (SNAP_STATIC_SCRATCH_BYTES) */
 };
 
 /* Per-sample status written to iters[b] when negative; iters[b] >= 0 = number of linear (Schur) solves. */
@@ -242,6 +243,29 @@ int snap_residual(const snap_problem* p, int batch, const double* u, const doubl
  * validation against an assembled J J^T. */
 int snap_schur_apply(const snap_problem* p, int batch, const double* u, const double* x, double* out,
                      void* workspace, size_t workspace_bytes, snap_stream stream);
+
+/* No-allocation variant of snap_schur_apply, for callers that cannot allocate device memory or hand over a workspace
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The scratch vector
+ * g = J(u)^T x lives in a file-scope `static __device__` array of SNAP_STATIC_SCRATCH_BYTES (8 MiB = 2^20 doubles) inside
+ * the library; every GPU that loads libsnap holds those 8 MiB until the process exits.
+ *   u, x, out   dev, as snap_schur_apply (kinds 0-4); same kernels, same result bit for bit.
+ *   Limit       batch * n <= SNAP_STATIC_SCRATCH_BYTES / 8 = 1 048 576 (e.g. 64 samples of 128 x 128, 16 of 256 x 256);
+ *               beyond it the call returns SNAP_ELIMIT and launches nothing.
+ *   Allocation  the call performs no cudaMalloc / cudaFree and calls no allocating library routine; it enqueues two
+ *               kernels on `stream` and returns.  The device address of the array is resolved once per device
+ *               (cudaGetSymbolAddress, on the device current at that moment): by snap_static_scratch_init(), which a
+ *               caller runs once per device at set-up (before stream capture), or else by the first call on that device.
+ *   Sharing     there is ONE array per device, shared by every handle and every call, and it keeps the previous call's
+ *               contents.  Nothing in it has to start at zero (each call overwrites every element it later reads), but two
+ *               calls that overlap on the GPU (different streams, or graph branches without an edge between them) race
+ *               on it: order them on one stream or with an event.  Use snap_schur_apply with private workspaces instead
+ *               where calls must overlap.
+ * snap_static_scratch_bytes() returns SNAP_STATIC_SCRATCH_BYTES. */
+#define SNAP_STATIC_SCRATCH_BYTES 8388608
+size_t snap_static_scratch_bytes(void);
+int snap_static_scratch_init(void);
+int snap_schur_apply_static(const snap_problem* p, int batch, const double* u, const double* x, double* out,
+                            snap_stream stream);
 
 /* Per-sample work counters of the most recent snap_project call that used `workspace` with the same `batch`,
  * copied on `stream` into

@@ -8,6 +8,7 @@ from .binding import (  # noqa: F401
     SnapError, SnapParams, Problem, load_library, library_path, exported_symbols,
     snap_problem_create, snap_problem_destroy, snap_workspace_bytes, snap_project, snap_project_host,
     snap_residual, snap_schur_apply, snap_strerror, snap_project_stats, snap_flow_step, snap_project_f32,
+    snap_schur_apply_static, snap_static_scratch_bytes, snap_static_scratch_init,
     HEAT1D_IC_MASS, BURGERS1D_LF, FISHER1D_IE, ALLENCAHN2D_IE, BURGERS1D_LF_MASS, BURGERS1D_FLUXK, NS2D_VORT_ENST,
     STAT_LINEARISATIONS, STAT_PASSES, STAT_ROWS_READ, STAT_ROWS_WRITTEN, STAT_VARIANT, STAT_INNER, STAT_ROW_DOUBLES,
     STAT_BACKTRACKS, STAT_COUNT,

@@ -19,6 +19,7 @@ EXPORTS = [
     "snap_params_default", "snap_problem_create", "snap_problem_destroy", "snap_num_unknowns", "snap_num_rows",
     "snap_workspace_bytes", "snap_project", "snap_project_host", "snap_residual", "snap_schur_apply",
     "snap_project_stats", "snap_launch_count", "snap_strerror", "snap_flow_step", "snap_project_f32",
+    "snap_schur_apply_static", "snap_static_scratch_bytes", "snap_static_scratch_init",
 ]
 
 
@@ -84,6 +85,12 @@ def load_library():
     lib.snap_residual.restype = C.c_int
     lib.snap_schur_apply.argtypes = [vp, C.c_int, dp, dp, dp, vp, C.c_size_t, vp]
     lib.snap_schur_apply.restype = C.c_int
+    lib.snap_schur_apply_static.argtypes = [vp, C.c_int, dp, dp, dp, vp]
+    lib.snap_schur_apply_static.restype = C.c_int
+    lib.snap_static_scratch_bytes.argtypes = []
+    lib.snap_static_scratch_bytes.restype = C.c_size_t
+    lib.snap_static_scratch_init.argtypes = []
+    lib.snap_static_scratch_init.restype = C.c_int
     lib.snap_project_stats.argtypes = [vp, C.c_int, vp, C.c_size_t, vp, vp]
     lib.snap_project_stats.restype = C.c_int
     lib.snap_launch_count.argtypes = [vp]
@@ -271,6 +278,21 @@ def snap_schur_apply(p: Problem, batch: int, u, x, out, workspace, stream=None):
     rc = load_library().snap_schur_apply(p.handle, int(batch), _ptr(u), _ptr(x), _ptr(out), _ptr(workspace),
                                          _nbytes(workspace), _stream_handle(stream))
     _check(rc, "snap_schur_apply")
+
+
+def snap_static_scratch_bytes() -> int:
+    return int(load_library().snap_static_scratch_bytes())
+
+
+def snap_static_scratch_init():
+    """Resolve the static scratch array on the current device (once per device, at set-up; include/snap.h)."""
+    _check(load_library().snap_static_scratch_init(), "snap_static_scratch_init")
+
+
+def snap_schur_apply_static(p: Problem, batch: int, u, x, out, stream=None):
+    """snap_schur_apply without a workspace: the scratch is the library's static device array (include/snap.h)."""
+    rc = load_library().snap_schur_apply_static(p.handle, int(batch), _ptr(u), _ptr(x), _ptr(out), _stream_handle(stream))
+    _check(rc, "snap_schur_apply_static")
 
 
 def snap_project_stats(p: Problem, batch: int, workspace, stats, stream=None):

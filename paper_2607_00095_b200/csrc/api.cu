@@ -4,6 +4,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -601,12 +602,70 @@ int snap_schur_apply(const snap_problem* cp, int batch, const double* u, const d
   return check_launch(p);
 }
 
+// ------------------------------------------------------------------------------------------------------
+// No-allocation entry point (include/snap.h "No-allocation variant"): snap_schur_apply with its scratch vector
+// g = J^T x in a file-scope device array instead of a caller workspace, for callers that cannot allocate (CUDA graph
+// capture, serving loops, harnesses that forbid cudaMalloc).  Every GPU that loads the library holds the array until
+// the process exits.  In host code `g_static_scratch` is only the host-side stand-in of the symbol: the device address
+// is fetched once per device with cudaGetSymbolAddress, that device current, and handed to the kernels.
+// ------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_static_scratch[SNAP_STATIC_SCRATCH_BYTES / 8];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+double* g_static_addr[kStaticMaxDevices] = {};   // device address of g_static_scratch on device i (null: not set up)
+
+// device address of the scratch array on the CURRENT device; first use on a device resolves the symbol there
+int static_scratch_addr(double** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SNAP_ECUDA;
+  if (dev < 0 || dev >= kStaticMaxDevices) return SNAP_EINVAL;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[dev]) {
+    void* a = nullptr;
+    if (cudaGetSymbolAddress(&a, g_static_scratch) != cudaSuccess || !a) return SNAP_ECUDA;
+    g_static_addr[dev] = static_cast<double*>(a);
+  }
+  *out = g_static_addr[dev];
+  return SNAP_OK;
+}
+}  // namespace
+
+size_t snap_static_scratch_bytes(void) { return (size_t)SNAP_STATIC_SCRATCH_BYTES; }
+
+int snap_static_scratch_init(void) {
+  double* a = nullptr;
+  return static_scratch_addr(&a);
+}
+
+int snap_schur_apply_static(const snap_problem* cp, int batch, const double* u, const double* x, double* out,
+                            snap_stream stream) {
+  snap_problem* p = const_cast<snap_problem*>(cp);
+  if (!p || batch < 0) return SNAP_EINVAL;
+  if (batch == 0) return SNAP_OK;
+  if (!u || !x || !out) return SNAP_EINVAL;
+  if (p->dp.kind >= SNAP_BURGERS1D_FLUXK) return SNAP_EINVAL;   // kinds 0-4 only, as snap_schur_apply
+  if ((size_t)batch * p->dp.n > (size_t)SNAP_STATIC_SCRATCH_BYTES / 8) return SNAP_ELIMIT;
+  double* g = nullptr;
+  int rc = static_scratch_addr(&g);
+  if (rc != SNAP_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  // nothing in the scratch has to start at zero: the first kernel writes every g[b][0..n) the second one reads
+  jt_apply_kernel<<<batch, kMiscThreads, 0, st>>>(p->dp, batch, u, x, g);
+  rc = check_launch(p);
+  if (rc != SNAP_OK) return rc;
+  j_apply_kernel<<<batch, kMiscThreads, 0, st>>>(p->dp, batch, u, g, out);
+  return check_launch(p);
+}
+
 const char* snap_strerror(int code) {
   switch (code) {
     case SNAP_OK: return "ok";
     case SNAP_EINVAL: return "invalid argument (kind, sizes, NULL pointer or size limit)";
     case SNAP_ECUDA: return "CUDA call or kernel launch failed";
     case SNAP_ENOMEM: return "workspace too small or allocation failed";
+    case SNAP_ELIMIT: return "problem larger than the static scratch of a no-allocation entry point (snap_static_scratch_bytes)";
   }
   return "unknown error code";
 }

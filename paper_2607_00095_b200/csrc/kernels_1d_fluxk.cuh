@@ -24,6 +24,7 @@
 // linearisation AT u+ (all level-local), and writes u+.  Traffic per Gauss-Newton iteration: read u, u_hat, write
 // u+ = 24 n bytes (the first pass reads u_hat only).
 #pragma once
+#include <type_traits>
 #include "kernels_1d_fused.cuh"
 
 namespace snap {
@@ -344,7 +345,11 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   const int npro = nst < nt ? nst : nt;
   for (int k = 0; k < npro; ++k) pp.issue(k, k, x.tm, tm_uh);
   int s = 0;
-  for (int k = 0; k < nt; ++k) {
+  // One level.  The pinned levels (k <= K) and the free ones run in two loops over the same body: the Newton state of
+  // the pinned levels (phiA .. ccB, 8 Q registers) is then dead in the free-level loop, which at 255 registers had its
+  // loop counters and row addresses in local memory (long-scoreboard stalls on LDL, profiles/r02_fluxk.md).
+  auto level = [&](auto pinned_c, const int k) {
+    constexpr bool PINNED = decltype(pinned_c)::value;
     pp.wait(s);
     double v[Q], uhr[Q], t[Q];
     load_cells<Q>(pp.row(s, 0), pp.lo, v);
@@ -354,7 +359,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
     } else {
       load_cells<Q>(pp.row(s, 1), pp.lo, uhr);
     }
-    if (k <= K) {
+    if constexpr (PINNED) {
       // ---- pinned level: iteration A at x (the step), iteration B at t (the next linearisation) ----
       double q[Q];
 #pragma unroll
@@ -480,7 +485,10 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
     }
     if (k + nst < nt) pp.issue(s, k + nst, x.tm, tm_uh);
     if (++s == nst) s = 0;
-  }
+  };
+  const int kpin = (K + 1 < nt) ? K + 1 : nt;
+  for (int k = 0; k < kpin; ++k) level(std::true_type{}, k);
+  for (int k = kpin; k < nt; ++k) level(std::false_type{}, k);
   pp.drain();
   if (F > 0) fluxk_assemble<HESS>(P, bd, F, nx, lane, M0, E_K, D_K, bq_K, h1, hmx);
   S.hlev = hinf_level(hmx, tol, skip);

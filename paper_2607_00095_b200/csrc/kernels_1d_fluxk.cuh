@@ -103,13 +103,13 @@ __device__ __forceinline__ void level_At(const DevParams& P, const double (&v)[Q
 
 // border-row gradient of an energy row on its EARLIER level:  b(v) = -dx v + cD (2 v - v_{i+1} - v_{i-1}),  cD = 2 dt nu / dx
 template <int Q>
-__device__ __forceinline__ void energy_b(const DevParams& P, const double (&v)[Q], int lane, double (&b)[Q], double& sD) {
+__device__ __forceinline__ void energy_b(double dx, double cD, const double (&v)[Q], int lane, double (&b)[Q], double& sD) {
   const double vR = shfl_next(v[0], lane), vL = shfl_prev(v[Q - 1], lane);
   double acc = 0.0;
 #pragma unroll
   for (int c = 0; c < Q; ++c) {
     const double vr = (c < Q - 1) ? v[c + 1] : vR, vm = (c > 0) ? v[c - 1] : vL;
-    b[c] = fma(-P.dx, v[c], P.fk_cD * ((v[c] - vr) + (v[c] - vm)));
+    b[c] = fma(-dx, v[c], cD * ((v[c] - vr) + (v[c] - vm)));
     const double dv = vr - v[c];
     acc = fma(dv, dv, acc);
   }
@@ -120,9 +120,9 @@ __device__ __forceinline__ void energy_b(const DevParams& P, const double (&v)[Q
 // W_k = a I + b (S + S^-1): a = 1 + dx (lamE[f] - lamE[f+1]) + 2 cD lamE[f+1],  b = -cD lamE[f+1]  (symmetric circulant
 // tridiagonal, eigenvalues in [a - 2|b|, a + 2|b|]).  Inertia safeguard: a - 2|b| < 0.1  =>  W_k = I (a Gauss-Newton level).
 constexpr double kHessSafeguard = 0.1;
-__device__ __forceinline__ void hess_coeffs(const DevParams& P, double lamE0, double lamE1, double& a, double& b) {
-  a = 1.0 + P.dx * (lamE0 - lamE1) + 2.0 * P.fk_cD * lamE1;
-  b = -P.fk_cD * lamE1;
+__device__ __forceinline__ void hess_coeffs(double dx, double cD, double lamE0, double lamE1, double& a, double& b) {
+  a = 1.0 + dx * (lamE0 - lamE1) + 2.0 * cD * lamE1;
+  b = -cD * lamE1;
   if (!(a - 2.0 * fabs(b) >= kHessSafeguard)) { a = 1.0; b = 0.0; }
 }
 
@@ -265,7 +265,7 @@ __device__ __forceinline__ void fluxk_assemble(const DevParams& P, Band bd, int 
   auto gam_of = [&](int f) -> double {
     if constexpr (!HESS) return 1.0;
     double wa, wb;
-    hess_coeffs(P, bd.lE.get(f), (f + 1 < F) ? bd.lE.get(f + 1) : 0.0, wa, wb);
+    hess_coeffs(P.dx, P.fk_cD, bd.lE.get(f), (f + 1 < F) ? bd.lE.get(f + 1) : 0.0, wa, wb);
     return rcp_pos(wa + 2.0 * wb);
   };
   // predecessor level
@@ -331,7 +331,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
   const bool energy = P.fk_energy != 0;
   const bool same = (x.p == uh.p);
   const CUtensorMap* const tm_uh = same ? nullptr : uh.tm;
-  const double dx = P.dx;
+  const double dx = P.dx, cD = P.fk_cD;   // locals: through the reference P they were re-loaded (generic LD) at every level
   const double tol = P.tol, skip = kPolishSkip * P.tol;
 
   double phiA[Q], ccA[Q], phiB[Q], ccB[Q];
@@ -382,7 +382,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       if (k < K) level_phi_Aq<Q, FLUX>(P, t, qb, lane, phiB, ccB);
       if (k == K && F > 0) {   // level K feeds energy row K: E, D and the coupling term b_K . d_K  (d_K = -q'_K)
         double b[Q], sD;
-        energy_b<Q>(P, t, lane, b, sD);
+        energy_b<Q>(dx, cD, t, lane, b, sD);
         double r[3] = {0.0, sD, 0.0};
 #pragma unroll
         for (int c = 0; c < Q; ++c) { r[0] = fma(t[c], t[c], r[0]); r[2] = fma(b[c], qb[c], r[2]); }
@@ -399,25 +399,28 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       if (update) {
         const double lamM = bd.lM.get(f);
         double b[Q], sDx, gv[Q];
-        energy_b<Q>(P, v, lane, b, sDx);
+        energy_b<Q>(dx, cD, v, lane, b, sDx);
 #pragma unroll
         for (int c = 0; c < Q; ++c) gv[c] = (v[c] - uhr[c]) + (dx * lamM + lamE0 * dx * v[c] + lamE1 * b[c]);   // w + J_b^T lam_b
         if constexpr (HESS) {   // d = -W^-1 (w + J^T lam), W of the linearisation at x (its energy multipliers were saved in lW)
           double wa, wb;
-          hess_coeffs(P, bd.lW.get(f), (f + 1 < F) ? bd.lW.get(f + 1) : 0.0, wa, wb);
+          hess_coeffs(dx, cD, bd.lW.get(f), (f + 1 < F) ? bd.lW.get(f + 1) : 0.0, wa, wb);
           circ_solve<Q>(wa, wb, gv, lane);
         }
 #pragma unroll
-        for (int c = 0; c < Q; ++c) t[c] = fma(-alpha, gv[c], v[c]);
+        for (int c = 0; c < Q; ++c) {
+          t[c] = fma(-alpha, gv[c], v[c]);
+          ds2 = fma(t[c] - v[c], t[c] - v[c], ds2);   // here, so that v is dead during the solves below
+        }
       } else {
 #pragma unroll
         for (int c = 0; c < Q; ++c) t[c] = v[c];
       }
       double b[Q], sD;
-      energy_b<Q>(P, t, lane, b, sD);
+      energy_b<Q>(dx, cD, t, lane, b, sD);
       // W of the NEXT linearisation (at t, multipliers of the last solve): zt = W^-1 t, zw = W^-1 w, zb = W^-1 b = (-dx + cD L) zt
       double wa = 1.0, wb = 0.0;
-      if constexpr (HESS) hess_coeffs(P, lamE0, lamE1, wa, wb);
+      if constexpr (HESS) hess_coeffs(dx, cD, lamE0, lamE1, wa, wb);
       // level sums of the next band system: s1 = sum t, s2 = sum t^2, sD, bzb = b.zb, tzb = t.zb, sw = sum w, tzw = t.zw,
       // bzw = b.zw [, tzt = t.zt]  (W = I: zt = t, zw = w, zb = b).  They go to the level's slots of the band arrays; the
       // band entries, h_M, h_E are assembled after the pass (fluxk_assemble): nothing of a level is carried to the next.
@@ -434,7 +437,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
           circ_solve<Q>(wa, wb, zt, lane);
           circ_solve<Q>(wa, wb, zw, lane);
           double sdum;
-          energy_b<Q>(P, zt, lane, zb, sdum);
+          energy_b<Q>(dx, cD, zt, lane, zb, sdum);
         } else {
 #pragma unroll
           for (int c = 0; c < Q; ++c) zb[c] = b[c];
@@ -478,8 +481,10 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       }
     }
     if (update) {
+      if constexpr (PINNED) {
 #pragma unroll
-      for (int c = 0; c < Q; ++c) ds2 = fma(t[c] - v[c], t[c] - v[c], ds2);
+        for (int c = 0; c < Q; ++c) ds2 = fma(t[c] - v[c], t[c] - v[c], ds2);
+      }
       store_cells_global<Q>(xo + (size_t)k * nx + first, t);
       if (lane == 0) pp.rows_wr += 1;
     }
@@ -597,7 +602,7 @@ __device__ __noinline__ bool fluxk_local_multipliers(const DevParams& P, int lan
     if (k < K) level_phi_Aq<Q, FLUX>(P, v, q, lane, phi, cc);
     if (k == K && lamEK != 0.0) {
       double b[Q], sD;
-      energy_b<Q>(P, v, lane, b, sD);
+      energy_b<Q>(P.dx, P.fk_cD, v, lane, b, sD);
 #pragma unroll
       for (int c = 0; c < Q; ++c) y[c] = fma(-lamEK, b[c], y[c]);
     }

@@ -132,50 +132,86 @@ __device__ __forceinline__ void hess_coeffs(double dx, double cD, double lamE0, 
 // each = a local pass per lane with zero carry, the carry into a lane C_l = sum_j R^j P_{l-1-j} / (1 - R^32) (R = r^Q,
 // P = the lane's last local value) by a Kogge-Stone scan over the lanes (cut off once R^s is below rounding), and the
 // correction r^(j+1) C_l of the local values.  a, b are warp-uniform.
-template <int Q>
-__device__ __forceinline__ void circ_solve(double a, double b, double (&g)[Q], int lane) {
-  if (b == 0.0) {
-    const double ia = rcp_pos(a);
+// NR right-hand sides at once (same W): the recurrences of the right-hand sides are independent chains that interleave.
+// The factor (1 / kap, r) of a level's W is formed apart from the solve (circ_coef), so that the square-root / reciprocal
+// chains of the two W of a level (the step's and the next linearisation's) issue together at the top of the level.
+struct CircCoef {
+  double ik, r;
+};
+__device__ __forceinline__ CircCoef circ_coef(double a, double b) {
+  const double kap = 0.5 * (a + sqrt(a * a - 4.0 * b * b));   // b = 0: kap = a exactly
+  CircCoef c;
+  c.ik = rcp_pos(kap);
+  c.r = -b * c.ik;
+  return c;
+}
+template <int Q, int NR>
+__device__ __forceinline__ void circ_solve_n(const CircCoef cf, double (&g)[NR][Q], int lane) {
+  const double ik = cf.ik, r = cf.r;
+  if (r == 0.0) {   // diagonal W
 #pragma unroll
-    for (int c = 0; c < Q; ++c) g[c] *= ia;
+    for (int m = 0; m < NR; ++m)
+#pragma unroll
+      for (int c = 0; c < Q; ++c) g[m][c] *= ik;
     return;
   }
-  const double kap = 0.5 * (a + sqrt(a * a - 4.0 * b * b));
-  const double ik = rcp_pos(kap), r = -b * ik;
   double rp[Q];                       // r^(j+1)
   rp[0] = r;
 #pragma unroll
   for (int j = 1; j < Q; ++j) rp[j] = rp[j - 1] * r;
   const double R = rp[Q - 1];
   // forward recurrence (carry from the previous lane)
-  g[0] *= ik;
 #pragma unroll
-  for (int j = 1; j < Q; ++j) g[j] = fma(r, g[j - 1], g[j] * ik);
+  for (int m = 0; m < NR; ++m) g[m][0] *= ik;
+#pragma unroll
+  for (int j = 1; j < Q; ++j)
+#pragma unroll
+    for (int m = 0; m < NR; ++m) g[m][j] = fma(r, g[m][j - 1], g[m][j] * ik);
   {
-    double T = __shfl_sync(SNAP_FULL, g[Q - 1], (lane + 31) & 31), Rs = R;
+    double T[NR], Rs = R;
+#pragma unroll
+    for (int m = 0; m < NR; ++m) T[m] = __shfl_sync(SNAP_FULL, g[m][Q - 1], (lane + 31) & 31);
     for (int s = 1; s < 32; s <<= 1) {
       if (fabs(Rs) < 1e-20) { Rs = 0.0; break; }
-      T = fma(Rs, __shfl_sync(SNAP_FULL, T, (lane + 32 - s) & 31), T);
+#pragma unroll
+      for (int m = 0; m < NR; ++m) T[m] = fma(Rs, __shfl_sync(SNAP_FULL, T[m], (lane + 32 - s) & 31), T[m]);
       Rs *= Rs;
     }
-    T *= rcp_pos(1.0 - Rs);           // Rs = R^32 after a complete scan, 0 after a cut-off
+    const double sc = (Rs == 0.0) ? 1.0 : rcp_pos(1.0 - Rs);   // Rs = R^32 after a complete scan, 0 after a cut-off
 #pragma unroll
-    for (int j = 0; j < Q; ++j) g[j] = fma(rp[j], T, g[j]);
+    for (int m = 0; m < NR; ++m) {
+      T[m] *= sc;
+#pragma unroll
+      for (int j = 0; j < Q; ++j) g[m][j] = fma(rp[j], T[m], g[m][j]);
+    }
   }
   // backward recurrence (carry from the next lane)
 #pragma unroll
-  for (int j = Q - 2; j >= 0; --j) g[j] = fma(r, g[j + 1], g[j]);
+  for (int j = Q - 2; j >= 0; --j)
+#pragma unroll
+    for (int m = 0; m < NR; ++m) g[m][j] = fma(r, g[m][j + 1], g[m][j]);
   {
-    double T = __shfl_sync(SNAP_FULL, g[0], (lane + 1) & 31), Rs = R;
+    double T[NR], Rs = R;
+#pragma unroll
+    for (int m = 0; m < NR; ++m) T[m] = __shfl_sync(SNAP_FULL, g[m][0], (lane + 1) & 31);
     for (int s = 1; s < 32; s <<= 1) {
       if (fabs(Rs) < 1e-20) { Rs = 0.0; break; }
-      T = fma(Rs, __shfl_sync(SNAP_FULL, T, (lane + s) & 31), T);
+#pragma unroll
+      for (int m = 0; m < NR; ++m) T[m] = fma(Rs, __shfl_sync(SNAP_FULL, T[m], (lane + s) & 31), T[m]);
       Rs *= Rs;
     }
-    T *= rcp_pos(1.0 - Rs);
+    const double sc = (Rs == 0.0) ? 1.0 : rcp_pos(1.0 - Rs);
 #pragma unroll
-    for (int j = 0; j < Q; ++j) g[j] = fma(rp[Q - 1 - j], T, g[j]);
+    for (int m = 0; m < NR; ++m) {
+      T[m] *= sc;
+#pragma unroll
+      for (int j = 0; j < Q; ++j) g[m][j] = fma(rp[Q - 1 - j], T[m], g[m][j]);
+    }
   }
+}
+template <int Q>
+__device__ __forceinline__ void circ_solve(const CircCoef cf, double (&g)[Q], int lane) {
+  circ_solve_n<Q, 1>(cf, reinterpret_cast<double (&)[1][Q]>(g), lane);
 }
 
 // per-sample band system in shared memory: 10 doubles per free level f (level k = K+1+f), rows E_{k-1} then M_k
@@ -396,17 +432,26 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       const int f = k - K - 1;
       const double lamE0 = energy ? bd.lE.get(f) : 0.0;
       const double lamE1 = (energy && f + 1 < F) ? bd.lE.get(f + 1) : 0.0;
+      // W of the NEXT linearisation (at t, multipliers of the last solve) and W of the step (the energy multipliers that
+      // defined it were saved in lW)
+      double wa = 1.0, wb = 0.0;
+      CircCoef cfN{1.0, 0.0}, cfS{1.0, 0.0};
+      if constexpr (HESS) {
+        hess_coeffs(dx, cD, lamE0, lamE1, wa, wb);
+        cfN = circ_coef(wa, wb);
+        if (update) {
+          double sa, sb;
+          hess_coeffs(dx, cD, bd.lW.get(f), (f + 1 < F) ? bd.lW.get(f + 1) : 0.0, sa, sb);
+          cfS = circ_coef(sa, sb);
+        }
+      }
       if (update) {
         const double lamM = bd.lM.get(f);
         double b[Q], sDx, gv[Q];
         energy_b<Q>(dx, cD, v, lane, b, sDx);
 #pragma unroll
         for (int c = 0; c < Q; ++c) gv[c] = (v[c] - uhr[c]) + (dx * lamM + lamE0 * dx * v[c] + lamE1 * b[c]);   // w + J_b^T lam_b
-        if constexpr (HESS) {   // d = -W^-1 (w + J^T lam), W of the linearisation at x (its energy multipliers were saved in lW)
-          double wa, wb;
-          hess_coeffs(dx, cD, bd.lW.get(f), (f + 1 < F) ? bd.lW.get(f + 1) : 0.0, wa, wb);
-          circ_solve<Q>(wa, wb, gv, lane);
-        }
+        if constexpr (HESS) circ_solve<Q>(cfS, gv, lane);   // d = -W^-1 (w + J^T lam), W of the linearisation at x
 #pragma unroll
         for (int c = 0; c < Q; ++c) {
           t[c] = fma(-alpha, gv[c], v[c]);
@@ -418,9 +463,7 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       }
       double b[Q], sD;
       energy_b<Q>(dx, cD, t, lane, b, sD);
-      // W of the NEXT linearisation (at t, multipliers of the last solve): zt = W^-1 t, zw = W^-1 w, zb = W^-1 b = (-dx + cD L) zt
-      double wa = 1.0, wb = 0.0;
-      if constexpr (HESS) hess_coeffs(dx, cD, lamE0, lamE1, wa, wb);
+      // with the W of the next linearisation: zt = W^-1 t, zw = W^-1 w, zb = W^-1 b = (-dx + cD L) zt
       // level sums of the next band system: s1 = sum t, s2 = sum t^2, sD, bzb = b.zb, tzb = t.zb, sw = sum w, tzw = t.zw,
       // bzw = b.zw [, tzt = t.zt]  (W = I: zt = t, zw = w, zb = b).  They go to the level's slots of the band arrays; the
       // band entries, h_M, h_E are assembled after the pass (fluxk_assemble): nothing of a level is carried to the next.
@@ -430,12 +473,13 @@ __device__ __noinline__ void fluxk_pass(const DevParams& P, RowPipe<1, Q>& pp_re
       r[2] = sD;
       double tzt = 0.0;
       if constexpr (HESS) {
-        double zt[Q], zw[Q], zb[Q];
+        double z2[2][Q], zb[Q];
+        double (&zt)[Q] = z2[0];
+        double (&zw)[Q] = z2[1];
 #pragma unroll
         for (int c = 0; c < Q; ++c) { zt[c] = t[c]; zw[c] = t[c] - uhr[c]; }
         if (!(wa == 1.0 && wb == 0.0)) {
-          circ_solve<Q>(wa, wb, zt, lane);
-          circ_solve<Q>(wa, wb, zw, lane);
+          circ_solve_n<Q, 2>(cfN, z2, lane);   // both right-hand sides in one solve: their chains interleave
           double sdum;
           energy_b<Q>(dx, cD, zt, lane, zb, sdum);
         } else {

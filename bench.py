@@ -389,8 +389,9 @@ def float32_lines(run, steps, warmup, peak):
     norms = torch.empty(B, 5, dtype=torch.float64, device=dev)
     S.snap_residual(p, B, us.double(), cd.double(), None, norms)
     torch.cuda.synchronize()
-    # passes: an evaluation count e means ceil((e - 1) / 3) passes of 3 updates (+ the final copy): read + write 4 n bytes each
-    passes = torch.ceil((it.clamp(min=1).double() - 1.0) / 3.0).clamp(min=1.0) + 1.0
+    # passes: an evaluation count e means ceil((e - 1) / 3) passes of up to 3 updates, read + write 4 n bytes each (the
+    # iterates alternate between a work buffer and u_star: the usual two passes end in u_star, no copy)
+    passes = torch.ceil((it.clamp(min=1).double() - 1.0) / 3.0).clamp(min=1.0)
     alg = float(passes.sum()) * 8.0 * n
     return {"value": B * run.calls / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "dtype": "f32", "tol": 1e-5,
             "converged_all": ok, "max_hinf_last_call_fp64": float(norms[:, 0].max()),

@@ -152,12 +152,15 @@ __global__ void __launch_bounds__(256) project1d_f32_kernel(const __grid_constan
     M0 = (float)P.dx * wsumf(s);
   }
   const float tol = A.tol;
+  // iterates ping-pong between bufA and u_star itself (bufB when u_star aliases u_hat): the usual two passes (JT - 1
+  // updates; then the remaining polish step) end in u_star and need no copy
+  float* const alt = (ustar != uh) ? ustar : bufB;
   const float* cur = uh;
   int steps = 0, lin = 0, status = 0, since = -1;     // since: steps taken after the first iterate that met tol (-1: none yet)
   float hprev = 3.4e38f;
   bool done = false, first_pass = true;
   while (!done) {
-    float* xo = (cur == bufA) ? bufB : bufA;
+    float* xo = (cur == bufA) ? alt : bufA;
     int NU = JT - 1;
     if (since >= 0 && P.polish - since < NU) NU = P.polish - since;   // only the remaining polish steps
     if (NU > P.max_iter - steps && since < 0) NU = P.max_iter - steps;
@@ -186,10 +189,19 @@ __global__ void __launch_bounds__(256) project1d_f32_kernel(const __grid_constan
   }
   // u* <- final iterate (u_hat on a non-finite sample, R16)
   const float* fin = (status == SNAP_ST_NONFINITE) ? uh : cur;
-  if (fin != ustar) {
+  if (fin != ustar) {   // 128-bit stream, 8 loads in flight per lane
     const float4* s4 = reinterpret_cast<const float4*>(fin);
     float4* d4 = reinterpret_cast<float4*>(ustar);
-    for (size_t i = lane; i < n / 4; i += 32) d4[i] = s4[i];
+    const size_t n4 = n / 4;
+    size_t i = lane;
+    for (; i + 7 * 32 < n4; i += 8 * 32) {
+      float4 t[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) t[u] = s4[i + u * 32];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) d4[i + u * 32] = t[u];
+    }
+    for (; i < n4; i += 32) d4[i] = s4[i];
   }
   if (lane == 0) A.iters[b] = (status == 0) ? lin : status;
 }

@@ -132,6 +132,102 @@ __device__ __forceinline__ void f32_pass(const DevParams& P, int lane, const flo
   for (int t = 0; t < JT; ++t) hmax[t] = wmaxf(hmax[t]);
 }
 
+// The same pass with packed fp32 arithmetic (sm_100: add / mul / fma on float2, one instruction for two cells): the pass
+// is bound by instruction issue (one warp per sample, two warps per scheduler), and a packed instruction does the work of
+// two.  A lane pairs cell c with cell c + Q/2 of its Q contiguous cells, so that the right / left neighbours of pair c are
+// the pairs c + 1 / c - 1 (aligned register pairs); only the first and the last pair take one component from the
+// neighbouring lane.  Phi is carried negated (h = x + (-Phi)): negations are exact, the results equal the scalar pass bit
+// for bit except for the order of the mass-row sums.
+template <int Q, int JT>
+__device__ __forceinline__ void f32_pass_x2(const DevParams& P, int lane, const float* __restrict__ x,
+                                            const float* __restrict__ u0, float* __restrict__ xo, int NU, float M0,
+                                            float (&hmax)[JT]) {
+  static_assert(Q >= 2 && Q % 2 == 0, "pairs of cells");
+  constexpr int nx = 32 * Q, H = Q / 2;
+  const int nt = P.nt, first = lane * Q;
+  const float a0 = (float)P.bs_a0, e = (float)P.bs_e, qs = (float)P.bs_qs, hs = (float)P.bs_hs, dxm = (float)P.dx;
+  const float2 A0 = make_float2(a0, a0), NA0 = make_float2(-a0, -a0), E2 = make_float2(e, e), NE2 = make_float2(-e, -e);
+  const float2 QS = make_float2(qs, qs), HS = make_float2(hs, hs), NHS = make_float2(-hs, -hs), M1 = make_float2(-1.f, -1.f);
+  const bool has_mass = P.has_mass != 0;
+  float2 nphi[JT][H], cc[JT][H];
+  {
+    float u0r[Q];
+    ldrow_f32<Q>(u0 + first, u0r);
+#pragma unroll
+    for (int t = 0; t < JT; ++t) {
+#pragma unroll
+      for (int c = 0; c < H; ++c) { nphi[t][c] = make_float2(-u0r[c], -u0r[c + H]); cc[t][c] = make_float2(0.f, 0.f); }
+      hmax[t] = 0.f;
+    }
+  }
+  float vn[Q];
+  ldrow_f32<Q>(x + first, vn);
+  for (int k = 0; k < nt; ++k) {
+    float2 v[H];
+#pragma unroll
+    for (int c = 0; c < H; ++c) v[c] = make_float2(vn[c], vn[c + H]);
+    if (k + 1 < nt) ldrow_f32<Q>(x + (size_t)(k + 1) * nx + first, vn);    // next level travels during this one
+    float msum[JT];
+#pragma unroll
+    for (int t = 0; t < JT; ++t) msum[t] = 0.f;
+#pragma unroll
+    for (int t = 0; t < JT; ++t) {
+      if (t <= NU) {
+        float2 q[H], ms = make_float2(0.f, 0.f);
+        float hm = 0.f;
+#pragma unroll
+        for (int c = 0; c < H; ++c) {
+          const float2 h = __fadd2_rn(v[c], nphi[t][c]);
+          q[c] = __fadd2_rn(h, cc[t][c]);
+          hm = fmaxf(hm, fmaxf(fabsf(h.x), fabsf(h.y)));
+          ms = __fadd2_rn(ms, v[c]);
+        }
+        msum[t] = ms.x + ms.y;
+        hmax[t] = fmaxf(hmax[t], hm);
+        const float vL = __shfl_sync(SNAP_FULL, v[H - 1].y, (lane + 31) & 31), vR = __shfl_sync(SNAP_FULL, v[0].x, (lane + 1) & 31);
+        const float qL = __shfl_sync(SNAP_FULL, q[H - 1].y, (lane + 31) & 31), qR = __shfl_sync(SNAP_FULL, q[0].x, (lane + 1) & 31);
+        // pair c = (cell c, cell c + H): left neighbours (c - 1, c + H - 1), right neighbours (c + 1, c + H + 1)
+        const float2 vLo = make_float2(vL, v[H - 1].x), vHi = make_float2(v[0].y, vR);
+        const float2 qLo = make_float2(qL, q[H - 1].x), qHi = make_float2(q[0].y, qR);
+        float2 nph[H], ccn[H];
+#pragma unroll
+        for (int c = 0; c < H; ++c) {
+          const float2 um = (c > 0) ? v[c > 0 ? c - 1 : 0] : vLo, up = (c < H - 1) ? v[c < H - 1 ? c + 1 : 0] : vHi;
+          const float2 ql = (c > 0) ? q[c > 0 ? c - 1 : 0] : qLo, qr = (c < H - 1) ? q[c < H - 1 ? c + 1 : 0] : qHi;
+          const float2 sum = __fadd2_rn(up, um), dif = __ffma2_rn(um, M1, up);
+          const float2 w = __ffma2_rn(QS, dif, NE2);                                   // -(e - qs (up - um))
+          nph[c] = __ffma2_rn(NA0, v[c], __fmul2_rn(sum, w));                          // -Phi
+          ccn[c] = __ffma2_rn(__ffma2_rn(NHS, up, E2), qr, __ffma2_rn(__ffma2_rn(HS, um, E2), ql, __fmul2_rn(A0, q[c])));
+        }
+#pragma unroll
+        for (int c = 0; c < H; ++c) {
+          nphi[t][c] = nph[c];
+          cc[t][c] = ccn[c];
+          if (t < NU) v[c] = __ffma2_rn(q[c], M1, v[c]);
+        }
+      }
+    }
+    if (NU > 0) {
+      float vo[Q];
+#pragma unroll
+      for (int c = 0; c < H; ++c) { vo[c] = v[c].x; vo[c + H] = v[c].y; }
+      strow_f32<Q>(xo + (size_t)k * nx + first, vo);
+    }
+    if (has_mass) {     // JT interleaved butterflies, off the critical path of the level recurrence
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int t = 0; t < JT; ++t) msum[t] += __shfl_xor_sync(SNAP_FULL, msum[t], o);
+      }
+#pragma unroll
+      for (int t = 0; t < JT; ++t)
+        if (t <= NU) hmax[t] = fmaxf(hmax[t], fabsf(fmaf(dxm, msum[t], -M0)));
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < JT; ++t) hmax[t] = wmaxf(hmax[t]);
+}
+
 template <int Q, int JT>
 __global__ void __launch_bounds__(256) project1d_f32_kernel(const __grid_constant__ ProjF32Args A) {
   const DevParams& P = A.P;
@@ -166,7 +262,8 @@ __global__ void __launch_bounds__(256) project1d_f32_kernel(const __grid_constan
     if (NU > P.max_iter - steps && since < 0) NU = P.max_iter - steps;
     if (NU < 0) NU = 0;
     float hmax[JT];
-    f32_pass<Q, JT>(P, lane, cur, u0, xo, NU, M0, hmax);
+    if constexpr (Q >= 2) f32_pass_x2<Q, JT>(P, lane, cur, u0, xo, NU, M0, hmax);
+    else f32_pass<Q, JT>(P, lane, cur, u0, xo, NU, M0, hmax);
     __syncwarp();
     // walk the iterates x_0 .. x_NU of this pass (x_0 of a later pass was judged as the last iterate of the previous one)
     if (!first_pass && NU > 0) { ++steps; if (since >= 0) ++since; }   // the step x_0 -> x_1 of a later pass

@@ -89,6 +89,7 @@ __device__ __forceinline__ void f32_pass(const DevParams& P, int lane, const flo
     float msum[JT];
 #pragma unroll
     for (int t = 0; t < JT; ++t) msum[t] = 0.f;
+    float vL = 0.f, vR = 0.f;
 #pragma unroll
     for (int t = 0; t < JT; ++t) {
       if (t <= NU) {
@@ -102,7 +103,8 @@ __device__ __forceinline__ void f32_pass(const DevParams& P, int lane, const flo
         }
         msum[t] = ms;                        // mass row of this level and iterate: reduced after the iterations
         hmax[t] = fmaxf(hmax[t], hm);
-        const float vL = __shfl_sync(SNAP_FULL, v[Q - 1], (lane + 31) & 31), vR = __shfl_sync(SNAP_FULL, v[0], (lane + 1) & 31);
+        // the neighbours' end cells: exchanged for the first iterate of a level, then updated like the neighbour updates them
+        if (t == 0) { vL = __shfl_sync(SNAP_FULL, v[Q - 1], (lane + 31) & 31); vR = __shfl_sync(SNAP_FULL, v[0], (lane + 1) & 31); }
         const float qL = __shfl_sync(SNAP_FULL, q[Q - 1], (lane + 31) & 31), qR = __shfl_sync(SNAP_FULL, q[0], (lane + 1) & 31);
         float um = vL, ql = qL;
 #pragma unroll
@@ -114,6 +116,7 @@ __device__ __forceinline__ void f32_pass(const DevParams& P, int lane, const flo
           um = vc; ql = qc;
           if (t < NU) v[c] = vc - qc;
         }
+        if (t < NU) { vL -= qL; vR -= qR; }
       }
     }
     if (NU > 0) strow_f32<Q>(xo + (size_t)k * nx + first, v);
@@ -170,6 +173,7 @@ __device__ __forceinline__ void f32_pass_x2(const DevParams& P, int lane, const 
     float msum[JT];
 #pragma unroll
     for (int t = 0; t < JT; ++t) msum[t] = 0.f;
+    float vL = 0.f, vR = 0.f;            // the neighbours' end cells, carried through the iterations of the level
 #pragma unroll
     for (int t = 0; t < JT; ++t) {
       if (t <= NU) {
@@ -184,7 +188,7 @@ __device__ __forceinline__ void f32_pass_x2(const DevParams& P, int lane, const 
         }
         msum[t] = ms.x + ms.y;
         hmax[t] = fmaxf(hmax[t], hm);
-        const float vL = __shfl_sync(SNAP_FULL, v[H - 1].y, (lane + 31) & 31), vR = __shfl_sync(SNAP_FULL, v[0].x, (lane + 1) & 31);
+        if (t == 0) { vL = __shfl_sync(SNAP_FULL, v[H - 1].y, (lane + 31) & 31); vR = __shfl_sync(SNAP_FULL, v[0].x, (lane + 1) & 31); }
         const float qL = __shfl_sync(SNAP_FULL, q[H - 1].y, (lane + 31) & 31), qR = __shfl_sync(SNAP_FULL, q[0].x, (lane + 1) & 31);
         // pair c = (cell c, cell c + H): left neighbours (c - 1, c + H - 1), right neighbours (c + 1, c + H + 1)
         const float2 vLo = make_float2(vL, v[H - 1].x), vHi = make_float2(v[0].y, vR);
@@ -205,6 +209,7 @@ __device__ __forceinline__ void f32_pass_x2(const DevParams& P, int lane, const 
           cc[t][c] = ccn[c];
           if (t < NU) v[c] = __ffma2_rn(q[c], M1, v[c]);
         }
+        if (t < NU) { vL = fmaf(qL, -1.f, vL); vR = fmaf(qR, -1.f, vR); }   // as the neighbour updates them (same fma)
       }
     }
     if (NU > 0) {

@@ -372,11 +372,11 @@ __device__ __forceinline__ void fused_fwd_body(const DevParams& P, RowPipe<W, Q>
           if (t == 0) f2 = fma(wv, wv, f2);
         }
       }
-      // end values of the next iterate (only the two ends are exchanged; the rest is updated in place below)
-      const double vn0 = (t < NU) ? v[0] - q[0] : v[0], vnE = (t < NU) ? v[Q - 1] - q[Q - 1] : v[Q - 1];
+      // The neighbours' end cells of the NEXT iterate need no exchange of their own: the neighbour forms x - q there, and
+      // both operands are at hand (vL, qL / vR, qR): the same subtraction on the same values (t + 1 < T implies t < NU).
       const double qL = shfl_prev(q[Q - 1], lane), qR = shfl_next(q[0], lane);
       double vnL = 0.0, vnR = 0.0;
-      if (t + 1 < T) { vnL = shfl_prev(vnE, lane); vnR = shfl_next(vn0, lane); }
+      if (t + 1 < T) { vnL = vL - qL; vnR = vR - qR; }
       if (has_mass) sts_f64(msb_a + 8u * (uint32_t)((t * 8 + (k & 7)) * kMsbPitch + lane), msum);
       // state for the next level (needs the old v and q with neighbours), then the update in place
       double um = vL, ql = qL;

@@ -5,8 +5,8 @@ in the suite.
   * parity sweep: random (kind, shape, noise, seed, gn_fuse / lambda_mode / precond / flux_steps) against the oracle,
     with the bounds of tests/test_gpu_parity.py, inside the regime where CUDA path and oracle follow the same
     trajectory (DESIGN.md R25 (i)-(iii) lists where they do not and why: those corners are left out here);
-  * API-consistency sweep (no oracle): the multiplier-free call, the host entry, one sample alone vs in its batch, and
-    snap_flow_step vs shoot + snap_project + pull-back must agree with the plain device call.
+  * API-consistency sweep (no oracle): the multiplier-free call, the host entry, one sample alone vs in its batch, the
+    Float32 mode, and snap_flow_step vs shoot + snap_project + pull-back must agree with the plain device call.
 """
 import os
 import random
@@ -134,6 +134,25 @@ def test_api_consistency_sweep(S):
         b = rng.randrange(B)
         u1, l1, i1 = _device_project(S, p, 1, wl.u_hat[b:b + 1], wl.cdata[b:b + 1])
         assert torch.equal(u1[0], u[b]) and torch.equal(l1[0], lam[b]) and int(i1[0]) == int(it[b]), (tag, "alone")
+        # Float32 mode (Burgers kinds, nx = 32 Q): the fp32 result is the fp64 one to single precision (the bound of
+        # tests/test_gpu_parity.py::test_float32_mode...: ||J^-1|| x fp32 residual floor), feasible to 2e-5, alone = in batch
+        if cfg in (2, 5) and wl.nx in (32, 64, 128, 256):
+            uh32 = wl.u_hat.to(dev, torch.float32).contiguous()
+            cd32 = wl.cdata.to(dev, torch.float32).contiguous()
+            u32 = torch.full_like(uh32, float("nan"))
+            it32 = torch.full((B,), -99, dtype=torch.int32, device=dev)
+            S.snap_project_f32(p, B, uh32, cd32, u32, it32, tol=1e-5)
+            nrm = torch.empty(B, 5, dtype=torch.float64, device=dev)
+            S.snap_residual(p, B, u32.double(), cd32.double(), None, nrm)
+            torch.cuda.synchronize()
+            assert (it32.cpu() > 0).all(), (tag, "f32 status", it32.cpu())
+            assert float(nrm[:, 0].max()) < 2e-5, (tag, "f32 feasibility", float(nrm[:, 0].max()))
+            err = float((u32.double().cpu() - u).abs().max()) / max(1e-300, float(u.abs().max()))
+            assert err <= 3e-4, (tag, "f32 vs f64", err)
+            one = torch.full_like(uh32[b:b + 1], float("nan"))
+            S.snap_project_f32(p, 1, uh32[b:b + 1].contiguous(), cd32[b:b + 1].contiguous(), one, it32[:1], tol=1e-5)
+            torch.cuda.synchronize()
+            assert torch.equal(one[0], u32[b]), (tag, "f32 alone")
         # one PCFM step = shoot (Eq. 1), projection, pull-back (Eq. 3) composed by hand
         g = torch.Generator().manual_seed(kw["seed"])
         tau, taun = 0.4, 0.5
